@@ -1,0 +1,357 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+CPU only.  Every expected value here comes from the paper's printed numbers (tests/golden/), a closed
+form, an invariant, an independent library routine (scipy ODE solver, numpy rolls / dense matrix) or
+brute force -- never from the oracle itself and never from the CUDA path.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import CHAOTIC, FREE, OSCILLON, QBALL, Oracle
+from paper_1201_5029_b200 import inputs
+
+from helpers import (DEFAULT_STENCIL, LD, SEVEN_POINT, composed_map, evolve_oscillator, laplacian_dense,
+                     laplacian_rolls, stencil_eigenvalue, weights)
+
+INF = math.inf
+
+
+# ---------------------------------------------------------------- P1: stage weights
+@pytest.mark.parametrize("order", [2, 4, 6, 8])
+def test_p1_order_conditions(order):
+    w = oracle.stage_weights(order)
+    assert len(w) == {2: 1, 4: 3, 6: 7, 8: 15}[order]
+    assert w == w[::-1]                                         # symmetric
+    assert abs(sum(w) - 1.0) < 4e-15                            # consistency
+    for p in range(3, order, 2):                                # sum w^3 = 0 (>=4), w^5 (>=6), w^7 (8)
+        assert abs(sum(x ** p for x in w)) < 2e-14, (order, p)
+
+
+@pytest.mark.parametrize("order", [6, 8])
+def test_p1_table1_values(order, golden_dir):
+    """The oracle's weights are the decimals printed in Table 1."""
+    want = [float(x) for x in weights(golden_dir, order)]
+    got = oracle.stage_weights(order)
+    assert np.allclose(got, want, rtol=0, atol=2e-16)
+
+
+def test_p1_yoshida_reading_g2():
+    """(2.44) as printed violates 2 z1 + z0 = 1; the corrected form satisfies both conditions."""
+    z1, z0, _ = oracle.stage_weights(4)
+    assert abs(2 * z1 + z0 - 1) < 1e-15 and abs(2 * z1 ** 3 + z0 ** 3) < 1e-14
+    assert abs(z1 - 1.3512071919596576) < 1e-15 and abs(z0 + 1.7024143839193153) < 1e-15
+    printed_z0 = -2 ** (1 / 3) / (2 - 2 ** (1 / 6))             # denominator as printed
+    assert abs(2 * z1 + printed_z0 - 1) > 0.2
+
+
+# ---------------------------------------------------------------- P2: homogeneous free field, static
+def _static_free(N, m2, order, dt, nf=1, stencil=(0, 0, 0, 0), L=5.0):
+    return Oracle(N, L, nf, FREE, [m2] * nf, order=order, dt=dt, mpl=INF, stencil=stencil)
+
+
+@pytest.mark.parametrize("order", [2, 4, 6])
+def test_p2_homogeneous_oscillator_closed_form(order, golden_dir):
+    N, m2, dt, n, q0 = 4, 1.7, 0.11, 40, 0.8
+    o = _static_free(N, m2, order, dt)
+    o.set_fields(np.full((1, N, N, N), q0), np.zeros((1, N, N, N)))
+    o.set_background(1.0, 0.0)
+    o.step(n)
+    phi, pi = o.read_fields()
+    assert np.ptp(phi) == 0.0 and np.ptp(pi) == 0.0             # D == 0 exactly in difference form
+    q, p = evolve_oscillator(m2, dt, weights(golden_dir, order), q0, 0.0, n)
+    assert abs(phi[0, 0, 0, 0] - q) < 5e-14 and abs(pi[0, 0, 0, 0] - p) < 5e-14
+    if order == 2:                                              # exact: q_n = q0 cos(n theta)
+        theta = math.acos(1 - m2 * dt * dt / 2)
+        assert abs(phi[0, 0, 0, 0] - q0 * math.cos(n * theta)) < 5e-14
+    # and the method converges to cos(m t) at its order
+    err = abs(phi[0, 0, 0, 0] - q0 * math.cos(math.sqrt(m2) * n * dt))
+    assert err < {2: 2e-2, 4: 2e-4, 6: 2e-6}[order]
+
+
+# ---------------------------------------------------------------- P3: single Fourier mode, dispersion
+MODES = [(1, 0, 0), (0, 1, 0), (0, 0, 1), (1, 1, 0), (1, 1, 1), (1, 2, 3), (4, 0, 0), (4, 4, 0), (4, 4, 4)]
+
+
+@pytest.mark.parametrize("stencil", [DEFAULT_STENCIL, SEVEN_POINT, (-4.0, 0.0, 1.0 / 3.0, 0.0)])
+@pytest.mark.parametrize("mode", MODES)
+def test_p3_plane_wave_eigenvalue(stencil, mode):
+    N = 8
+    z, y, x = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    wave = np.cos(2 * math.pi * (mode[0] * x + mode[1] * y + mode[2] * z) / N + 0.3)
+    o = _static_free(N, 0.0, 2, 0.1, stencil=stencil)
+    o.set_fields(wave[None], np.zeros((1, N, N, N)))
+    lam = stencil_eigenvalue(stencil, mode, N)
+    assert np.allclose(o.laplacian(0), lam * wave, rtol=0, atol=2e-14)
+
+
+def test_p3_default_stencil_extremes():
+    for mode, val in [((4, 0, 0), -4.0), ((4, 4, 0), -16.0 / 3.0), ((4, 4, 4), -92.0 / 15.0)]:
+        assert abs(stencil_eigenvalue(DEFAULT_STENCIL, mode, 8) - val) < 1e-14
+
+
+@pytest.mark.parametrize("order", [2, 4])
+def test_p3_mode_follows_lattice_dispersion(order, golden_dir):
+    """A plane wave in a static background is an oscillator with w^2 = k_eff^2/dx^2 + m^2 (P3)."""
+    N, L, m2, dt, n, mode = 8, 5.0, 0.5, 0.02, 25, (1, 2, 3)
+    dx = L / N
+    z, y, x = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    wave = np.cos(2 * math.pi * (mode[0] * x + mode[1] * y + mode[2] * z) / N)
+    o = _static_free(N, m2, order, dt, L=L)
+    o.set_fields(0.3 * wave[None], np.zeros((1, N, N, N)))
+    o.set_background(1.0, 0.0)
+    o.step(n)
+    phi, pi = o.read_fields()
+    w2 = -stencil_eigenvalue(DEFAULT_STENCIL, mode, N) / dx ** 2 + m2
+    q, p = evolve_oscillator(w2, dt, weights(golden_dir, order), 0.3, 0.0, n)
+    assert np.allclose(phi[0], q * wave, rtol=0, atol=1e-13)
+    assert np.allclose(pi[0], p * wave, rtol=0, atol=1e-12)
+
+
+# ---------------------------------------------------------------- P10 / P7: brute force, identity (2.17)
+@pytest.mark.parametrize("N", [3, 4, 5])
+def test_p10_dense_matrix_bruteforce(N):
+    rng = np.random.default_rng(10 + N)
+    phi = rng.standard_normal((1, N, N, N))
+    o = _static_free(N, 0.0, 2, 0.1)
+    o.set_fields(phi, np.zeros_like(phi))
+    A = laplacian_dense(N, DEFAULT_STENCIL)
+    want = (A @ phi[0].ravel()).reshape(N, N, N)
+    assert np.allclose(o.laplacian(0), want, rtol=0, atol=5e-14)
+    assert np.allclose(laplacian_rolls(phi[0], DEFAULT_STENCIL), want, rtol=0, atol=5e-14)
+
+
+def test_p7_sum_phi_D_phi_equals_minus_sum_G():
+    N = 7
+    phi, pi = inputs.random_fields(N, 2, seed=7, mean=0.4)
+    o = Oracle(N, 3.0, 2, FREE, [1.0, 2.0], order=2, dt=0.1, mpl=INF)
+    o.set_fields(phi, pi)
+    for f in range(2):
+        D, G = o.laplacian(f), o.gradient_energy(f)
+        assert np.all(G >= 0)
+        assert abs(np.sum(phi[f] * D) + np.sum(G)) < 1e-11 * np.sum(G)          # (2.17)
+        # G from its definition (2.8) with rolls
+        want = np.zeros((N, N, N))
+        for dz in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for dx in (-1, 0, 1):
+                    d = (dx != 0) + (dy != 0) + (dz != 0)
+                    want += 0.5 * DEFAULT_STENCIL[d] * (np.roll(phi[f], (-dz, -dy, -dx), (0, 1, 2)) - phi[f]) ** 2
+        assert np.allclose(G, want, rtol=1e-13, atol=0)
+    e = o.energies()
+    assert abs(e.grad[0] - e.sum_phiDphi[0]) < 1e-12 * e.grad[0]
+
+
+# ---------------------------------------------------------------- P11: dV/dphi vs finite differences
+@pytest.mark.parametrize("model,nf,p,pt", [
+    (FREE, 2, (1.3, 0.7), (0.4, -1.1)),
+    (CHAOTIC, 2, (1.0, 1.0e4), (0.97, 3.0e-3)),
+    (OSCILLON, 1, (1.0, 1.0, 0.3), (1.7,)),
+    (QBALL, 2, (1.0, -0.1, 1.0, 0.5), (1.2, -0.6)),
+])
+def test_p11_potential_derivative(model, nf, p, pt):
+    o = Oracle(4, 1.0, nf, model, p, order=2, dt=0.1, mpl=2.0)
+    V0, dV = o.potential(pt)
+    for f in range(nf):
+        h = 1e-5 * max(1.0, abs(pt[f]))
+        up, dn = list(pt), list(pt)
+        up[f] += h
+        dn[f] -= h
+        fd = (o.potential(up)[0] - o.potential(dn)[0]) / (2 * h)
+        assert abs(fd - dV[f]) < 2e-8 * max(1.0, abs(dV[f]))
+
+
+def test_p11_potential_values():
+    """V itself against the formulas printed in the paper (3.2)-(3.4) evaluated by hand here."""
+    o = Oracle(4, 1.0, 2, CHAOTIC, (2.0, 3.0), order=2, dt=0.1, mpl=1.0)
+    assert abs(o.potential((0.5, 0.25))[0] - (0.5 * 2.0 * 0.25 + 0.5 * 3.0 * 0.25 * 0.0625)) < 1e-15
+    o = Oracle(4, 1.0, 1, OSCILLON, (1.0, 1.0, 0.3), order=2, dt=0.1, mpl=1.0)
+    assert abs(o.potential((2.0,))[0] - (2.0 - 4.0 + 0.3 * 64 / 6)) < 1e-14
+    o = Oracle(4, 1.0, 2, QBALL, (1.0, -0.1, 1.0, 0.0), order=2, dt=0.1, mpl=1.0)
+    r2 = (1.2 ** 2 + 0.6 ** 2) / 2                               # |Phi|^2 with Phi = (phi1 + i phi2)/sqrt2 (G7)
+    assert abs(o.potential((1.2, -0.6))[0] - r2 * (1 - 0.1 * math.log(r2))) < 1e-15
+    assert o.potential((0.0, 0.0))[0] == 0.0                     # G8: r^2 ln r^2 -> 0
+
+
+# ---------------------------------------------------------------- P8: homogeneous radiation / matter
+def test_p8_radiation_only_linear_a():
+    N, mpl, rg = 3, 1.5, 3.0
+    o = Oracle(N, 1.0, 1, FREE, [0.0], order=4, dt=0.05, mpl=mpl, rho_gamma0=rg)
+    o.set_fields(np.zeros((1, N, N, N)), np.zeros((1, N, N, N)))
+    o.set_background(1.0)                                        # p_a from (2.18)
+    pa0 = o.energies().p_a
+    assert abs(pa0 + 6 * N ** 3 * mpl ** 2 * math.sqrt(rg / 3) / mpl) < 1e-12 * abs(pa0)   # (2.11),(2.18)
+    o.step(20)
+    e = o.energies()
+    assert abs(e.a - (1 + 1.0 * math.sqrt(rg / 3) / mpl)) < 1e-14   # radiation drops out
+    assert e.p_a == pa0 and e.residual < 1e-14
+
+
+def test_p8_matter_only_quadratic_a():
+    N, mpl, rm = 3, 0.8, 2.0
+    o = Oracle(N, 1.0, 1, FREE, [0.0], order=2, dt=0.1, mpl=mpl, rho_m0=rm)
+    o.set_fields(np.zeros((1, N, N, N)), np.zeros((1, N, N, N)))
+    o.set_background(1.0)
+    ap0 = math.sqrt(rm / 3) / mpl
+    o.step(10)
+    eta = 1.0
+    e = o.energies()
+    assert abs(e.a - (1 + ap0 * eta + rm * eta ** 2 / (12 * mpl ** 2))) < 1e-14   # p_a' = -V_L rho_m0
+    assert e.residual < 1e-13                                    # a'^2 = a rho_m0/(3 mpl^2) holds exactly
+
+
+# ---------------------------------------------------------------- P9: homogeneous FRW + field vs ODE solver
+def test_p9_homogeneous_frw_against_ode_solver():
+    from scipy.integrate import solve_ivp
+    N, mpl, m2, q0, v0, T = 3, 2.0, 1.3, 1.0, -0.4, 1.0
+
+    def rhs(_, y):
+        # Textbook FRW in conformal time: a'' = +a^3 (rho - 3P)/(6 mpl^2), phi'' + 2 (a'/a) phi' + a^2 V' = 0.
+        # (2.19) prints a minus sign; that contradicts the paper's own (2.14) and its matter case
+        # (a'' = rho_m0/(6 mpl^2) > 0) -- reading G20 in DESIGN.md.
+        a, ap, q, v = y
+        rho_minus_3P = -v * v / (a * a) + 4 * 0.5 * m2 * q * q
+        return [ap, a ** 3 / (6 * mpl ** 2) * rho_minus_3P, v, -2 * ap / a * v - a * a * m2 * q]
+
+    rho0 = 0.5 * v0 * v0 + 0.5 * m2 * q0 * q0
+    sol = solve_ivp(rhs, (0, T), [1.0, math.sqrt(rho0 / 3) / mpl, q0, v0], method="DOP853", rtol=1e-13, atol=1e-15)
+    a_T, ap_T, q_T, v_T = sol.y[:, -1]
+    o = Oracle(N, 4.0, 1, FREE, [m2], order=6, dt=0.01, mpl=mpl)
+    o.set_fields(np.full((1, N, N, N), q0), np.full((1, N, N, N), v0))    # pi = a^2 phi' with a = 1
+    o.set_background(1.0)
+    o.step(100)
+    e = o.energies()
+    phi, pi = o.read_fields()
+    assert abs(e.a - a_T) < 1e-10 and abs(phi[0, 0, 0, 0] - q_T) < 1e-10
+    assert abs(pi[0, 0, 0, 0] - a_T ** 2 * v_T) < 1e-10          # (2.12)
+    assert abs(-e.p_a / (6 * N ** 3 * mpl ** 2) - ap_T) < 1e-10  # (2.11)
+    assert e.residual < 1e-10
+
+
+# ---------------------------------------------------------------- P4-P6: whole non-linear step
+def _small_chaotic(order, dt, precision=64, N=6, g2=25.0, seed=4):
+    phi, pi = inputs.random_fields(N, 2, seed=seed, amp=0.05)
+    phi[0] += 1.0
+    pi[0] -= 0.7
+    o = Oracle(N, 7.5, 2, CHAOTIC, (1.0, g2), order=order, dt=dt, mpl=1.0, precision=precision)
+    o.set_fields(phi, pi)
+    o.set_background(1.0)
+    return o, phi, pi
+
+
+@pytest.mark.parametrize("order", [2, 4, 6])
+def test_p4_convergence_order(order):
+    T = 0.64
+    ref, _, _ = _small_chaotic(6, T / 512, precision=80)
+    ref.step(512)
+    rphi, rpi = ref.read_fields()
+    ra = ref.energies().a
+    errs = []
+    for n in (8, 16, 32):
+        o, _, _ = _small_chaotic(order, T / n, precision=80)
+        o.step(n)
+        phi, pi = o.read_fields()
+        errs.append(max(np.max(np.abs(phi - rphi)), np.max(np.abs(pi - rpi)), abs(o.energies().a - ra)))
+    slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert all(order - 0.35 < s < order + 0.9 for s in slopes), (errs, slopes)
+
+
+@pytest.mark.parametrize("order", [2, 4, 6])
+def test_p5_time_reversibility(order):
+    o, phi0, pi0 = _small_chaotic(order, 0.02)
+    e0 = o.energies()
+    o.step(25)
+    mid = o.read_fields()[0]
+    assert np.max(np.abs(mid - phi0)) > 1e-2                     # it really moved
+    o.set_dt(-0.02)
+    o.step(25)
+    phi, pi = o.read_fields()
+    e = o.energies()
+    assert np.max(np.abs(phi - phi0)) < 2e-13 and np.max(np.abs(pi - pi0)) < 2e-13
+    assert abs(e.a - e0.a) < 1e-13 and abs(e.p_a - e0.p_a) < 1e-12 * abs(e0.p_a)
+
+
+@pytest.mark.parametrize("order", [2, 4])
+def test_p6_friedmann_residual(order):
+    res = []
+    for n in (16, 32):
+        o, _, _ = _small_chaotic(order, 0.64 / n)
+        assert o.energies().residual < 1e-14                     # G10: starts on the constraint
+        worst = 0.0
+        for _ in range(4):
+            o.step(n // 4)
+            worst = max(worst, o.energies().residual)
+        res.append(worst)
+    assert res[0] < 1e-2 and math.log2(res[0] / res[1]) > order - 0.5, res
+
+
+def test_p12_matter_like_stage():
+    """An oscillating massive field averages to matter: a^(-3/2) H^(-1) is roughly constant."""
+    N = 3
+    o = Oracle(N, 1.0, 1, FREE, [1.0], order=4, dt=0.02, mpl=1.0)
+    o.set_fields(np.full((1, N, N, N), 0.3), np.zeros((1, N, N, N)))
+    o.set_background(1.0)
+    vals = []
+    for _ in range(20):                                          # to eta = 40: a m dt stays < 0.3 (fixed d eta)
+        o.step(100)
+        e = o.energies()
+        vals.append(e.a ** -1.5 / e.hubble)
+    tail = np.array(vals[5:])
+    assert tail.std() / tail.mean() < 0.02 and o.energies().a > 5.0
+
+
+# ---------------------------------------------------------------- P13: linear stability edges
+@pytest.mark.parametrize("order", [2, 4, 6])
+def test_p13_linear_stability_edge(order, golden_dir):
+    ws = weights(golden_dir, order)
+    # edge from the trace of the composed 2x2 map (|tr| = 2), by bisection on w dt
+    lo, hi = 0.5, 3.0
+    xs = np.linspace(lo, hi, 2501)
+    unstable = [x for x in xs if abs(float(np.trace(composed_map(1.0, x, ws)))) > 2.0]
+    edge = unstable[0]
+    assert abs(edge - {2: 2.0, 4: 1.5737, 6: 2.2696}[order]) < 2e-3
+    N = 3
+    for dt, bounded in ((edge - 0.02, True), (edge + 0.02, False)):
+        o = _static_free(N, 1.0, order, dt)
+        o.set_fields(np.full((1, N, N, N), 1.0), np.zeros((1, N, N, N)))
+        o.set_background(1.0, 0.0)
+        o.step(400)
+        amp = np.max(np.abs(o.read_fields()[0]))
+        assert (amp < 1e2) if bounded else (amp > 1e4), (order, dt, amp)
+
+
+# ---------------------------------------------------------------- ABI behaviour
+def test_abi_errors_and_state():
+    with pytest.raises(oracle.OracleError):
+        Oracle(2, 1.0, 1, FREE, [1.0])                           # N < 3
+    with pytest.raises(oracle.OracleError):
+        Oracle(4, 1.0, 1, CHAOTIC, [1.0, 1.0])                   # chaotic needs 2 fields
+    with pytest.raises(oracle.OracleError):
+        Oracle(4, 1.0, 1, FREE, [1.0], order=5)
+    with pytest.raises(oracle.OracleError):
+        Oracle(4, 1.0, 1, FREE, [1.0], stencil=(-5.0, 1.0, 0.0, 0.0))   # does not annihilate constants
+    o = Oracle(4, 1.0, 1, FREE, [1.0], mpl=INF)
+    with pytest.raises(oracle.OracleError) as ei:
+        o.step(1)
+    assert ei.value.code == oracle.ESTATE
+
+
+def test_fp32_state_fp64_sums():
+    """Reading G16: float fields, double scalars -- one step stays within float rounding of the fp64 run."""
+    N = 6
+    phi, pi = inputs.random_fields(N, 2, seed=3, amp=0.05)
+    phi[0] += 1.0
+    outs = []
+    for prec in (64, 32):
+        o = Oracle(N, 7.5, 2, CHAOTIC, (1.0, 25.0), order=4, dt=0.02, mpl=1.0, precision=prec)
+        o.set_fields(phi.astype(np.float32), pi.astype(np.float32))
+        o.set_background(1.0)
+        o.step(3)
+        outs.append((o.read_fields(), o.energies()))
+    (p64, q64), e64 = outs[0]
+    (p32, q32), e32 = outs[1]
+    assert p32.dtype == np.float32
+    assert np.max(np.abs(p32 - p64)) < 2e-6 and np.max(np.abs(q32 - q64)) < 2e-6
+    assert abs(e32.a - e64.a) < 1e-7
