@@ -1,0 +1,281 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the symplectic lattice step (arXiv 1201.5029 §2.3) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4_chaotic512] [--order 4]
+                    [--precision 64] [--impl ours|reference]
+
+One "step" is one whole composite step of the chosen order (all stages: merged drift + kick + lattice sums +
+scalar update) over the whole lattice.  The metric is BASELINE.json's: lattice
+site-updates per second per field, SU/s = N^3 * nfields * steps / time.  One JSON line on stdout (rank 0).
+
+  value     inputs resident in HBM; CUDA events on the launching stream around K steps (one pycool_step(K)).
+  e2e       same job from pinned HOST buffers to HOST buffers through the public API: set_fields (H2D), K steps,
+            energies, read_fields (D2H), all inside the timed region.
+  roofline  the fused drift+kick kernel: algorithmic bytes per launch (4 * sizeof(real) per field-site)
+            / its average duration, bracketed per launch by CUDA events inside the same timed region.
+  cpu_baseline  the CPU oracle, as it stands, on a bounded sub-lattice of the same workload (1 thread).
+--impl reference times that oracle alone (there is no reference implementation to install: the paper ships no
+code).  Multi-GPU: the path does not shard (north_star: one GPU); --gpus N runs N
+independent replicas, one per rank ("replicas only", weak scaling, no collective on the data path).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "lattice site-updates/sec (fp64, per field)"
+UNIT = "site-updates/s"
+ORACLE_SAMPLE_N = 64          # sub-lattice the oracle is timed on (same dx, dt, model, order)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4_chaotic512")
+    ap.add_argument("--order", type=int, default=None)
+    ap.add_argument("--precision", type=int, default=64, choices=[32, 64])
+    ap.add_argument("--tile", type=int, default=-1)
+    ap.add_argument("--zchunk", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def recorded_traffic(key):
+    """DRAM bytes per launch of the fused kernel from the committed ncu --set full capture, if any."""
+    p = os.path.join(ROOT, "profiles", "kick_traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(key)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        busy = [x for x in sm if mx and x > 0.5 * mx] or sm
+        med = busy[len(busy) // 2] if busy else None
+        return {"sm_mhz": med, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle(cfg, order, steps, warmup, precision):
+    """The oracle on an ORACLE_SAMPLE_N^3 sub-lattice with the workload's dx, dt, model and order."""
+    import oracle
+    from paper_1201_5029_b200 import inputs
+    n = min(ORACLE_SAMPLE_N, cfg["N"])
+    sub = dict(cfg)
+    sub["N"], sub["L"] = n, cfg["L"] * n / cfg["N"]
+    phi, pi = inputs.make_initial(sub, precision=precision, fft_max=n)
+    o = oracle.Oracle(n, sub["L"], sub["nfields"], sub["model"], sub["p"], order=order, dt=cfg["dt"],
+                      mpl=sub["mpl"], rho_gamma0=sub["rho_gamma0"], rho_m0=sub["rho_m0"], precision=precision)
+    o.set_fields(phi, pi)
+    o.set_background(1.0)
+    o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    units = float(n) ** 3 * sub["nfields"] * steps
+    sample = "%d^3 sub-lattice of %s (same dx, dt, model, order %d), %d steps, %.1f s" % (n, cfg["name"], order, steps, dt)
+    return units / dt, dt / steps * 1e3, sample
+
+
+def main():
+    a = parse()
+    from paper_1201_5029_b200 import inputs
+    cfg = inputs.config(a.workload)
+    cfg["name"] = a.workload
+    order = a.order or cfg["order"]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    N, nf = cfg["N"], cfg["nfields"]
+    config = {"workload": "%s: %d^3 x %d fields, model %d, order %d, dt=%g, %d-bit" %
+              (a.workload, N, nf, cfg["model"], order, cfg["dt"], a.precision),
+              "l2": "inputs larger than L2 (state %.1f GiB vs 126 MB)" % (2 * nf * N ** 3 * (a.precision // 8) / 2 ** 30),
+              "parallelism": "replicas only" if a.gpus > 1 else "single GPU"}
+
+    if a.impl == "reference":
+        if rank != 0:
+            return 0
+        osteps = max(1, min(a.steps, 50))
+        v, ms, sample = time_oracle(cfg, order, osteps, min(a.warmup, 1), a.precision)
+        line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+                "warmup": a.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f%d" % a.precision, "data": "synthetic", "config": config,
+                "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    from paper_1201_5029_b200 import binding, build
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    phi, pi = inputs.make_initial(cfg, precision=a.precision)
+    tdt = torch.float32 if a.precision == 32 else torch.float64
+    h_phi = torch.from_numpy(phi).pin_memory()
+    h_pi = torch.from_numpy(pi).pin_memory()
+    del phi, pi
+    lat = binding.from_config(cfg, device=dev, order=order, precision=a.precision)
+    if a.tile >= 0:
+        lat.set_tile(a.tile)
+    if a.zchunk > 0:
+        lat.set_zchunk(a.zchunk)
+    lat.set_fields(h_phi, h_pi)
+    lat.set_background(1.0)
+    lat.step(a.warmup)
+    lat.sync()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing, kernel brackets live in the same region
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    c0 = lat.launch_counts()
+    lat.set_profiling(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(lat.stream)
+    lat.step(a.steps)
+    ev1.record(lat.stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    kick_ms, kick_n = lat.kick_time_ms()
+    lat.set_profiling(False)
+    c1 = lat.launch_counts()
+    clocks = sampler.stop() if rank == 0 else None
+    lat.sync()
+    launches = sum(c1) - sum(c0)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    units = float(N) ** 3 * nf * a.steps * world
+    value = units / (ms * 1e-3)
+
+    # ---- end to end: host buffers -> host buffers
+    e2e = None
+    if not a.no_e2e:
+        esz = a.precision // 8
+        barrier()
+        t0 = time.perf_counter()
+        lat.set_fields(h_phi, h_pi)
+        lat.set_background(1.0)
+        lat.step(a.steps)
+        en = lat.energies()
+        lat.read_fields(h_phi, h_pi)
+        barrier()
+        te = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([te], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            te = float(t.item())
+        e2e = {"value": units / te, "unit": UNIT, "h2d_bytes_per_step": 2 * nf * N ** 3 * esz / a.steps,
+               "d2h_bytes_per_step": (2 * nf * N ** 3 * esz + 208) / a.steps,
+               "what": "set_fields(H2D) + set_background + %d steps + energies + read_fields(D2H), pinned host buffers, "
+                       "wall clock; bytes are per step of the %d-step job" % (a.steps, a.steps),
+               "a_final": en.a}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = measured_peaks()
+    esz = a.precision // 8
+    alg_bytes = 4.0 * esz * N ** 3 * nf                       # read phi, pi; write phi, pi
+    kick_avg_ms = kick_ms / max(kick_n, 1)
+    achieved = alg_bytes / (kick_avg_ms * 1e-3) / 1e9
+    geo = lat.kick_geometry()
+    roof = {"bound": "hbm", "kernel": "kick_fused", "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak, "peak_source": peak_src,
+            "traffic": recorded_traffic("%s/order%d/fp%d" % (a.workload, order, a.precision)),
+            "algorithmic_bytes_per_launch": alg_bytes, "launches_timed": kick_n, "avg_launch_ms": kick_avg_ms,
+            "kernel_share_of_step": kick_ms / ms, "geometry": geo}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f%d" % a.precision, "data": "synthetic", "config": config, "clocks": clocks,
+            "gpu_launches": launches, "roofline": roof}
+    if e2e:
+        line["e2e"] = e2e
+    if not a.no_cpu_baseline and world == 1:
+        stages = {2: 1, 4: 3, 6: 7, 8: 15}[order]
+        v, _, sample = time_oracle(cfg, order, max(1, round(36 / stages)), 1, a.precision)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,172 @@
+/*
+ * pycool.h -- C ABI of libpycool.so: the non-linear symplectic lattice step of PyCOOL
+ *             (J. Sainio, arXiv 1201.5029, §2.1-2.4) as hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * What the library evolves (eq. (2.47)): the state (a, p_a, phi_{f,x}, pi_{f,x}) of nf real
+ * scalar fields phi_f and their conjugate momenta pi_f = a^2 phi_f' (2.12) on a periodic N^3 lattice of side
+ * L (dx = L/N, V_L = N^3), coupled to the scale factor a and its momentum p_a = -6 a' V_L mpl^2 (2.11) of a
+ * flat FRW background, in conformal time eta.  One step of length dt is the composition
+ *     step = Phi2(w_1 dt) ... Phi2(w_s dt)                          (2.43)-(2.45), Table 1
+ *     Phi2(h) = H1(h/2) H2(h/2) H3(h) H2(h/2) H1(h/2)               (2.48)
+ *     H1(e): a   -= p_a/(6 V_L mpl^2) e                              (2.47)
+ *     H2(e): p_a += (sum_{f,x} pi^2/a^3 - V_L rho_m0) e;  phi_f += pi_f/a^2 e          "drift"
+ *     H3(e): p_a += (a sum phi D[phi]/dx^2 - 4 a^3 sum V) e;
+ *            pi_f += (a^2 D[phi_f]/dx^2 - a^4 dV/dphi_f) e                             "kick"
+ * with D the 27-point periodic Laplacian stencil (2.7) and the lattice-wide sums computed
+ * on the device in a fixed order.  Energies follow (2.16)-(2.20), the residual (3.1).
+ *
+ * Conventions for every entry point
+ *   - returns a status (enum below); never throws, aborts or exits; no CPU fallback exists: without a usable
+ *     CUDA device pycool_create returns PYCOOL_ECUDA.
+ *   - "host" pointers are caller-owned host memory, read or written only during the call;
+ *     "device" pointers are caller-owned CUDA device memory that must stay valid for the life of the context.
+ *   - field buffers hold nf*N^3 elements in layout [field][z][y][x] (x fastest); element type is double when
+ *     params.precision is 64 (or 0), float when it is 32.  Scalars, sums and energies are always double
+ *     (reading G16).
+ *   - work is enqueued on the context's CUDA stream; calls that return data synchronise that stream first.
+ *   - a context is not thread-safe; distinct contexts are independent.
+ */
+#ifndef PYCOOL_H
+#define PYCOOL_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default) /* the library is built with -fvisibility=hidden: only this ABI is exported */
+#endif
+
+typedef struct pycool_ctx pycool_ctx; /* opaque; created by pycool_create*, released by pycool_destroy */
+
+enum {
+  PYCOOL_OK = 0,
+  PYCOOL_EINVAL = 1,     /* bad argument; pycool_last_error says which                                   */
+  PYCOOL_ENOMEM = 2,     /* host or device allocation failed                                             */
+  PYCOOL_ECUDA = 3,      /* CUDA runtime error (no device, launch failure, ...)                          */
+  PYCOOL_ESTATE = 4,     /* call order: e.g. step before set_fields                                      */
+  PYCOOL_ENONFINITE = 5  /* a lattice sum became NaN/Inf; sticky until the next set_fields               */
+};
+
+/* Potentials V(phi_1..phi_nf); the derivative dV/dphi_f is compiled in per model (C++ template instance),
+ * replacing the paper's run-time code generation. */
+enum {
+  PYCOOL_FREE = 0,     /* V = sum_f 1/2 m_f^2 phi_f^2                 p = {m_1^2, .., m_nf^2}; nf = 1..4      */
+  PYCOOL_CHAOTIC = 1,  /* (3.2) PAPER.md:427: 1/2 m^2 phi^2 + 1/2 g^2 phi^2 chi^2   p = {m^2, g^2}; nf = 2   */
+  PYCOOL_OSCILLON = 2, /* (3.3) PAPER.md:456: 1/2 m^2 phi^2 - lambda/4 phi^4 + g6/6 phi^6
+                                                                      p = {m^2, lambda, g6}; nf = 1           */
+  PYCOOL_QBALL = 3     /* (3.4) PAPER.md:481: m^2 r2 (1 + K ln(r2/M^2)) + lambda6 r2^3/mpl^2,
+                          r2 = |Phi|^2 = (phi_1^2+phi_2^2)/2 (reading G7); the log term is 0 for r2 < DBL_MIN
+                          (G8)                                        p = {m^2, K, M^2, lambda6}; nf = 2      */
+};
+
+typedef struct {
+  int model;         /* enum above                                                                        */
+  double p[8];       /* model parameters, see enum                                                        */
+  double mpl;        /* reduced Planck mass in program units; +INF = static background     */
+  double rho_gamma0; /* homogeneous radiation density of (2.20); enters rho only      */
+  double rho_m0;     /* homogeneous matter density of (2.20); enters rho and p_a'                         */
+  double stencil[4]; /* c_0..c_3 of (2.7) by neighbour class (centre, face, edge, corner).  All zero selects
+                        (-128, 14, 3, 1)/30 (reading G1: the paper does not print them).  Must satisfy
+                        c_0 = -(6 c_1 + 12 c_2 + 8 c_3), else PYCOOL_EINVAL                               */
+  int precision;     /* 64 (also 0) or 32: element type of the field arrays                               */
+} pycool_params;
+
+/* Lattice averages at the current (time-synchronised) state.  Always double. */
+typedef struct {
+  double a, p_a, eta;
+  double kin[4];         /* K_f  = sum_x pi_f^2 / (2 a^6 V_L)          first term of (2.16)   */
+  double grad[4];        /* Gr_f = sum_x G[phi_f] / (2 a^2 dx^2 V_L)   (2.8) PAPER.md:92                     */
+  double pot;            /* <V>                                                                              */
+  double rho, pressure;  /* (2.16) plus rho_gamma0/a^4 (+ /3 in P) and rho_m0/a^3 of (2.20)                  */
+  double hubble;         /* H = a'/a^2 with a' = -p_a/(6 V_L mpl^2)    (2.14) PAPER.md:123                   */
+  double residual;       /* |rho/(3 mpl^2 H^2) - 1|                    (3.1) PAPER.md:415-419; 0 if static   */
+  double sum_phiDphi[4]; /* -sum_x phi_f D[phi_f] / (2 a^2 dx^2 V_L); equals grad[f] by (2.17) PAPER.md:146  */
+} pycool_energy;
+
+/* Create a context that owns its device memory (2 x the state for ping-pong, plus partial sums) and its own
+ * stream.  N >= 3 sites per side; L > 0; nfields 1..4 consistent with the model; order in {2,4,6,8}
+ * (stages 1/3/7/15: (2.42), triple jump (2.43)-(2.44) with reading G2, Table 1); dt finite and non-zero
+ * (negative runs backwards).  Initial state: a = 1, p_a = 0, eta = 0, no fields.  *out is NULL on failure. */
+int pycool_create(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
+                  double dt);
+
+/* Bytes of device work memory pycool_create_ext needs for this lattice (0 if the arguments are invalid). */
+size_t pycool_work_bytes(int N, int nfields, int precision);
+
+/* As pycool_create, on caller-owned device memory and stream (e.g. PyTorch tensors / torch stream):
+ *   d_phi, d_pi : device, nf*N^3 elements each; the library reads and writes them (state buffer 0)
+ *   d_work      : device, >= pycool_work_bytes(...) bytes, 256-byte aligned; state buffer 1, partial sums,
+ *                 scalars
+ *   cuda_stream : a cudaStream_t (NULL = the legacy default stream)
+ * The caller keeps ownership; pycool_destroy frees none of them. */
+int pycool_create_ext(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
+                      double dt, void* d_phi, void* d_pi, void* d_work, size_t work_bytes, void* cuda_stream);
+
+/* Upload phi and pi from host memory (H2D on the context stream, synchronous to the caller) and compute
+ * sum pi^2 on the device.  Clears PYCOOL_ENONFINITE. */
+int pycool_set_fields(pycool_ctx*, const void* phi_host, const void* pi_host);
+/* Same from device memory (D2D on the context stream, asynchronous). */
+int pycool_set_fields_device(pycool_ctx*, const void* d_phi_src, const void* d_pi_src);
+
+/* Set a (> 0) and p_a.  p_a = NaN asks the library to solve the first Friedmann equation (2.18) on the
+ * current lattice, expanding branch (reading G10): p_a = -6 V_L mpl a^2 sqrt(rho/3); needs fields and a
+ * finite mpl.  With mpl = +INF pass p_a = 0. */
+int pycool_set_background(pycool_ctx*, double a, double p_a);
+
+int pycool_set_dt(pycool_ctx*, double dt);
+
+/* Advance nsteps >= 0 whole steps of length dt.  Asynchronous: kernels are enqueued on the context stream
+ * (no host synchronisation inside, a and p_a live on the device).  On return from a later synchronising call
+ * the state is time-synchronised at eta + nsteps*dt.  Returns PYCOOL_ENONFINITE if an EARLIER call left the
+ * sticky flag set and it has been observed by a synchronising call. */
+int pycool_step(pycool_ctx*, int nsteps);
+
+/* Wait for the context stream; returns PYCOOL_ENONFINITE / PYCOOL_ECUDA if the enqueued work failed. */
+int pycool_sync(pycool_ctx*);
+
+/* Download phi and/or pi (either may be NULL) to host memory.  Synchronises. */
+int pycool_read_fields(pycool_ctx*, void* phi_host, void* pi_host);
+
+/* Device pointers of the current state arrays (they alternate between the two state buffers); valid until
+ * the next pycool_step/set_fields.  Does not synchronise. */
+int pycool_device_fields(pycool_ctx*, void** d_phi, void** d_pi);
+
+/* Lattice sums of the current state (one stencil pass with G of (2.8)) -> rho, P, H, residual.
+ * Synchronises. */
+int pycool_energies(pycool_ctx*, pycool_energy* out);
+
+int pycool_destroy(pycool_ctx*);
+
+/* Library-owned, NUL-terminated description of the last error of this context (valid until the next call
+ * on it); a static string for ctx == NULL. */
+const char* pycool_last_error(const pycool_ctx*);
+
+/* Stage weights w_1..w_s of one step of the given order into w[cap]; returns s, or 0 if order is not
+ * supported or cap < s.  (2.42)-(2.45), Table 1. */
+int pycool_stage_weights(int order, double* w, int cap);
+
+/* ---- instrumentation (does not change results) ---- */
+/* Number of kernels this context has launched so far, by kind:
+ *   counts[0] fused drift+kick, [1] reduce+scalar update, [2] closing drift, [3] energy/sum kernels. */
+int pycool_launch_counts(const pycool_ctx*, unsigned long long counts[4]);
+/* profiling on: bracket every fused drift+kick launch with CUDA events on the context stream. */
+int pycool_set_profiling(pycool_ctx*, int on);
+/* Sum of the bracketed durations (ms) and their number since profiling was switched on.  Synchronises. */
+int pycool_kick_time_ms(pycool_ctx*, double* total_ms, unsigned long long* launches);
+/* Launch geometry of the fused kernel: tile[0..2] = TX, TY, z-chunk; tile[3] = threads per block;
+ * tile[4] = blocks per launch; tile[5] = dynamic shared memory bytes. */
+int pycool_kick_geometry(const pycool_ctx*, int tile[6]);
+/* Override the z-chunk length (planes per block; 0 = automatic) before the next step. */
+int pycool_set_zchunk(pycool_ctx*, int planes);
+/* Select the x-y tile variant of the fused kernel: 0 = 32x8, 1 = 32x16, 2 = 64x16 sites; -1 = automatic. */
+int pycool_set_tile(pycool_ctx*, int tile);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYCOOL_H */

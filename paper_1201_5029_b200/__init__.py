@@ -9,7 +9,9 @@ from . import inputs  # noqa: F401
 
 
 def __getattr__(name):  # lazy: importing the package (e.g. for `inputs`) must not need the CUDA library
-    if name in ("Lattice", "PycoolError", "lib", "binding", "stage_weights", "work_bytes"):
-        from . import binding
-        return binding if name == "binding" else getattr(binding, name)
+    import importlib
+    if name in ("binding", "build"):
+        return importlib.import_module(__name__ + "." + name)
+    if name in ("Lattice", "PycoolError", "lib", "stage_weights", "work_bytes", "from_config"):
+        return getattr(importlib.import_module(__name__ + ".binding"), name)
     raise AttributeError(name)

@@ -1,0 +1,261 @@
+"""Thin Python binding of libpycool.so (include/pycool.h): argument marshalling only.
+
+PyTorch supplies device memory (the state and work buffers are torch tensors handed to
+`pycool_create_ext`) and the CUDA stream; every step of the path runs in the library's sm_100a kernels.
+There is no fallback: if the library is missing or no CUDA device is present, calls raise.
+"""
+import ctypes as C
+import math
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpycool.so")
+
+FREE, CHAOTIC, OSCILLON, QBALL = 0, 1, 2, 3
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = 0, 1, 2, 3, 4, 5
+
+# every symbol include/pycool.h declares (tests check the library exports exactly these)
+SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_set_fields",
+           "pycool_set_fields_device", "pycool_set_background", "pycool_set_dt", "pycool_step", "pycool_sync",
+           "pycool_read_fields", "pycool_device_fields", "pycool_energies", "pycool_destroy",
+           "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
+           "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile")
+
+
+class Params(C.Structure):
+    _fields_ = [("model", C.c_int), ("p", C.c_double * 8), ("mpl", C.c_double),
+                ("rho_gamma0", C.c_double), ("rho_m0", C.c_double), ("stencil", C.c_double * 4),
+                ("precision", C.c_int)]
+
+
+class Energy(C.Structure):
+    _fields_ = [("a", C.c_double), ("p_a", C.c_double), ("eta", C.c_double), ("kin", C.c_double * 4),
+                ("grad", C.c_double * 4), ("pot", C.c_double), ("rho", C.c_double),
+                ("pressure", C.c_double), ("hubble", C.c_double), ("residual", C.c_double),
+                ("sum_phiDphi", C.c_double * 4)]
+
+    def asdict(self):
+        d = {}
+        for name, _ in self._fields_:
+            v = getattr(self, name)
+            d[name] = list(v) if hasattr(v, "__len__") else v
+        return d
+
+
+class PycoolError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("pycool status %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libpycool.so (built in-tree by `python -m paper_1201_5029_b200.build`).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libpycool.so is not built: run `python -m paper_1201_5029_b200.build` "
+                               "(there is no CPU or PyTorch fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, ip, d = C.c_void_p, C.c_int, C.c_double
+        pp = C.POINTER(Params)
+        L.pycool_create.argtypes = [C.POINTER(vp), ip, d, ip, pp, ip, d]
+        L.pycool_work_bytes.argtypes = [ip, ip, ip]
+        L.pycool_work_bytes.restype = C.c_size_t
+        L.pycool_create_ext.argtypes = [C.POINTER(vp), ip, d, ip, pp, ip, d, vp, vp, vp, C.c_size_t, vp]
+        L.pycool_set_fields.argtypes = [vp, vp, vp]
+        L.pycool_set_fields_device.argtypes = [vp, vp, vp]
+        L.pycool_set_background.argtypes = [vp, d, d]
+        L.pycool_set_dt.argtypes = [vp, d]
+        L.pycool_step.argtypes = [vp, ip]
+        L.pycool_sync.argtypes = [vp]
+        L.pycool_read_fields.argtypes = [vp, vp, vp]
+        L.pycool_device_fields.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+        L.pycool_energies.argtypes = [vp, C.POINTER(Energy)]
+        L.pycool_destroy.argtypes = [vp]
+        L.pycool_last_error.argtypes = [vp]
+        L.pycool_last_error.restype = C.c_char_p
+        L.pycool_stage_weights.argtypes = [ip, C.POINTER(d), ip]
+        L.pycool_launch_counts.argtypes = [vp, C.POINTER(C.c_ulonglong)]
+        L.pycool_set_profiling.argtypes = [vp, ip]
+        L.pycool_kick_time_ms.argtypes = [vp, C.POINTER(d), C.POINTER(C.c_ulonglong)]
+        L.pycool_kick_geometry.argtypes = [vp, C.POINTER(ip)]
+        L.pycool_set_zchunk.argtypes = [vp, ip]
+        L.pycool_set_tile.argtypes = [vp, ip]
+        _lib = L
+    return _lib
+
+
+def make_params(model, p=(), mpl=1.0, rho_gamma0=0.0, rho_m0=0.0, stencil=(0, 0, 0, 0), precision=64):
+    mp = Params()
+    mp.model = model
+    for i, v in enumerate(p):
+        mp.p[i] = v
+    mp.mpl = mpl
+    mp.rho_gamma0 = rho_gamma0
+    mp.rho_m0 = rho_m0
+    for i, v in enumerate(stencil):
+        mp.stencil[i] = v
+    mp.precision = precision
+    return mp
+
+
+def stage_weights(order):
+    w = (C.c_double * 16)()
+    n = lib().pycool_stage_weights(order, w, 16)
+    return [w[i] for i in range(n)]
+
+
+def work_bytes(N, nfields, precision=64):
+    return lib().pycool_work_bytes(N, nfields, precision)
+
+
+class Lattice:
+    """One simulation context on a CUDA device.  Same call names as the C ABI.
+
+    device: a torch device (default cuda:0).  The field and work buffers are torch tensors owned by this
+    object; the library computes in them on torch's current stream for that device.
+    """
+
+    def __init__(self, N, L, nfields, model, p=(), order=4, dt=0.01, device=None, **kw):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1201_5029_b200 needs a CUDA device (no CPU fallback)")
+        self._torch = torch
+        self.N, self.L, self.nf, self.order = N, L, nfields, order
+        self.precision = kw.get("precision", 64)
+        self._np = np.float32 if self.precision == 32 else np.float64
+        self._tdtype = torch.float32 if self.precision == 32 else torch.float64
+        self.device = torch.device("cuda:0" if device is None else device)
+        self._mp = make_params(model, p, **kw)
+        self._h = C.c_void_p()
+        need = work_bytes(N, nfields, self.precision)
+        if need == 0:
+            raise PycoolError(EINVAL, "invalid lattice shape")
+        shape = (nfields, N, N, N)
+        with torch.cuda.device(self.device):
+            self._phi0 = torch.empty(shape, dtype=self._tdtype, device=self.device)
+            self._pi0 = torch.empty(shape, dtype=self._tdtype, device=self.device)
+            self._work = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+            wptr = (self._work.data_ptr() + 255) // 256 * 256
+            self.stream = torch.cuda.current_stream(self.device)
+            st = lib().pycool_create_ext(C.byref(self._h), N, L, nfields, C.byref(self._mp), order, dt,
+                                         self._phi0.data_ptr(), self._pi0.data_ptr(), wptr, need,
+                                         self.stream.cuda_stream)
+        if st != OK:
+            raise PycoolError(st, lib().pycool_last_error(None).decode())
+
+    def _chk(self, st):
+        if st != OK:
+            raise PycoolError(st, lib().pycool_last_error(self._h).decode())
+
+    def _host(self, x):
+        x = np.ascontiguousarray(x, dtype=self._np)
+        if x.size != self.nf * self.N ** 3:
+            raise PycoolError(EINVAL, "field buffer has %d elements" % x.size)
+        return x
+
+    def set_fields(self, phi, pi):
+        """phi, pi: host arrays (numpy, or pinned torch CPU tensors) of nf*N^3 elements."""
+        torch = self._torch
+        if isinstance(phi, torch.Tensor) and not phi.is_cuda:
+            assert phi.dtype == self._tdtype and phi.is_contiguous() and pi.is_contiguous()
+            self._chk(lib().pycool_set_fields(self._h, phi.data_ptr(), pi.data_ptr()))
+            return
+        if isinstance(phi, torch.Tensor):
+            assert phi.dtype == self._tdtype and phi.is_contiguous() and pi.is_contiguous()
+            self._chk(lib().pycool_set_fields_device(self._h, phi.data_ptr(), pi.data_ptr()))
+            return
+        phi, pi = self._host(phi), self._host(pi)
+        self._chk(lib().pycool_set_fields(self._h, phi.ctypes.data, pi.ctypes.data))
+
+    def set_background(self, a=1.0, p_a=math.nan):
+        self._chk(lib().pycool_set_background(self._h, a, p_a))
+
+    def set_dt(self, dt):
+        self._chk(lib().pycool_set_dt(self._h, dt))
+
+    def step(self, n=1):
+        self._chk(lib().pycool_step(self._h, n))
+
+    def sync(self):
+        self._chk(lib().pycool_sync(self._h))
+
+    def read_fields(self, out_phi=None, out_pi=None):
+        """Download to new numpy arrays, or into given host buffers (numpy or pinned torch tensors)."""
+        shape = (self.nf, self.N, self.N, self.N)
+        phi = np.empty(shape, self._np) if out_phi is None else out_phi
+        pi = np.empty(shape, self._np) if out_pi is None else out_pi
+        ptr = lambda t: t.data_ptr() if isinstance(t, self._torch.Tensor) else t.ctypes.data
+        self._chk(lib().pycool_read_fields(self._h, ptr(phi), ptr(pi)))
+        return phi, pi
+
+    def device_fields(self):
+        """(phi, pi) as torch views [nf,N,N,N] of the CURRENT state buffers (no copy, no sync)."""
+        a, b = C.c_void_p(), C.c_void_p()
+        self._chk(lib().pycool_device_fields(self._h, C.byref(a), C.byref(b)))
+        return self._view(a.value), self._view(b.value)
+
+    def _view(self, ptr):
+        n = self.nf * self.N ** 3
+        esize = 4 if self.precision == 32 else 8
+        for base in (self._phi0, self._pi0):
+            if ptr == base.data_ptr():
+                return base
+        off = ptr - self._work.data_ptr()
+        assert 0 <= off and off + n * esize <= self._work.numel()
+        return self._work[off:off + n * esize].view(self._tdtype).view(self.nf, self.N, self.N, self.N)
+
+    def energies(self):
+        e = Energy()
+        self._chk(lib().pycool_energies(self._h, C.byref(e)))
+        return e
+
+    def launch_counts(self):
+        c = (C.c_ulonglong * 4)()
+        self._chk(lib().pycool_launch_counts(self._h, c))
+        return [int(x) for x in c]
+
+    def set_profiling(self, on=True):
+        self._chk(lib().pycool_set_profiling(self._h, int(on)))
+
+    def kick_time_ms(self):
+        ms, n = C.c_double(), C.c_ulonglong()
+        self._chk(lib().pycool_kick_time_ms(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, int(n.value)
+
+    def kick_geometry(self):
+        t = (C.c_int * 6)()
+        self._chk(lib().pycool_kick_geometry(self._h, t))
+        return dict(tx=t[0], ty=t[1], zchunk=t[2], threads=t[3], blocks=t[4], smem_bytes=t[5])
+
+    def set_zchunk(self, planes):
+        self._chk(lib().pycool_set_zchunk(self._h, planes))
+
+    def set_tile(self, tile):
+        self._chk(lib().pycool_set_tile(self._h, tile))
+
+    def close(self):
+        if self._h:
+            lib().pycool_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def from_config(cfg, device=None, **over):
+    """Lattice for a config dict of `inputs.CONFIGS` (parameters only; fields are set by the caller)."""
+    kw = dict(mpl=cfg["mpl"], rho_gamma0=cfg["rho_gamma0"], rho_m0=cfg["rho_m0"])
+    kw.update(over)
+    order = kw.pop("order", cfg["order"])
+    dt = kw.pop("dt", cfg["dt"])
+    return Lattice(cfg["N"], cfg["L"], cfg["nfields"], cfg["model"], cfg["p"], order=order, dt=dt,
+                   device=device, **kw)

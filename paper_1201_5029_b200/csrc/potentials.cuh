@@ -1,0 +1,106 @@
+// potentials.cuh -- per-model potentials V(phi_1..phi_nf) and dV/dphi_f as C++ template instances.
+//
+// Replaces PyCOOL's run-time textual code generation (jinja2/SymPy -> CUDA source): each
+// model is a struct with a static, fully inlined `eval`, so the kick kernel is compiled once per
+// <Real, Model> pair with the potential folded into its finalize step.
+//
+// Models (the paper prints V only; the derivatives are spelled out here):
+//   Free<NF>   V = sum_f 1/2 m_f^2 phi_f^2                                      (test model)
+//   Chaotic    V = 1/2 m^2 phi^2 + 1/2 g^2 phi^2 chi^2                          (3.2) PAPER.md:427
+//   Oscillon   V = 1/2 m^2 phi^2 - lambda/4 phi^4 + g6/6 phi^6                  (3.3) PAPER.md:456 (reading G6)
+//   QBall      V = m^2 r2 (1 + K ln(r2/M^2)) + lambda6 r2^3/mpl^2, r2 = (phi1^2+phi2^2)/2
+//                                                                               (3.4) PAPER.md:481 (G6-G8)
+#pragma once
+#include <cfloat>
+
+namespace pycool {
+
+struct ModelParams {
+  double p[8];       // as in pycool_params.p
+  double inv_mpl2;   // 1/mpl^2 (0 for a static background)
+};
+
+template <typename T> __device__ __forceinline__ T min_normal();
+template <> __device__ __forceinline__ double min_normal<double>() { return DBL_MIN; }
+template <> __device__ __forceinline__ float min_normal<float>() { return FLT_MIN; }
+
+__device__ __forceinline__ double log_of(double x) { return log(x); }
+__device__ __forceinline__ float log_of(float x) { return logf(x); }
+
+// Coefficients are converted to the compute type T once per thread (Coef), then eval() is pure T arithmetic.
+template <int NF_>
+struct Free {
+  static constexpr int NF = NF_;
+  template <typename T> struct Coef {
+    T m2[NF_];
+    __device__ explicit Coef(const ModelParams& mp) {
+#pragma unroll
+      for (int f = 0; f < NF_; ++f) m2[f] = T(mp.p[f]);
+    }
+  };
+  template <typename T>
+  static __device__ __forceinline__ T eval(const Coef<T>& c, const T* phi, T* dV) {
+    T v = T(0);
+#pragma unroll
+    for (int f = 0; f < NF_; ++f) {
+      dV[f] = c.m2[f] * phi[f];
+      v += T(0.5) * dV[f] * phi[f];
+    }
+    return v;
+  }
+};
+
+struct Chaotic {
+  static constexpr int NF = 2;
+  template <typename T> struct Coef {
+    T m2, g2;
+    __device__ explicit Coef(const ModelParams& mp) : m2(T(mp.p[0])), g2(T(mp.p[1])) {}
+  };
+  template <typename T>
+  static __device__ __forceinline__ T eval(const Coef<T>& c, const T* phi, T* dV) {
+    const T ph = phi[0], ch = phi[1];
+    const T ph2 = ph * ph;
+    const T u = c.m2 + c.g2 * (ch * ch);   // m^2 + g^2 chi^2
+    dV[0] = ph * u;                        // m^2 phi + g^2 phi chi^2
+    dV[1] = c.g2 * ph2 * ch;               // g^2 phi^2 chi
+    return T(0.5) * ph2 * u;
+  }
+};
+
+struct Oscillon {
+  static constexpr int NF = 1;
+  template <typename T> struct Coef {
+    T m2, lam, g6, hm2, ql, sg;
+    __device__ explicit Coef(const ModelParams& mp)
+        : m2(T(mp.p[0])), lam(T(mp.p[1])), g6(T(mp.p[2])), hm2(T(0.5 * mp.p[0])), ql(T(mp.p[1] / 4.0)),
+          sg(T(mp.p[2] / 6.0)) {}
+  };
+  template <typename T>
+  static __device__ __forceinline__ T eval(const Coef<T>& c, const T* phi, T* dV) {
+    const T ph = phi[0], p2 = ph * ph;
+    dV[0] = ph * (c.m2 + p2 * (c.g6 * p2 - c.lam));       // m^2 phi - lambda phi^3 + g6 phi^5
+    return p2 * (c.hm2 + p2 * (c.sg * p2 - c.ql));
+  }
+};
+
+struct QBall {
+  static constexpr int NF = 2;
+  template <typename T> struct Coef {
+    T m2, K, invM2, six;
+    __device__ explicit Coef(const ModelParams& mp)
+        : m2(T(mp.p[0])), K(T(mp.p[1])), invM2(T(1.0 / mp.p[2])), six(T(mp.p[3] * mp.inv_mpl2)) {}
+  };
+  template <typename T>
+  static __device__ __forceinline__ T eval(const Coef<T>& c, const T* phi, T* dV) {
+    const T r2 = T(0.5) * (phi[0] * phi[0] + phi[1] * phi[1]);      // |Phi|^2, Phi = (phi1 + i phi2)/sqrt 2
+    const T lg = (r2 < min_normal<T>()) ? T(0) : log_of(r2 * c.invM2);   // reading G8
+    const T klg = c.K * lg;
+    const T r4 = r2 * r2;
+    const T common = c.m2 * (T(1) + c.K + klg) + T(3) * c.six * r4;
+    dV[0] = common * phi[0];
+    dV[1] = common * phi[1];
+    return c.m2 * r2 * (T(1) + klg) + c.six * r4 * r2;
+  }
+};
+
+}  // namespace pycool

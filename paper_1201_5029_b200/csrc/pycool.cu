@@ -1,0 +1,668 @@
+// pycool.cu -- context, launch sequencing and the C ABI of libpycool.so (declared in include/pycool.h).
+//
+// The host side only validates arguments, owns buffers and enqueues kernels; a, p_a and every lattice sum live
+// on the device, so pycool_step never synchronises (the paper copies the sums to the host at every sub-step,
+// PAPER.md:395).  Sequence of one pycool_step(n) call, stages h_1..h_S (S = n * stages(order), h = w dt):
+//     scalar_update(mode 0, h_next = h_1)
+//     for i in 1..S:  kick_fused (drift by c_drift, kick by h_i, sums)  ->  scalar_update(mode 1, h_i, h_{i+1})
+//     drift_flush  (closing half drift, c_drift = h_S/(2 a^2))
+// which is (2.48) composed per (2.43)-(2.45) with adjacent H1 and H2 halves merged.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/pycool.h"
+#include "kernels.cuh"
+
+using namespace pycool;
+
+namespace {
+
+// ---- stage weights: (2.42); (2.43)-(2.44) with n = 1 (reading G2); Table 1 ----
+int stage_weights_ld(int order, long double* w) {
+  if (order == 2) { w[0] = 1.0L; return 1; }
+  if (order == 4) {
+    const long double r = cbrtl(2.0L);
+    w[0] = w[2] = 1.0L / (2.0L - r);
+    w[1] = -r / (2.0L - r);
+    return 3;
+  }
+  if (order == 6) {
+    const long double t[3] = {0.78451361047755726382L, 0.23557321335935813368L, -1.17767998417887100695L};
+    const long double mid = 1.0L - 2.0L * (t[0] + t[1] + t[2]);
+    for (int i = 0; i < 3; ++i) w[i] = w[6 - i] = t[i];
+    w[3] = mid;
+    return 7;
+  }
+  if (order == 8) {
+    const long double t[7] = {0.74167036435061295345L, -0.40910082580003159400L, 0.19075471029623837995L,
+                              -0.57386247111608226666L, 0.29906418130365592384L, 0.33462491824529818378L,
+                              0.31529309239676659663L};
+    long double s = 0.0L;
+    for (int i = 0; i < 7; ++i) { s += t[i]; w[i] = w[14 - i] = t[i]; }
+    w[7] = 1.0L - 2.0L * s;
+    return 15;
+  }
+  return 0;
+}
+
+constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
+constexpr int kNumTiles = 3;
+
+struct TileInfo { int tx, ty, k, nt; };
+
+}  // namespace
+
+struct pycool_ctx {
+  int N = 0, nf = 0, order = 0, model = 0, precision = 64;
+  double L = 0, dx = 0, dt = 0, eta = 0, mpl = 1, rho_g = 0, rho_m = 0;
+  size_t V = 0, elems = 0, esize = 8;
+  double c[4] = {0, 0, 0, 0};
+  ModelParams mp{};
+  ScalarConst kc{};
+  int nstages = 0;
+  double w[16];
+  // device memory
+  void* phi[2] = {nullptr, nullptr};
+  void* pi[2] = {nullptr, nullptr};
+  int cur = 0;
+  double* partials = nullptr;   // max(3 * kick blocks, 13 * kMaxSumBlocks) doubles
+  size_t partials_cap = 0;
+  double* sums = nullptr;       // 16 doubles: reduced rows
+  Scalars* sc = nullptr;
+  bool own_mem = false, own_stream = false;
+  void* owned_block = nullptr;  // one allocation when own_mem
+  cudaStream_t stream = nullptr;
+  // launch geometry
+  int tile = -1, zc = 0, zc_user = 0;
+  dim3 grid;
+  // state
+  bool have_fields = false, nonfinite_seen = false;
+  unsigned long long counts[4] = {0, 0, 0, 0};
+  bool profiling = false;
+  std::vector<cudaEvent_t> ev;   // pairs
+  size_t ev_used = 0;
+  double prof_ms = 0;
+  unsigned long long prof_n = 0;
+  std::string err;
+};
+
+namespace {
+
+thread_local std::string g_create_err = "no error";
+
+int fail(pycool_ctx* c, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (c) c->err = buf; else g_create_err = buf;
+  return code;
+}
+#define CUDA_TRY(c, expr)                                                                         \
+  do {                                                                                            \
+    cudaError_t e_ = (expr);                                                                      \
+    if (e_ != cudaSuccess) return fail((c), PYCOOL_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+const TileInfo kTiles[kNumTiles] = {{32, 8, 2, 128}, {32, 16, 2, 256}, {64, 16, 2, 512}};
+using Tile0 = Tile<32, 8, 2>;
+using Tile1 = Tile<32, 16, 2>;
+using Tile2 = Tile<64, 16, 2>;
+
+int auto_tile(int N) { return N <= 64 ? 0 : 1; }
+
+int blocks_xy(int N, int tile) {
+  const TileInfo& t = kTiles[tile];
+  return ((N + t.tx - 1) / t.tx) * ((N + t.ty - 1) / t.ty);
+}
+// z-chunk: enough blocks to fill 148 SMs several times over, chunks not shorter than 16 planes unless N is
+int auto_zchunk(int N, int tile) {
+  const int bxy = blocks_xy(N, tile);
+  int zc = N;
+  while (zc > 16 && (long long)bxy * ((N + zc - 1) / zc) < 148LL * 16) zc = (zc + 1) / 2;
+  return zc < 1 ? 1 : zc;
+}
+// partial-sum capacity actually reserved: automatic geometry of every tile with zc >= min(N, 4)
+size_t partials_capacity(int N) {
+  size_t m = 13 * (size_t)kMaxSumBlocks;
+  const int zmin = N < 4 ? N : 4;
+  for (int t = 0; t < kNumTiles; ++t) {
+    size_t b = 3 * (size_t)blocks_xy(N, t) * (size_t)((N + zmin - 1) / zmin);
+    if (b > m) m = b;
+  }
+  return m;
+}
+
+size_t work_layout(int N, int nf, size_t esize, size_t* off_phi1, size_t* off_pi1, size_t* off_part,
+                   size_t* off_sums, size_t* off_sc) {
+  const size_t bytes = align_up((size_t)nf * N * N * N * esize, 256);
+  size_t o = 0;
+  *off_phi1 = o; o += bytes;
+  *off_pi1 = o; o += bytes;
+  *off_part = o; o += align_up(partials_capacity(N) * sizeof(double), 256);
+  *off_sums = o; o += 256;
+  *off_sc = o; o += 256;
+  return o;
+}
+
+bool valid_shape(int N, int nf, int precision) {
+  return N >= 3 && N <= 2048 && nf >= 1 && nf <= 4 && (precision == 0 || precision == 32 || precision == 64);
+}
+
+// ---- kernel dispatch: <precision, model, nf, tile> -> template instance ----
+template <typename Real, class Model, class T>
+int launch_kick_t(pycool_ctx* c) {
+  static bool attr_done = false;
+  constexpr size_t smem = kick_smem_bytes<Real, Model, T>();
+  if (!attr_done) {
+    CUDA_TRY(c, cudaFuncSetAttribute(kick_fused<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)smem));
+    attr_done = true;
+  }
+  KickArgs<Real> g;
+  g.phi_in = (const Real*)c->phi[c->cur];
+  g.pi_in = (const Real*)c->pi[c->cur];
+  g.phi_out = (Real*)c->phi[c->cur ^ 1];
+  g.pi_out = (Real*)c->pi[c->cur ^ 1];
+  g.sc = c->sc;
+  g.partials = c->partials;
+  g.N = c->N;
+  g.zc = c->zc;
+  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
+  g.mp = c->mp;
+  kick_fused<Real, Model, T><<<c->grid, T::NT, smem, c->stream>>>(g);
+  CUDA_TRY(c, cudaGetLastError());
+  return PYCOOL_OK;
+}
+template <typename Real, class Model>
+int launch_kick_m(pycool_ctx* c) {
+  switch (c->tile) {
+    case 0: return launch_kick_t<Real, Model, Tile0>(c);
+    case 1: return launch_kick_t<Real, Model, Tile1>(c);
+    default: return launch_kick_t<Real, Model, Tile2>(c);
+  }
+}
+template <typename Real, class Model>
+size_t kick_smem_m(int tile) {
+  switch (tile) {
+    case 0: return kick_smem_bytes<Real, Model, Tile0>();
+    case 1: return kick_smem_bytes<Real, Model, Tile1>();
+    default: return kick_smem_bytes<Real, Model, Tile2>();
+  }
+}
+template <typename Real, class Model>
+int launch_energy_m(pycool_ctx* c, int nb) {
+  energy_sums<Real, Model><<<nb, 256, 0, c->stream>>>((const Real*)c->phi[c->cur], (const Real*)c->pi[c->cur],
+                                                      c->N, c->c[1], c->c[2], c->c[3], c->mp, c->partials);
+  CUDA_TRY(c, cudaGetLastError());
+  return PYCOOL_OK;
+}
+
+enum Op { OP_KICK, OP_ENERGY, OP_SMEM };
+template <typename Real>
+long long dispatch_model(pycool_ctx* c, Op op, int arg) {
+#define PYCOOL_CASE(M)                                                    \
+  do {                                                                    \
+    if (op == OP_KICK) return launch_kick_m<Real, M>(c);                  \
+    if (op == OP_ENERGY) return launch_energy_m<Real, M>(c, arg);         \
+    return (long long)kick_smem_m<Real, M>(arg);                          \
+  } while (0)
+  switch (c->model) {
+    case PYCOOL_FREE:
+      switch (c->nf) {
+        case 1: PYCOOL_CASE(Free<1>);
+        case 2: PYCOOL_CASE(Free<2>);
+        case 3: PYCOOL_CASE(Free<3>);
+        default: PYCOOL_CASE(Free<4>);
+      }
+    case PYCOOL_CHAOTIC: PYCOOL_CASE(Chaotic);
+    case PYCOOL_OSCILLON: PYCOOL_CASE(Oscillon);
+    default: PYCOOL_CASE(QBall);
+  }
+#undef PYCOOL_CASE
+}
+long long dispatch(pycool_ctx* c, Op op, int arg) {
+  return c->precision == 32 ? dispatch_model<float>(c, op, arg) : dispatch_model<double>(c, op, arg);
+}
+
+void set_geometry(pycool_ctx* c) {
+  const TileInfo& t = kTiles[c->tile];
+  int zc = c->zc_user > 0 ? c->zc_user : auto_zchunk(c->N, c->tile);
+  if (zc > c->N) zc = c->N;
+  // never exceed the reserved partial-sum capacity
+  while (3 * (size_t)blocks_xy(c->N, c->tile) * (size_t)((c->N + zc - 1) / zc) > c->partials_cap) ++zc;
+  c->zc = zc;
+  c->grid = dim3((c->N + t.tx - 1) / t.tx, (c->N + t.ty - 1) / t.ty, (c->N + zc - 1) / zc);
+}
+
+int launch_scalar(pycool_ctx* c, double h, double h_next, int mode) {
+  const int nb = (int)(c->grid.x * c->grid.y * c->grid.z);
+  scalar_update<<<1, kReduceThreads, 0, c->stream>>>(c->sc, c->partials, nb, c->kc, h, h_next, mode);
+  CUDA_TRY(c, cudaGetLastError());
+  c->counts[1]++;
+  return PYCOOL_OK;
+}
+
+int launch_flush(pycool_ctx* c) {
+  const size_t n = c->elems;
+  int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 32);
+  if (c->precision == 32)
+    drift_flush<float><<<nb, 256, 0, c->stream>>>((float*)c->phi[c->cur], (const float*)c->pi[c->cur], c->sc, n);
+  else
+    drift_flush<double><<<nb, 256, 0, c->stream>>>((double*)c->phi[c->cur], (const double*)c->pi[c->cur], c->sc, n);
+  CUDA_TRY(c, cudaGetLastError());
+  c->counts[2]++;
+  return PYCOOL_OK;
+}
+
+int launch_sum_pi2(pycool_ctx* c) {
+  const size_t n = c->elems;
+  int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)kMaxSumBlocks);
+  if (c->precision == 32) sumsq<float><<<nb, 256, 0, c->stream>>>((const float*)c->pi[c->cur], n, c->partials);
+  else sumsq<double><<<nb, 256, 0, c->stream>>>((const double*)c->pi[c->cur], n, c->partials);
+  CUDA_TRY(c, cudaGetLastError());
+  reduce_rows<<<1, kReduceThreads, 0, c->stream>>>(c->partials, nb, c->sums);
+  CUDA_TRY(c, cudaGetLastError());
+  store_spi2<<<1, 1, 0, c->stream>>>(c->sc, c->sums);
+  CUDA_TRY(c, cudaGetLastError());
+  c->counts[3] += 3;
+  return PYCOOL_OK;
+}
+
+// sums[0 .. 3 nf] <- per field (sum pi^2, sum G, sum phi D phi), then sum V; synchronises
+int energy_sums_host(pycool_ctx* c, double* out /* 3 nf + 1 */) {
+  const int nq = 3 * c->nf + 1;
+  int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)kMaxSumBlocks);
+  int st = (int)dispatch(c, OP_ENERGY, nb);
+  if (st != PYCOOL_OK) return st;
+  reduce_rows<<<nq, kReduceThreads, 0, c->stream>>>(c->partials, nb, c->sums);
+  CUDA_TRY(c, cudaGetLastError());
+  c->counts[3] += 2;
+  CUDA_TRY(c, cudaMemcpyAsync(out, c->sums, nq * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return PYCOOL_OK;
+}
+
+int read_scalars(pycool_ctx* c, Scalars* s) {
+  CUDA_TRY(c, cudaMemcpyAsync(s, c->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (s->nonfinite) {
+    c->nonfinite_seen = true;
+    return fail(c, PYCOOL_ENONFINITE, "a lattice sum became non-finite");
+  }
+  return PYCOOL_OK;
+}
+
+struct Averages { double K[4], Gr[4], GrD[4], Vbar; };
+
+// lattice averages entering rho and P at scale factor a: (2.16), (2.8), (2.17)
+int averages(pycool_ctx* c, double a, Averages* av) {
+  double s[16];
+  int st = energy_sums_host(c, s);
+  if (st != PYCOOL_OK) return st;
+  const double a2 = a * a, a6 = a2 * a2 * a2, Vs = (double)c->V, dx2 = c->dx * c->dx;
+  for (int f = 0; f < c->nf; ++f) {
+    av->K[f] = s[3 * f] / (2.0 * a6 * Vs);
+    av->Gr[f] = s[3 * f + 1] / (2.0 * a2 * dx2 * Vs);
+    av->GrD[f] = -s[3 * f + 2] / (2.0 * a2 * dx2 * Vs);
+  }
+  av->Vbar = s[3 * c->nf] / Vs;
+  return PYCOOL_OK;
+}
+
+int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params* p, int order, double dt,
+                  void* d_phi, void* d_pi, void* d_work, size_t work_bytes, void* stream, bool ext) {
+  if (!out) return fail(nullptr, PYCOOL_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!p) return fail(nullptr, PYCOOL_EINVAL, "params is NULL");
+  if (!valid_shape(N, nf, p->precision)) return fail(nullptr, PYCOOL_EINVAL, "N must be 3..2048, nfields 1..4, precision 0/32/64");
+  if (!(L > 0) || !std::isfinite(L)) return fail(nullptr, PYCOOL_EINVAL, "L must be finite and > 0");
+  long double wl[16];
+  const int ns = stage_weights_ld(order, wl);
+  if (ns == 0) return fail(nullptr, PYCOOL_EINVAL, "order must be 2, 4, 6 or 8");
+  if (dt == 0 || !std::isfinite(dt)) return fail(nullptr, PYCOOL_EINVAL, "dt must be finite and non-zero");
+  if (p->model < PYCOOL_FREE || p->model > PYCOOL_QBALL) return fail(nullptr, PYCOOL_EINVAL, "unknown model");
+  if ((p->model == PYCOOL_CHAOTIC || p->model == PYCOOL_QBALL) && nf != 2)
+    return fail(nullptr, PYCOOL_EINVAL, "this model needs nfields = 2");
+  if (p->model == PYCOOL_OSCILLON && nf != 1) return fail(nullptr, PYCOOL_EINVAL, "oscillon needs nfields = 1");
+  if (!(p->mpl > 0)) return fail(nullptr, PYCOOL_EINVAL, "mpl must be > 0 (+INF = static background)");
+  if (p->model == PYCOOL_QBALL && !(p->p[2] > 0)) return fail(nullptr, PYCOOL_EINVAL, "Q-ball needs M^2 > 0");
+  const double* cs = p->stencil;
+  const bool dflt = cs[0] == 0 && cs[1] == 0 && cs[2] == 0 && cs[3] == 0;
+  if (!dflt) {
+    const double s = 6 * cs[1] + 12 * cs[2] + 8 * cs[3];
+    if (!(std::fabs(cs[0] + s) <= 1e-12 * (std::fabs(cs[0]) + std::fabs(s))))
+      return fail(nullptr, PYCOOL_EINVAL, "stencil must satisfy c0 = -(6 c1 + 12 c2 + 8 c3)");
+  }
+  if (ext && (!d_phi || !d_pi || !d_work)) return fail(nullptr, PYCOOL_EINVAL, "device buffers are NULL");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(nullptr, PYCOOL_ECUDA, "no CUDA device: libpycool has no CPU path");
+  }
+  pycool_ctx* c = new (std::nothrow) pycool_ctx();
+  if (!c) return fail(nullptr, PYCOOL_ENOMEM, "host allocation failed");
+  c->N = N; c->nf = nf; c->order = order; c->model = p->model;
+  c->precision = p->precision == 32 ? 32 : 64;
+  c->esize = c->precision == 32 ? 4 : 8;
+  c->L = L; c->dx = L / N; c->dt = dt; c->mpl = p->mpl; c->rho_g = p->rho_gamma0; c->rho_m = p->rho_m0;
+  c->V = (size_t)N * N * N; c->elems = c->V * nf;
+  if (dflt) { c->c[0] = -128.0 / 30.0; c->c[1] = 14.0 / 30.0; c->c[2] = 3.0 / 30.0; c->c[3] = 1.0 / 30.0; }
+  else for (int i = 0; i < 4; ++i) c->c[i] = cs[i];
+  for (int i = 0; i < 8; ++i) c->mp.p[i] = p->p[i];
+  c->mp.inv_mpl2 = std::isinf(p->mpl) ? 0.0 : 1.0 / (p->mpl * p->mpl);
+  c->kc.den = 6.0 * (double)c->V * p->mpl * p->mpl;
+  c->kc.Vrho_m = (double)c->V * p->rho_m0;
+  c->kc.dx2 = c->dx * c->dx;
+  c->nstages = ns;
+  for (int i = 0; i < ns; ++i) c->w[i] = (double)wl[i];
+
+  size_t o_phi1, o_pi1, o_part, o_sums, o_sc;
+  const size_t need = work_layout(N, nf, c->esize, &o_phi1, &o_pi1, &o_part, &o_sums, &o_sc);
+  const size_t state_bytes = align_up(c->elems * c->esize, 256);
+  unsigned char* work = nullptr;
+  int rc = PYCOOL_OK;
+  if (ext) {
+    if (work_bytes < need) { rc = fail(nullptr, PYCOOL_EINVAL, "work buffer too small: need %zu bytes", need); goto bad; }
+    if (((uintptr_t)d_work & 255) != 0) { rc = fail(nullptr, PYCOOL_EINVAL, "work buffer must be 256-byte aligned"); goto bad; }
+    c->phi[0] = d_phi; c->pi[0] = d_pi;
+    work = (unsigned char*)d_work;
+    c->stream = (cudaStream_t)stream;
+  } else {
+    void* blk = nullptr;
+    if (cudaMalloc(&blk, need + 2 * state_bytes) != cudaSuccess) {
+      cudaGetLastError();
+      rc = fail(nullptr, PYCOOL_ENOMEM, "cudaMalloc of %zu bytes failed", need + 2 * state_bytes);
+      goto bad;
+    }
+    c->owned_block = blk; c->own_mem = true;
+    c->phi[0] = blk;
+    c->pi[0] = (unsigned char*)blk + state_bytes;
+    work = (unsigned char*)blk + 2 * state_bytes;
+    if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) {
+      cudaGetLastError();
+      rc = fail(nullptr, PYCOOL_ECUDA, "cudaStreamCreate failed");
+      goto bad;
+    }
+    c->own_stream = true;
+  }
+  c->phi[1] = work + o_phi1; c->pi[1] = work + o_pi1;
+  c->partials = (double*)(work + o_part);
+  c->partials_cap = partials_capacity(N);
+  c->sums = (double*)(work + o_sums);
+  c->sc = (Scalars*)(work + o_sc);
+  c->tile = auto_tile(N);
+  set_geometry(c);
+  {
+    Scalars s0;
+    std::memset(&s0, 0, sizeof s0);
+    s0.a = 1.0;
+    if (cudaMemcpyAsync(c->sc, &s0, sizeof s0, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess) {
+      rc = fail(nullptr, PYCOOL_ECUDA, "initialising device scalars failed: %s", cudaGetErrorString(cudaGetLastError()));
+      goto bad;
+    }
+  }
+  *out = c;
+  return PYCOOL_OK;
+bad:
+  if (c->own_stream) cudaStreamDestroy(c->stream);
+  if (c->owned_block) cudaFree(c->owned_block);
+  delete c;
+  return rc;
+}
+
+}  // namespace
+
+// =================================================================================================== C ABI
+extern "C" {
+
+int pycool_create(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
+                  double dt) {
+  return create_common(out, N, L, nfields, params, order, dt, nullptr, nullptr, nullptr, 0, nullptr, false);
+}
+
+size_t pycool_work_bytes(int N, int nfields, int precision) {
+  if (!valid_shape(N, nfields, precision)) return 0;
+  size_t a, b, c, d, e;
+  return work_layout(N, nfields, precision == 32 ? 4 : 8, &a, &b, &c, &d, &e);
+}
+
+int pycool_create_ext(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
+                      double dt, void* d_phi, void* d_pi, void* d_work, size_t work_bytes, void* cuda_stream) {
+  return create_common(out, N, L, nfields, params, order, dt, d_phi, d_pi, d_work, work_bytes, cuda_stream, true);
+}
+
+static int after_upload(pycool_ctx* c) {
+  c->have_fields = true;
+  c->nonfinite_seen = false;
+  int zero = 0;
+  CUDA_TRY(c, cudaMemcpyAsync(&c->sc->nonfinite, &zero, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  return launch_sum_pi2(c);
+}
+
+int pycool_set_fields(pycool_ctx* c, const void* phi_host, const void* pi_host) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!phi_host || !pi_host) return fail(c, PYCOOL_EINVAL, "phi_host / pi_host is NULL");
+  c->cur = 0;
+  const size_t bytes = c->elems * c->esize;
+  CUDA_TRY(c, cudaMemcpyAsync(c->phi[0], phi_host, bytes, cudaMemcpyHostToDevice, c->stream));
+  CUDA_TRY(c, cudaMemcpyAsync(c->pi[0], pi_host, bytes, cudaMemcpyHostToDevice, c->stream));
+  int st = after_upload(c);
+  if (st != PYCOOL_OK) return st;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return PYCOOL_OK;
+}
+
+int pycool_set_fields_device(pycool_ctx* c, const void* d_phi_src, const void* d_pi_src) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!d_phi_src || !d_pi_src) return fail(c, PYCOOL_EINVAL, "source pointer is NULL");
+  c->cur = 0;
+  const size_t bytes = c->elems * c->esize;
+  if (d_phi_src != c->phi[0])
+    CUDA_TRY(c, cudaMemcpyAsync(c->phi[0], d_phi_src, bytes, cudaMemcpyDeviceToDevice, c->stream));
+  if (d_pi_src != c->pi[0])
+    CUDA_TRY(c, cudaMemcpyAsync(c->pi[0], d_pi_src, bytes, cudaMemcpyDeviceToDevice, c->stream));
+  return after_upload(c);
+}
+
+int pycool_set_background(pycool_ctx* c, double a, double p_a) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!(a > 0) || !std::isfinite(a)) return fail(c, PYCOOL_EINVAL, "a must be finite and > 0");
+  if (std::isnan(p_a)) {                                   // reading G10: (2.18), expanding branch
+    if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "p_a = NaN needs fields (call set_fields first)");
+    if (std::isinf(c->mpl)) return fail(c, PYCOOL_EINVAL, "p_a = NaN with a static background (mpl = INF)");
+    Averages av;
+    int st = averages(c, a, &av);
+    if (st != PYCOOL_OK) return st;
+    const double a2 = a * a;
+    double rho = av.Vbar + c->rho_g / (a2 * a2) + c->rho_m / (a2 * a);
+    for (int f = 0; f < c->nf; ++f) rho += av.K[f] + av.Gr[f];
+    if (!(rho >= 0)) return fail(c, PYCOOL_EINVAL, "negative or non-finite energy density");
+    const double ap = a2 * (double)sqrtl((long double)(rho / 3.0)) / c->mpl;      // (2.18)
+    p_a = -6.0 * (double)c->V * c->mpl * c->mpl * ap;                              // (2.11)
+  }
+  set_scalars<<<1, 1, 0, c->stream>>>(c->sc, a, p_a, 1);
+  CUDA_TRY(c, cudaGetLastError());
+  return PYCOOL_OK;
+}
+
+int pycool_set_dt(pycool_ctx* c, double dt) {
+  if (!c) return PYCOOL_EINVAL;
+  if (dt == 0 || !std::isfinite(dt)) return fail(c, PYCOOL_EINVAL, "dt must be finite and non-zero");
+  c->dt = dt;
+  return PYCOOL_OK;
+}
+
+int pycool_step(pycool_ctx* c, int nsteps) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "step before set_fields");
+  if (nsteps < 0) return fail(c, PYCOOL_EINVAL, "nsteps < 0");
+  if (c->nonfinite_seen) return fail(c, PYCOOL_ENONFINITE, "a lattice sum became non-finite");
+  if (nsteps == 0) return PYCOOL_OK;
+  const int ns = c->nstages;
+  const long long S = (long long)nsteps * ns;
+  int st = launch_scalar(c, 0.0, c->w[0] * c->dt, 0);
+  if (st != PYCOOL_OK) return st;
+  if (c->profiling && c->ev.size() < c->ev_used + 2 * (size_t)S) {
+    const size_t want = c->ev_used + 2 * (size_t)S;
+    while (c->ev.size() < want) {
+      cudaEvent_t e;
+      CUDA_TRY(c, cudaEventCreate(&e));
+      c->ev.push_back(e);
+    }
+  }
+  for (long long i = 0; i < S; ++i) {
+    const double h = c->w[i % ns] * c->dt;
+    const double h_next = (i + 1 < S) ? c->w[(i + 1) % ns] * c->dt : 0.0;
+    if (c->profiling) CUDA_TRY(c, cudaEventRecord(c->ev[c->ev_used++], c->stream));
+    st = (int)dispatch(c, OP_KICK, 0);
+    if (st != PYCOOL_OK) return st;
+    if (c->profiling) CUDA_TRY(c, cudaEventRecord(c->ev[c->ev_used++], c->stream));
+    c->counts[0]++;
+    c->cur ^= 1;
+    st = launch_scalar(c, h, h_next, 1);
+    if (st != PYCOOL_OK) return st;
+  }
+  st = launch_flush(c);
+  if (st != PYCOOL_OK) return st;
+  for (int i = 0; i < nsteps; ++i) c->eta += c->dt;
+  return PYCOOL_OK;
+}
+
+int pycool_sync(pycool_ctx* c) {
+  if (!c) return PYCOOL_EINVAL;
+  Scalars s;
+  return read_scalars(c, &s);
+}
+
+int pycool_read_fields(pycool_ctx* c, void* phi_host, void* pi_host) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "read before set_fields");
+  const size_t bytes = c->elems * c->esize;
+  if (phi_host) CUDA_TRY(c, cudaMemcpyAsync(phi_host, c->phi[c->cur], bytes, cudaMemcpyDeviceToHost, c->stream));
+  if (pi_host) CUDA_TRY(c, cudaMemcpyAsync(pi_host, c->pi[c->cur], bytes, cudaMemcpyDeviceToHost, c->stream));
+  Scalars s;
+  return read_scalars(c, &s);
+}
+
+int pycool_device_fields(pycool_ctx* c, void** d_phi, void** d_pi) {
+  if (!c) return PYCOOL_EINVAL;
+  if (d_phi) *d_phi = c->phi[c->cur];
+  if (d_pi) *d_pi = c->pi[c->cur];
+  return PYCOOL_OK;
+}
+
+int pycool_energies(pycool_ctx* c, pycool_energy* o) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!o) return fail(c, PYCOOL_EINVAL, "out is NULL");
+  if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "energies before set_fields");
+  Scalars s;
+  int st = read_scalars(c, &s);
+  if (st != PYCOOL_OK) return st;
+  Averages av;
+  st = averages(c, s.a, &av);
+  if (st != PYCOOL_OK) return st;
+  std::memset(o, 0, sizeof *o);
+  const double a = s.a, a2 = a * a;
+  double rho = av.Vbar + c->rho_g / (a2 * a2) + c->rho_m / (a2 * a);               // (2.16) + (2.20)
+  double P = -av.Vbar + c->rho_g / (3.0 * a2 * a2);
+  for (int f = 0; f < c->nf; ++f) {
+    rho += av.K[f] + av.Gr[f];
+    P += av.K[f] - av.Gr[f] / 3.0;
+    o->kin[f] = av.K[f]; o->grad[f] = av.Gr[f]; o->sum_phiDphi[f] = av.GrD[f];
+  }
+  const double ap = -s.p_a / (6.0 * (double)c->V * c->mpl * c->mpl);               // (2.14)
+  const double H = ap / a2;
+  o->a = a; o->p_a = s.p_a; o->eta = c->eta;
+  o->pot = av.Vbar; o->rho = rho; o->pressure = P; o->hubble = H;
+  o->residual = std::isinf(c->mpl) ? 0.0 : std::fabs(rho / (3.0 * c->mpl * c->mpl * H * H) - 1.0);   // (3.1)
+  return PYCOOL_OK;
+}
+
+int pycool_destroy(pycool_ctx* c) {
+  if (!c) return PYCOOL_EINVAL;
+  if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->own_stream) cudaStreamDestroy(c->stream);
+  if (c->owned_block) cudaFree(c->owned_block);
+  delete c;
+  return PYCOOL_OK;
+}
+
+const char* pycool_last_error(const pycool_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+int pycool_stage_weights(int order, double* w, int cap) {
+  long double t[16];
+  const int s = stage_weights_ld(order, t);
+  if (s == 0 || !w || cap < s) return 0;
+  for (int i = 0; i < s; ++i) w[i] = (double)t[i];
+  return s;
+}
+
+int pycool_launch_counts(const pycool_ctx* c, unsigned long long counts[4]) {
+  if (!c || !counts) return PYCOOL_EINVAL;
+  for (int i = 0; i < 4; ++i) counts[i] = c->counts[i];
+  return PYCOOL_OK;
+}
+
+int pycool_set_profiling(pycool_ctx* c, int on) {
+  if (!c) return PYCOOL_EINVAL;
+  c->profiling = on != 0;
+  c->ev_used = 0; c->prof_ms = 0; c->prof_n = 0;
+  return PYCOOL_OK;
+}
+
+int pycool_kick_time_ms(pycool_ctx* c, double* total_ms, unsigned long long* launches) {
+  if (!c) return PYCOOL_EINVAL;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+    float ms = 0;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+    c->prof_ms += ms;
+    c->prof_n++;
+  }
+  c->ev_used = 0;
+  if (total_ms) *total_ms = c->prof_ms;
+  if (launches) *launches = c->prof_n;
+  return PYCOOL_OK;
+}
+
+int pycool_kick_geometry(const pycool_ctx* c, int tile[6]) {
+  if (!c || !tile) return PYCOOL_EINVAL;
+  const TileInfo& t = kTiles[c->tile];
+  tile[0] = t.tx; tile[1] = t.ty; tile[2] = c->zc; tile[3] = t.nt;
+  tile[4] = (int)(c->grid.x * c->grid.y * c->grid.z);
+  tile[5] = (int)dispatch(const_cast<pycool_ctx*>(c), OP_SMEM, c->tile);
+  return PYCOOL_OK;
+}
+
+int pycool_set_zchunk(pycool_ctx* c, int planes) {
+  if (!c) return PYCOOL_EINVAL;
+  if (planes < 0) return fail(c, PYCOOL_EINVAL, "planes < 0");
+  c->zc_user = planes;
+  set_geometry(c);
+  return PYCOOL_OK;
+}
+
+int pycool_set_tile(pycool_ctx* c, int tile) {
+  if (!c) return PYCOOL_EINVAL;
+  if (tile < -1 || tile >= kNumTiles) return fail(c, PYCOOL_EINVAL, "tile must be -1 (auto) .. %d", kNumTiles - 1);
+  c->tile = tile < 0 ? auto_tile(c->N) : tile;
+  set_geometry(c);
+  return PYCOOL_OK;
+}
+
+}  // extern "C"

@@ -20,7 +20,7 @@ except Exception:  # pragma: no cover
     from numpy import fft as _fft
     _FFT_KW = {}
 
-# model ids of the C ABI (include/pycool.h and oracle/oracle.h declare the same values independently)
+# model ids of the C ABI (the CUDA library's header and the CPU checker's header each declare these values)
 FREE, CHAOTIC, OSCILLON, QBALL = 0, 1, 2, 3
 
 # Chaotic model in program units (time, length in 1/m; fields in m_pl): PAPER.md:427-432, readings G11/G12/G19

@@ -1,0 +1,115 @@
+"""Host-side checks of the C-ABI library that need no GPU: it builds, loads, exports every symbol
+include/pycool.h declares, validates arguments, and refuses to run without a CUDA device."""
+import ctypes as C
+import math
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_1201_5029_b200 import build
+    build.build()
+    from paper_1201_5029_b200 import binding
+    return binding.lib()
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "pycool.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return set(re.findall(r"\b(pycool_[a-z0-9_]+)\s*\(", src))
+
+
+def test_header_symbols_all_exported(L):
+    from paper_1201_5029_b200 import binding
+    declared = _declared()
+    assert declared == set(binding.SYMBOLS)
+    for name in declared:
+        assert getattr(L, name) is not None
+
+
+def test_only_abi_symbols_are_exported(L):
+    import subprocess
+    from paper_1201_5029_b200 import binding
+    out = subprocess.run(["nm", "-D", "--defined-only", binding.LIB_PATH], capture_output=True, text=True).stdout
+    names = {ln.split()[-1] for ln in out.splitlines() if " T " in ln}
+    assert {n for n in names if n.startswith("pycool_")} == set(binding.SYMBOLS)
+    assert not any("oracle" in n for n in names)
+
+
+def test_struct_sizes_match_header():
+    """ctypes mirrors of pycool_params / pycool_energy against a C compiler's view of the header."""
+    import subprocess
+    import tempfile
+    from paper_1201_5029_b200 import binding
+    code = '#include <stdio.h>\n#include "pycool.h"\nint main(){printf("%zu %zu\\n", sizeof(pycool_params), sizeof(pycool_energy));return 0;}\n'
+    with tempfile.TemporaryDirectory() as d:
+        src, exe = os.path.join(d, "s.c"), os.path.join(d, "s")
+        open(src, "w").write(code)
+        subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), src, "-o", exe], check=True)
+        a, b = map(int, subprocess.run([exe], capture_output=True, text=True).stdout.split())
+    assert a == C.sizeof(binding.Params) and b == C.sizeof(binding.Energy)
+
+
+def test_stage_weights_host_logic(L, golden_dir):
+    from paper_1201_5029_b200 import binding
+    from helpers import weights
+    for order, n in ((2, 1), (4, 3), (6, 7), (8, 15)):
+        w = binding.stage_weights(order)
+        assert len(w) == n and w == w[::-1] and abs(sum(w) - 1) < 4e-15
+        want = [float(x) for x in weights(golden_dir, order)]
+        assert max(abs(a - b) for a, b in zip(w, want)) < 2e-16
+    assert binding.stage_weights(3) == [] and binding.stage_weights(10) == []
+
+
+def test_work_bytes(L):
+    from paper_1201_5029_b200 import binding
+    assert binding.work_bytes(2, 1) == 0 and binding.work_bytes(32, 5) == 0 and binding.work_bytes(32, 1, 16) == 0
+    b64, b32 = binding.work_bytes(64, 2, 64), binding.work_bytes(64, 2, 32)
+    assert b64 >= 2 * 2 * 64 ** 3 * 8 and b32 >= 2 * 2 * 64 ** 3 * 4 and b32 < b64
+    assert binding.work_bytes(1024, 2, 64) >= 2 * 2 * 1024 ** 3 * 8
+
+
+def test_create_validates_then_needs_a_gpu(L):
+    import torch
+    from paper_1201_5029_b200 import binding
+    h = C.c_void_p()
+
+    def create(N=8, Lbox=1.0, nf=1, model=binding.FREE, order=4, dt=0.1, **kw):
+        mp = binding.make_params(model, kw.pop("p", (1.0,)), **kw)
+        return L.pycool_create(C.byref(h), N, Lbox, nf, C.byref(mp), order, dt)
+
+    for bad in (dict(N=2), dict(Lbox=0.0), dict(nf=0), dict(nf=5), dict(order=5), dict(dt=0.0),
+                dict(dt=math.nan), dict(model=7), dict(model=binding.CHAOTIC, nf=1),
+                dict(model=binding.OSCILLON, nf=2), dict(mpl=0.0), dict(stencil=(-5.0, 1.0, 0.0, 0.0)),
+                dict(precision=16), dict(model=binding.QBALL, nf=2, p=(1.0, -0.1, 0.0, 0.0))):
+        assert create(**bad) == binding.EINVAL, bad
+        assert h.value is None
+        assert len(L.pycool_last_error(None)) > 0
+    if not torch.cuda.is_available():
+        assert create() == binding.ECUDA                      # no CPU path, by design
+        assert b"no CPU path" in L.pycool_last_error(None)
+        with pytest.raises(RuntimeError):
+            binding.Lattice(8, 1.0, 1, binding.FREE, (1.0,))
+    assert L.pycool_step(None, 1) == binding.EINVAL
+    assert L.pycool_destroy(None) == binding.EINVAL
+
+
+def test_product_does_not_touch_the_oracle():
+    """Nothing under the package or include/ may import, include or link the oracle."""
+    pkg = os.path.join(ROOT, "paper_1201_5029_b200")
+    for base, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(base, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", txt, flags=re.M), f
+                assert not re.search(r'#\s*include\s*["<][^">]*oracle', txt) and "liboracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp", ".h")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_1201_5029_b200" not in txt and "from paper_1201_5029_b200" not in txt, f
+            assert "pycool.h" not in txt or f == "oracle.h", f

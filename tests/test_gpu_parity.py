@@ -1,0 +1,313 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  All tests here need a B200 (`-m gpu`).
+
+Tolerances (north_star, fp64): per-site max relative error (reading G18) <= 1e-12 after 1 step and <= 1e-9
+after 100 steps on configs[0]; scale factor and energy components <= 1e-10 relative.  fp32: <= 1e-5 after one
+step.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+from paper_1201_5029_b200 import inputs
+from helpers import SEVEN_POINT, rel_err_per_site
+
+INF = math.inf
+
+
+@pytest.fixture(scope="module")
+def pc():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1201_5029_b200 import build
+    build.build()
+    from paper_1201_5029_b200 import binding
+    binding.lib()
+    return binding
+
+
+def make_pair(pc, cfg, precision=64, **over):
+    kw = dict(mpl=cfg["mpl"], rho_gamma0=cfg["rho_gamma0"], rho_m0=cfg["rho_m0"], precision=precision)
+    kw.update(over)
+    order, dt = kw.pop("order", cfg["order"]), kw.pop("dt", cfg["dt"])
+    g = pc.Lattice(cfg["N"], cfg["L"], cfg["nfields"], cfg["model"], cfg["p"], order=order, dt=dt, **kw)
+    o = oracle.Oracle(cfg["N"], cfg["L"], cfg["nfields"], cfg["model"], cfg["p"], order=order, dt=dt, **kw)
+    return g, o
+
+
+def start(g, o, phi, pi, a=1.0, p_a=math.nan):
+    for s in (g, o):
+        s.set_fields(phi, pi)
+        s.set_background(a, p_a)
+
+
+def rel(a, b):
+    return abs(a - b) / max(abs(b), 1e-300)
+
+
+def check_scalars(eg, eo, nf, tol=1e-10, static=False):
+    assert rel(eg.a, eo.a) <= tol and rel(eg.eta, eo.eta) <= 1e-14
+    if not static:
+        assert rel(eg.p_a, eo.p_a) <= tol and rel(eg.hubble, eo.hubble) <= tol
+    for f in range(nf):
+        assert rel(eg.kin[f], eo.kin[f]) <= tol, ("kin", f, eg.kin[f], eo.kin[f])
+        assert rel(eg.grad[f], eo.grad[f]) <= tol, ("grad", f, eg.grad[f], eo.grad[f])
+        assert rel(eg.sum_phiDphi[f], eo.sum_phiDphi[f]) <= max(tol, 1e-9), ("phiDphi", f)
+    assert rel(eg.pot, eo.pot) <= tol and rel(eg.rho, eo.rho) <= tol and rel(eg.pressure, eo.pressure) <= tol
+
+
+def compare(g, o, nf, tol_site, tol_scalar=1e-10, static=False):
+    pg, qg = g.read_fields()
+    po, qo = o.read_fields()
+    e1, e2 = rel_err_per_site(pg, po), rel_err_per_site(qg, qo)
+    assert e1 <= tol_site and e2 <= tol_site, (e1, e2)
+    check_scalars(g.energies(), o.energies(), nf, tol_scalar, static)
+    return max(e1, e2)
+
+
+# ------------------------------------------------------------------------------------- configs[0]
+def test_cfg0_one_step_and_100_steps(pc):
+    cfg = inputs.config("cfg0_chaotic32")
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    start(g, o, phi, pi)
+    check_scalars(g.energies(), o.energies(), 2)            # initial energies and the (2.18) solve
+    g.step(1); o.step(1)
+    compare(g, o, 2, 1e-12)
+    g.step(99); o.step(99)
+    compare(g, o, 2, 1e-9)
+    assert g.energies().residual < 1e-6
+
+
+def test_cfg0_resolved_dt(pc):
+    cfg = inputs.config("cfg0b_chaotic32_resolved")
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    start(g, o, phi, pi)
+    g.step(1); o.step(1)
+    compare(g, o, 2, 1e-12)
+    g.step(99); o.step(99)
+    compare(g, o, 2, 1e-9)
+
+
+def test_cfg0_paper_phi0_reading_g19(pc):
+    """The paper's phi0 = 1.009343 with the resolved dt (G19)."""
+    cfg = inputs.config("cfg0b_chaotic32_resolved", phi0=(1.009343, 0.0))
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    start(g, o, phi, pi)
+    assert rel(g.energies().hubble, 0.50467) < 2e-5          # H printed in the paper
+    g.step(20); o.step(20)
+    compare(g, o, 2, 1e-10)
+
+
+# ------------------------------------------------------------------------------------- reduced-size cfg1-3
+@pytest.mark.parametrize("name,N,steps", [("cfg1_chaotic128", 48, 6), ("cfg2_oscillon256", 40, 20),
+                                          ("cfg3_qball256", 40, 20)])
+def test_models_reduced_size(pc, name, N, steps):
+    cfg = inputs.config(name, N=N)
+    if name == "cfg2_oscillon256":
+        cfg["L"] = 400.0 * N / 256                          # keep dx of the full configuration
+    if name == "cfg3_qball256":
+        cfg["L"] = 8.0 * N / 256
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    start(g, o, phi, pi)
+    g.step(1); o.step(1)
+    compare(g, o, cfg["nfields"], 1e-12)
+    g.step(steps - 1); o.step(steps - 1)
+    compare(g, o, cfg["nfields"], 1e-10)
+
+
+# ------------------------------------------------------------------------------------- orders, tiles, chunks
+@pytest.mark.parametrize("order", [2, 4, 6, 8])
+def test_all_orders(pc, order):
+    cfg = inputs.config("cfg0_chaotic32", N=20, dt=0.004, order=order)
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    start(g, o, phi, pi)
+    g.step(3); o.step(3)
+    compare(g, o, 2, 5e-12)
+    assert g.launch_counts()[0] == 3 * {2: 1, 4: 3, 6: 7, 8: 15}[order]
+
+
+@pytest.mark.parametrize("tile", [0, 1, 2])
+@pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32)])
+def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
+    """Several tiles with ragged tails in x, y and z, wrap-around at every face, for each tile variant."""
+    cfg = inputs.config("cfg0_chaotic32", N=N, dt=0.002, order=4)
+    cfg["init"], cfg["amp"] = "white", 1e-3
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    g.set_tile(tile)
+    g.set_zchunk(zc)
+    geo = g.kick_geometry()
+    assert geo["zchunk"] >= 1 and geo["blocks"] >= 1
+    start(g, o, phi, pi)
+    g.step(2); o.step(2)
+    compare(g, o, 2, 2e-12)
+
+
+def test_bitwise_reproducible(pc):
+    cfg = inputs.config("cfg0_chaotic32", N=48)
+    phi, pi = inputs.make_initial(cfg)
+    outs = []
+    for _ in range(2):
+        g = pc.from_config(cfg)
+        g.set_fields(phi, pi)
+        g.set_background(1.0)
+        g.step(5)
+        p, q = g.read_fields()
+        e = g.energies()
+        outs.append((p.copy(), q.copy(), e.a, e.p_a, e.kin[0], e.grad[1], e.pot))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert outs[0][2:] == outs[1][2:]
+
+
+def test_step_split_equals_one_call(pc):
+    """pycool_step(3) and three pycool_step(1) calls agree to rounding (merged vs separate half drifts)."""
+    cfg = inputs.config("cfg0_chaotic32", N=24)
+    phi, pi = inputs.make_initial(cfg)
+    a, b = pc.from_config(cfg), pc.from_config(cfg)
+    for g in (a, b):
+        g.set_fields(phi, pi)
+        g.set_background(1.0)
+    a.step(3)
+    for _ in range(3):
+        b.step(1)
+    pa, qa = a.read_fields()
+    pb, qb = b.read_fields()
+    assert rel_err_per_site(pa, pb) < 1e-14 and rel_err_per_site(qa, qb) < 1e-14
+    assert rel(a.energies().a, b.energies().a) < 1e-14 and abs(a.energies().eta - 3 * cfg["dt"]) < 1e-15
+
+
+# ------------------------------------------------------------------------------------- free model, stencils
+@pytest.mark.parametrize("nf", [1, 2, 3, 4])
+@pytest.mark.parametrize("stencil", [(0, 0, 0, 0), SEVEN_POINT])
+def test_free_fields_static_background(pc, nf, stencil):
+    N = 18
+    phi, pi = inputs.random_fields(N, nf, seed=nf, mean=0.5, amp=0.1)
+    kw = dict(order=4, dt=0.01, mpl=INF, stencil=stencil)
+    m2 = [0.5 + f for f in range(nf)]
+    g = pc.Lattice(N, 4.0, nf, pc.FREE, m2, **kw)
+    o = oracle.Oracle(N, 4.0, nf, oracle.FREE, m2, **kw)
+    start(g, o, phi, pi, 1.0, 0.0)
+    g.step(4); o.step(4)
+    compare(g, o, nf, 5e-13, static=True)
+
+
+def test_kick_alone_gives_the_laplacian(pc):
+    """V = 0, static, one 2nd-order step from pi = 0: pi' = dt D[phi + dt/2 * 0]/dx^2, so the GPU stencil is
+    compared with the oracle's D of (2.7) directly, site by site."""
+    N, L, dt = 21, 3.0, 0.125
+    phi, _ = inputs.random_fields(N, 1, seed=5, mean=1.0, amp=1e-5)
+    g = pc.Lattice(N, L, 1, pc.FREE, [0.0], order=2, dt=dt, mpl=INF)
+    o = oracle.Oracle(N, L, 1, oracle.FREE, [0.0], order=2, dt=dt, mpl=INF)
+    zero = np.zeros_like(phi)
+    start(g, o, phi, zero, 1.0, 0.0)
+    D = o.laplacian(0)
+    g.step(1)
+    _, q = g.read_fields()
+    want = dt * D / (L / N) ** 2
+    # fluctuations are 1e-5 on a mean of 1: a weight-form sum would lose 5 digits here
+    assert np.max(np.abs(q[0] - want)) <= 1e-13 * np.max(np.abs(want))
+
+
+# ------------------------------------------------------------------------------------- invariants on the GPU
+def test_time_reversal_on_gpu(pc):
+    cfg = inputs.config("cfg0_chaotic32", N=24, dt=0.004)
+    phi, pi = inputs.make_initial(cfg)
+    g = pc.from_config(cfg)
+    g.set_fields(phi, pi)
+    g.set_background(1.0)
+    e0 = g.energies()
+    g.step(10)
+    g.set_dt(-cfg["dt"])
+    g.step(10)
+    p, q = g.read_fields()
+    assert rel_err_per_site(p, phi) < 1e-12 and rel_err_per_site(q, pi) < 1e-12
+    assert rel(g.energies().a, e0.a) < 1e-13
+
+
+def test_nonfinite_is_reported_and_sticky(pc):
+    cfg = inputs.config("cfg0_chaotic32", N=16)
+    phi, pi = inputs.make_initial(cfg)
+    bad = pi.copy()
+    bad[1, 3, 4, 5] = np.inf
+    g = pc.from_config(cfg)
+    g.set_fields(phi, bad)
+    g.set_background(1.0, -1.0e5)
+    g.step(1)
+    with pytest.raises(pc.PycoolError) as ei:
+        g.sync()
+    assert ei.value.code == pc.ENONFINITE
+    with pytest.raises(pc.PycoolError):
+        g.step(1)
+    g.set_fields(phi, pi)                                    # clears the flag
+    g.set_background(1.0)
+    g.step(1)
+    g.sync()
+
+
+def test_state_errors(pc):
+    g = pc.Lattice(8, 1.0, 1, pc.FREE, [1.0])
+    with pytest.raises(pc.PycoolError) as ei:
+        g.step(1)
+    assert ei.value.code == pc.ESTATE
+    with pytest.raises(pc.PycoolError):
+        g.set_background(-1.0, 0.0)
+
+
+# ------------------------------------------------------------------------------------- fp32 option
+def test_fp32_one_step(pc):
+    cfg = inputs.config("cfg0b_chaotic32_resolved", N=40)
+    cfg["amp"] = 1e-3
+    phi, pi = inputs.make_initial(cfg, precision=32)
+    g, o = make_pair(pc, cfg, precision=32)
+    start(g, o, phi, pi)
+    g.step(1); o.step(1)
+    pg, qg = g.read_fields()
+    po, qo = o.read_fields()
+    assert pg.dtype == np.float32
+    assert rel_err_per_site(pg, po) <= 1e-5 and rel_err_per_site(qg, qo) <= 1e-5
+    check_scalars(g.energies(), o.energies(), 2, tol=1e-5)
+
+
+# ------------------------------------------------------------------------------------- full size, bench config
+@pytest.mark.parametrize("N,base", [(512, 32)])
+def test_full_size_periodic_replication(pc, N, base):
+    """At BASELINE's 512^3 in the launch configuration bench.py times: the input is a base^3 lattice
+    replicated periodically; the method is translation-equivariant, so every output site must equal the
+    oracle's base^3 evolution of the same tile (sums scale with the volume, a is unchanged)."""
+    r = N // base
+    small = inputs.config("cfg4_chaotic512", N=base)
+    small["L"] = 10.0 * base / N                             # same dx and dt as the 512^3 configuration
+    small["dt"] = 10.0 / N / 20.0
+    phi_s, pi_s = inputs.make_initial(small)
+    big = inputs.config("cfg4_chaotic512", N=N)
+    g = pc.from_config(big)
+    o = oracle.Oracle(base, small["L"], 2, oracle.CHAOTIC, small["p"], order=4, dt=small["dt"], mpl=1.0)
+    g.set_fields(np.tile(phi_s, (1, r, r, r)), np.tile(pi_s, (1, r, r, r)))
+    g.set_background(1.0)
+    o.set_fields(phi_s, pi_s)
+    o.set_background(1.0)
+    g.step(2); o.step(2)
+    po, qo = o.read_fields()
+    pg, qg = g.read_fields()
+    eg, eo = g.energies(), o.energies()
+    assert rel(eg.a, eo.a) < 1e-12 and rel(eg.p_a / r ** 3, eo.p_a) < 1e-12
+    assert rel(eg.kin[0], eo.kin[0]) < 1e-10 and rel(eg.grad[1], eo.grad[1]) < 1e-10 and rel(eg.pot, eo.pot) < 1e-10
+    for arr_g, arr_o in ((pg, po), (qg, qo)):
+        worst = 0.0
+        for f in range(2):
+            rms = math.sqrt(float(np.mean(arr_o[f] ** 2)))
+            den = np.maximum(np.abs(arr_o[f]), rms)
+            blocks = arr_g[f].reshape(r, base, r, base, r, base)
+            for iz in range(r):                              # every replica, every site
+                d = np.abs(blocks[iz] - arr_o[f][:, None, :, None, :]) / den[:, None, :, None, :]
+                worst = max(worst, float(d.max()))
+        assert worst <= 2e-12, worst
