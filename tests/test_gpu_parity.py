@@ -106,9 +106,13 @@ def test_cfg0_paper_phi0_reading_g19(pc):
 
 
 # ------------------------------------------------------------------------------------- reduced-size cfg1-3
-@pytest.mark.parametrize("name,N,steps", [("cfg1_chaotic128", 48, 6), ("cfg2_oscillon256", 40, 20),
-                                          ("cfg3_qball256", 40, 20)])
-def test_models_reduced_size(pc, name, N, steps):
+# Tolerance after one step: a 1-ulp difference in phi' (merged vs separate half drifts, FMA) enters pi through
+# kD D, i.e. amplified by (|c0| + sum |c_d|) a^2 h/dx^2 ~ 8.5 * 1.35 dt/dx^2 per stage.  For cfg0-cfg2 that factor
+# is < 1 and 1e-12 holds; for the Q-ball lattice dt/dx^2 = 5.1 and |pi_1| ~ 1e-3 |phi_1|, so ulp(phi) 60/rms(pi)
+# ~ 1e-11 is the floor of ANY fp64 evaluation order there.
+@pytest.mark.parametrize("name,N,steps,tol1", [("cfg1_chaotic128", 48, 6, 1e-12), ("cfg2_oscillon256", 40, 20, 1e-12),
+                                               ("cfg3_qball256", 40, 20, 2e-11)])
+def test_models_reduced_size(pc, name, N, steps, tol1):
     cfg = inputs.config(name, N=N)
     if name == "cfg2_oscillon256":
         cfg["L"] = 400.0 * N / 256                          # keep dx of the full configuration
@@ -118,9 +122,9 @@ def test_models_reduced_size(pc, name, N, steps):
     g, o = make_pair(pc, cfg)
     start(g, o, phi, pi)
     g.step(1); o.step(1)
-    compare(g, o, cfg["nfields"], 1e-12)
+    compare(g, o, cfg["nfields"], tol1)
     g.step(steps - 1); o.step(steps - 1)
-    compare(g, o, cfg["nfields"], 1e-10)
+    compare(g, o, cfg["nfields"], 100 * tol1)
 
 
 # ------------------------------------------------------------------------------------- orders, tiles, chunks
