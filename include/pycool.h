@@ -92,22 +92,21 @@ typedef struct {
 int pycool_create(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
                   double dt);
 
-/* Bytes of device work memory pycool_create_ext needs for this lattice (0 if the arguments are invalid). */
+/* Bytes of device work memory pycool_create_ext needs for this lattice (0 if the arguments are invalid):
+ * both state buffers in the library's internal layout (ghost columns/rows for even N), partial sums, scalars. */
 size_t pycool_work_bytes(int N, int nfields, int precision);
 
-/* As pycool_create, on caller-owned device memory and stream (e.g. PyTorch tensors / torch stream):
- *   d_phi, d_pi : device, nf*N^3 elements each; the library reads and writes them (state buffer 0)
- *   d_work      : device, >= pycool_work_bytes(...) bytes, 256-byte aligned; state buffer 1, partial sums,
- *                 scalars
+/* As pycool_create, on caller-owned device memory and stream (e.g. a PyTorch tensor / torch stream):
+ *   d_work      : device, >= pycool_work_bytes(...) bytes, 256-byte aligned; holds the whole state
  *   cuda_stream : a cudaStream_t (NULL = the legacy default stream)
- * The caller keeps ownership; pycool_destroy frees none of them. */
+ * The caller keeps ownership; pycool_destroy frees neither. */
 int pycool_create_ext(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
-                      double dt, void* d_phi, void* d_pi, void* d_work, size_t work_bytes, void* cuda_stream);
+                      double dt, void* d_work, size_t work_bytes, void* cuda_stream);
 
-/* Upload phi and pi from host memory (H2D on the context stream, synchronous to the caller) and compute
- * sum pi^2 on the device.  Clears PYCOOL_ENONFINITE. */
+/* Upload phi and pi from dense host arrays [field][z][y][x] (H2D on the context stream, synchronous to the
+ * caller), write the periodic ghost images and compute sum pi^2 on the device.  Clears PYCOOL_ENONFINITE. */
 int pycool_set_fields(pycool_ctx*, const void* phi_host, const void* pi_host);
-/* Same from device memory (D2D on the context stream, asynchronous). */
+/* Same from dense device arrays (D2D on the context stream, asynchronous). */
 int pycool_set_fields_device(pycool_ctx*, const void* d_phi_src, const void* d_pi_src);
 
 /* Set a (> 0) and p_a.  p_a = NaN asks the library to solve the first Friedmann equation (2.18) on the
@@ -129,9 +128,14 @@ int pycool_sync(pycool_ctx*);
 /* Download phi and/or pi (either may be NULL) to host memory.  Synchronises. */
 int pycool_read_fields(pycool_ctx*, void* phi_host, void* pi_host);
 
-/* Device pointers of the current state arrays (they alternate between the two state buffers); valid until
- * the next pycool_step/set_fields.  Does not synchronise. */
-int pycool_device_fields(pycool_ctx*, void** d_phi, void** d_pi);
+/* Download into dense device arrays (either may be NULL).  D2D on the context stream, asynchronous. */
+int pycool_read_fields_device(pycool_ctx*, void* d_phi_dst, void* d_pi_dst);
+
+/* Device pointers of the current state arrays (they alternate between the two state buffers; valid until
+ * the next pycool_step/set_fields) and their layout: element (f, z, y, x) is at
+ *   ((f*N + z)*layout[1] + y + layout[3]) * layout[0] + x + layout[2]
+ * (layout = row pitch, rows per plane, ghost columns, ghost rows).  Does not synchronise. */
+int pycool_device_fields(pycool_ctx*, void** d_phi, void** d_pi, size_t layout[4]);
 
 /* Lattice sums of the current state (one stencil pass with G of (2.8)) -> rho, P, H, residual.
  * Synchronises. */
@@ -156,11 +160,14 @@ int pycool_set_profiling(pycool_ctx*, int on);
 /* Sum of the bracketed durations (ms) and their number since profiling was switched on.  Synchronises. */
 int pycool_kick_time_ms(pycool_ctx*, double* total_ms, unsigned long long* launches);
 /* Launch geometry of the fused kernel: tile[0..2] = TX, TY, z-chunk; tile[3] = threads per block;
- * tile[4] = blocks per launch; tile[5] = dynamic shared memory bytes. */
-int pycool_kick_geometry(const pycool_ctx*, int tile[6]);
+ * tile[4] = blocks per launch; tile[5] = dynamic shared memory bytes; tile[6] = variant index (pycool_set_tile);
+ * tile[7] = TMA ring stages (0 = the register-prefetch kernel). */
+int pycool_kick_geometry(const pycool_ctx*, int tile[8]);
 /* Override the z-chunk length (planes per block; 0 = automatic) before the next step. */
 int pycool_set_zchunk(pycool_ctx*, int planes);
-/* Select the x-y tile variant of the fused kernel: 0 = 32x8, 1 = 32x16, 2 = 64x16 sites; -1 = automatic. */
+/* Select the variant of the fused kernel; -1 = automatic.
+ *   0..2: register-prefetch kernel, tiles 32x8, 32x16, 64x16 sites (any N);
+ *   3..7: TMA-fed kernel (even N only, else PYCOOL_EINVAL), tiles 64x16, 32x16, 64x8, 32x32, 128x8. */
 int pycool_set_tile(pycool_ctx*, int tile);
 
 #if defined(__GNUC__)

@@ -19,7 +19,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENONFINITE = 0, 1, 2, 3, 4, 5
 # every symbol include/pycool.h declares (tests check the library exports exactly these)
 SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_set_fields",
            "pycool_set_fields_device", "pycool_set_background", "pycool_set_dt", "pycool_step", "pycool_sync",
-           "pycool_read_fields", "pycool_device_fields", "pycool_energies", "pycool_destroy",
+           "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile")
 
@@ -66,7 +66,7 @@ def lib():
         L.pycool_create.argtypes = [C.POINTER(vp), ip, d, ip, pp, ip, d]
         L.pycool_work_bytes.argtypes = [ip, ip, ip]
         L.pycool_work_bytes.restype = C.c_size_t
-        L.pycool_create_ext.argtypes = [C.POINTER(vp), ip, d, ip, pp, ip, d, vp, vp, vp, C.c_size_t, vp]
+        L.pycool_create_ext.argtypes = [C.POINTER(vp), ip, d, ip, pp, ip, d, vp, C.c_size_t, vp]
         L.pycool_set_fields.argtypes = [vp, vp, vp]
         L.pycool_set_fields_device.argtypes = [vp, vp, vp]
         L.pycool_set_background.argtypes = [vp, d, d]
@@ -74,7 +74,8 @@ def lib():
         L.pycool_step.argtypes = [vp, ip]
         L.pycool_sync.argtypes = [vp]
         L.pycool_read_fields.argtypes = [vp, vp, vp]
-        L.pycool_device_fields.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
+        L.pycool_read_fields_device.argtypes = [vp, vp, vp]
+        L.pycool_device_fields.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_size_t)]
         L.pycool_energies.argtypes = [vp, C.POINTER(Energy)]
         L.pycool_destroy.argtypes = [vp]
         L.pycool_last_error.argtypes = [vp]
@@ -136,16 +137,12 @@ class Lattice:
         need = work_bytes(N, nfields, self.precision)
         if need == 0:
             raise PycoolError(EINVAL, "invalid lattice shape")
-        shape = (nfields, N, N, N)
         with torch.cuda.device(self.device):
-            self._phi0 = torch.empty(shape, dtype=self._tdtype, device=self.device)
-            self._pi0 = torch.empty(shape, dtype=self._tdtype, device=self.device)
             self._work = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
             wptr = (self._work.data_ptr() + 255) // 256 * 256
             self.stream = torch.cuda.current_stream(self.device)
             st = lib().pycool_create_ext(C.byref(self._h), N, L, nfields, C.byref(self._mp), order, dt,
-                                         self._phi0.data_ptr(), self._pi0.data_ptr(), wptr, need,
-                                         self.stream.cuda_stream)
+                                         wptr, need, self.stream.cuda_stream)
         if st != OK:
             raise PycoolError(st, lib().pycool_last_error(None).decode())
 
@@ -194,21 +191,30 @@ class Lattice:
         self._chk(lib().pycool_read_fields(self._h, ptr(phi), ptr(pi)))
         return phi, pi
 
-    def device_fields(self):
-        """(phi, pi) as torch views [nf,N,N,N] of the CURRENT state buffers (no copy, no sync)."""
-        a, b = C.c_void_p(), C.c_void_p()
-        self._chk(lib().pycool_device_fields(self._h, C.byref(a), C.byref(b)))
-        return self._view(a.value), self._view(b.value)
+    def read_fields_device(self):
+        """(phi, pi) as new dense torch tensors [nf,N,N,N] on the device (D2D copy on the context stream)."""
+        torch = self._torch
+        shape = (self.nf, self.N, self.N, self.N)
+        phi = torch.empty(shape, dtype=self._tdtype, device=self.device)
+        pi = torch.empty(shape, dtype=self._tdtype, device=self.device)
+        self._chk(lib().pycool_read_fields_device(self._h, phi.data_ptr(), pi.data_ptr()))
+        return phi, pi
 
-    def _view(self, ptr):
-        n = self.nf * self.N ** 3
+    def device_fields(self):
+        """(phi, pi) as strided torch views [nf,N,N,N] of the CURRENT state buffers inside the work tensor (no
+        copy, no sync): the library's padded layout with the ghost columns/rows sliced away."""
+        a, b, lay = C.c_void_p(), C.c_void_p(), (C.c_size_t * 4)()
+        self._chk(lib().pycool_device_fields(self._h, C.byref(a), C.byref(b), lay))
+        pitch, rows, gx, gy = (int(v) for v in lay)
+        return self._view(a.value, pitch, rows, gx, gy), self._view(b.value, pitch, rows, gx, gy)
+
+    def _view(self, ptr, pitch, rows, gx, gy):
+        n = self.nf * self.N * rows * pitch
         esize = 4 if self.precision == 32 else 8
-        for base in (self._phi0, self._pi0):
-            if ptr == base.data_ptr():
-                return base
         off = ptr - self._work.data_ptr()
         assert 0 <= off and off + n * esize <= self._work.numel()
-        return self._work[off:off + n * esize].view(self._tdtype).view(self.nf, self.N, self.N, self.N)
+        full = self._work[off:off + n * esize].view(self._tdtype).view(self.nf, self.N, rows, pitch)
+        return full[:, :, gy:gy + self.N, gx:gx + self.N]
 
     def energies(self):
         e = Energy()
@@ -229,9 +235,10 @@ class Lattice:
         return ms.value, int(n.value)
 
     def kick_geometry(self):
-        t = (C.c_int * 6)()
+        t = (C.c_int * 8)()
         self._chk(lib().pycool_kick_geometry(self._h, t))
-        return dict(tx=t[0], ty=t[1], zchunk=t[2], threads=t[3], blocks=t[4], smem_bytes=t[5])
+        return dict(tx=t[0], ty=t[1], zchunk=t[2], threads=t[3], blocks=t[4], smem_bytes=t[5], variant=t[6],
+                    tma_stages=t[7])
 
     def set_zchunk(self, planes):
         self._chk(lib().pycool_set_zchunk(self._h, planes))

@@ -17,6 +17,48 @@
 
 namespace pycool {
 
+// ------------------------------------------------------------------------------------------------ layout
+// Field arrays in HBM: [field][z][y + gy][x + gx], x fastest, rows `pitch` elements apart, `rows` rows per
+// plane.  gx = gy = 0 is the plain N^3 layout.  With ghosts (gx = 16 bytes of elements, gy = 1) column x = -1
+// holds the periodic image of x = N-1, x = N that of x = 0, likewise rows y = -1 and y = N, so that a TMA box
+// with a one-site halo never leaves the array (kick_tma.cuh).  Every kernel that writes phi or pi keeps the
+// images equal to their sources.
+struct Layout {
+  int N;
+  int pitch, rows;
+  int gx, gy;
+  size_t plane;    // pitch * rows
+  size_t field;    // plane * N
+  size_t total;    // field * nf  (elements per array, padding included)
+  __host__ __device__ __forceinline__ size_t at(int f, int z, int y, int x) const {
+    return (size_t)f * field + (size_t)z * plane + (size_t)(y + gy) * pitch + (size_t)(x + gx);
+  }
+};
+
+// Store v at site (x, y) of the (field, z) plane starting at `plane_base`, and at its periodic images in the
+// ghost columns / rows.
+template <typename Real>
+__device__ __forceinline__ void store_site(Real* plane_base, const Layout& L, int x, int y, Real v) {
+  Real* p = plane_base + (size_t)(y + L.gy) * L.pitch + (x + L.gx);
+  *p = v;
+  if (L.gx == 0) return;
+  const bool xl = x < L.gx, xh = x >= L.N - L.gx, yl = y < L.gy, yh = y >= L.N - L.gy;
+  if (!(xl | xh | yl | yh)) return;
+  const long long dy = (long long)L.N * L.pitch;
+  if (xl) p[L.N] = v;
+  if (xh) p[-L.N] = v;
+  if (yl) {
+    p[dy] = v;
+    if (xl) p[dy + L.N] = v;
+    if (xh) p[dy - L.N] = v;
+  }
+  if (yh) {
+    p[-dy] = v;
+    if (xl) p[-dy + L.N] = v;
+    if (xh) p[-dy - L.N] = v;
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ scalars
 struct Scalars {          // device-resident; one per context
   double a, p_a;
@@ -145,7 +187,7 @@ struct KickArgs {
   Real* pi_out;
   const Scalars* sc;
   double* partials;      // [3][nblocks]: SD, SV, Spi2
-  int N;
+  Layout L;
   int zc;                // planes per z-chunk
   double c1, c2, c3;     // stencil weights by neighbour class (c0 = -(6c1+12c2+8c3))
   ModelParams mp;
@@ -186,8 +228,9 @@ kick_fused(const KickArgs<Real> g) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Real* sm = reinterpret_cast<Real*>(smem_raw);          // [2][NF][TY+2][PX]
 
-  const int N = g.N;
-  const size_t V = (size_t)N * N * N;
+  const Layout& L = g.L;
+  const int N = L.N;
+  const size_t V = L.field;
   const int tid = threadIdx.x;
   const int tx = tid % TX, ty = tid / TX;
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * g.zc;
@@ -200,7 +243,7 @@ kick_fused(const KickArgs<Real> g) {
 
   Real ref[NF];
 #pragma unroll
-  for (int f = 0; f < NF; ++f) ref[f] = g.phi_in[f * V + ((size_t)z0 * N + y0) * N + x0];
+  for (int f = 0; f < NF; ++f) ref[f] = g.phi_in[L.at(f, z0, y0, x0)];
 
   // own sites
   const int gx = x0 + tx;
@@ -210,7 +253,7 @@ kick_fused(const KickArgs<Real> g) {
   for (int j = 0; j < K; ++j) {
     const int ly = ty * K + j;
     valid[j] = (tx < wx) && (ly < wy);
-    own_off[j] = (size_t)(y0 + ly) * N + gx;
+    own_off[j] = (size_t)(y0 + ly + L.gy) * L.pitch + gx + L.gx;
   }
   // halo site of this thread (ring of the (wy+2) x (wx+2) smem tile)
   const int nh = 2 * (wx + 2) + 2 * wy;
@@ -226,7 +269,7 @@ kick_fused(const KickArgs<Real> g) {
     int hx = x0 - 1 + hsx, hy = y0 - 1 + hsy;              // periodic wrap
     hx = hx < 0 ? hx + N : (hx >= N ? hx - N : hx);
     hy = hy < 0 ? hy + N : (hy >= N ? hy - N : hy);
-    halo_off = (size_t)hy * N + hx;
+    halo_off = (size_t)(hy + L.gy) * L.pitch + hx + L.gx;
   }
 
   Real rphi[NF][K], rpi[NF][K], hphi[NF], hpi[NF];         // loads in flight (plane p+1)
@@ -242,7 +285,7 @@ kick_fused(const KickArgs<Real> g) {
   auto zplane = [&](int p) -> size_t {
     int gz = z0 + p;
     gz = gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
-    return (size_t)gz * N * N;
+    return (size_t)gz * L.plane;
   };
   auto load = [&](int p) {
     const size_t zp = zplane(p);
@@ -280,7 +323,7 @@ kick_fused(const KickArgs<Real> g) {
         const Real ph = fma(cd, rpi[f][j], rphi[f][j]);     // phi' = phi + c_drift pi
         cphi[f][j] = ph; cpi[f][j] = rpi[f][j];
         if (valid[j]) {
-          if (own_plane) g.phi_out[f * V + zp + own_off[j]] = ph;
+          if (own_plane) store_site(g.phi_out + f * V + zp, L, gx, y0 + ty * K + j, ph);
           buf[f * T::PLANE + (ty * K + j + 1) * PX + tx + 1] = ph - ref[f];
         }
       }
@@ -325,7 +368,7 @@ kick_fused(const KickArgs<Real> g) {
 #pragma unroll
           for (int f = 0; f < NF; ++f) {
             const Real pn = fma(kD, D[f][j], fma(-kV, dV[f], ppi[f][j]));   // pi' = pi + kD D - kV dV
-            g.pi_out[f * V + zq + own_off[j]] = pn;
+            store_site(g.pi_out + f * V + zq, L, gx, y0 + ty * K + j, pn);
             sD = fma((double)ph[f], (double)D[f][j], sD);
             sP = fma((double)pn, (double)pn, sP);
           }
@@ -352,7 +395,8 @@ kick_fused(const KickArgs<Real> g) {
 }
 
 // ------------------------------------------------------------------------------------------------ pointwise
-// Closing half drift of a pycool_step call: phi += c_drift pi, in place.
+// Closing half drift of a pycool_step call: phi += c_drift pi, in place, over the whole padded array (ghost
+// images of pi equal their sources, so the images of phi stay equal too).
 template <typename Real>
 __global__ void __launch_bounds__(256) drift_flush(Real* __restrict__ phi, const Real* __restrict__ pi,
                                                    const Scalars* __restrict__ sc, size_t n) {
@@ -362,14 +406,40 @@ __global__ void __launch_bounds__(256) drift_flush(Real* __restrict__ phi, const
     phi[i] = fma(cd, pi[i], phi[i]);
 }
 
-// sum of squares -> per-block partials (fixed assignment of elements to threads, fixed-order block reduce)
+// Periodic images into the ghost columns / rows of one array (after an upload).  One thread per padded site.
 template <typename Real>
-__global__ void __launch_bounds__(256) sumsq(const Real* __restrict__ v, size_t n, double* __restrict__ partials) {
-  __shared__ double sh[8];
-  double acc[1] = {0.0};
+__global__ void __launch_bounds__(256) fill_ghosts(Real* __restrict__ v, Layout L, int nf) {
+  const int W = L.N + 2 * L.gx, H = L.N + 2 * L.gy;
+  const size_t per_plane = (size_t)W * H, n = per_plane * L.N * nf;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const double x = (double)v[i];
+    const size_t pl = i / per_plane;                       // f * N + z
+    const int r = (int)(i - pl * per_plane);
+    const int y = r / W - L.gy, x = r % W - L.gx;
+    if (x >= 0 && x < L.N && y >= 0 && y < L.N) continue;
+    int sx = x < 0 ? x + L.N : (x >= L.N ? x - L.N : x);
+    int sy = y < 0 ? y + L.N : (y >= L.N ? y - L.N : y);
+    sx = sx < 0 ? sx + L.N : (sx >= L.N ? sx - L.N : sx);  // N < gx (tiny lattices): wrap twice
+    Real* base = v + pl * L.plane;
+    base[(size_t)(y + L.gy) * L.pitch + (x + L.gx)] = base[(size_t)(sy + L.gy) * L.pitch + (sx + L.gx)];
+  }
+}
+
+// sum of squares over the lattice sites (ghosts excluded) -> per-block partials (fixed assignment of elements
+// to threads, fixed-order block reduce)
+template <typename Real>
+__global__ void __launch_bounds__(256) sumsq(const Real* __restrict__ v, Layout L, int nf,
+                                             double* __restrict__ partials) {
+  __shared__ double sh[8];
+  double acc[1] = {0.0};
+  const size_t n = (size_t)L.N * L.N * L.N * nf;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const size_t row = i / L.N;                            // (f * N + z) * N + y
+    const int xx = (int)(i - row * L.N);
+    const size_t pl = row / L.N;
+    const int yy = (int)(row - pl * L.N);
+    const double x = (double)v[pl * L.plane + (size_t)(yy + L.gy) * L.pitch + (xx + L.gx)];
     acc[0] = fma(x, x, acc[0]);
   }
   block_reduce<1, 256>(acc, sh);
@@ -399,10 +469,11 @@ __global__ void set_scalars(Scalars* sc, double a, double p_a, int set_pa) {
 // partials: [3 NF + 1][gridDim.x]
 template <typename Real, class Model>
 __global__ void __launch_bounds__(256)
-energy_sums(const Real* __restrict__ phi, const Real* __restrict__ pi, int N, double c1, double c2, double c3,
+energy_sums(const Real* __restrict__ phi, const Real* __restrict__ pi, Layout L, double c1, double c2, double c3,
             ModelParams mp, double* __restrict__ partials) {
   constexpr int NF = Model::NF, NQ = 3 * NF + 1;
   __shared__ double sh[NQ * 8];
+  const int N = L.N;
   const size_t V = (size_t)N * N * N;
   const typename Model::template Coef<double> coef(mp);
   const double cw[4] = {0.0, c1, c2, c3};
@@ -418,8 +489,9 @@ energy_sums(const Real* __restrict__ phi, const Real* __restrict__ pi, int N, do
     double ph[NF], dV[NF];
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
-      const Real* pf = phi + f * V;
-      const double ctr = (double)pf[i];
+      const Real* pf = phi + f * L.field;
+      const size_t ic = L.at(0, z, y, x);
+      const double ctr = (double)pf[ic];
       double s[4] = {0, 0, 0, 0}, q2[4] = {0, 0, 0, 0};
 #pragma unroll
       for (int dz = 0; dz < 3; ++dz)
@@ -429,13 +501,13 @@ energy_sums(const Real* __restrict__ phi, const Real* __restrict__ pi, int N, do
           for (int dx = 0; dx < 3; ++dx) {
             const int d = (dx != 1) + (dy != 1) + (dz != 1);
             if (d == 0) continue;
-            const double df = (double)pf[((size_t)zs[dz] * N + ys[dy]) * N + xs[dx]] - ctr;
+            const double df = (double)pf[L.at(0, zs[dz], ys[dy], xs[dx])] - ctr;
             s[d] += df;
             q2[d] = fma(df, df, q2[d]);
           }
       const double Dv = cw[1] * s[1] + cw[2] * s[2] + cw[3] * s[3];
       const double Gv = 0.5 * (cw[1] * q2[1] + cw[2] * q2[2] + cw[3] * q2[3]);
-      const double pv = (double)pi[f * V + i];
+      const double pv = (double)pi[f * L.field + ic];
       acc[3 * f] = fma(pv, pv, acc[3 * f]);
       acc[3 * f + 1] += Gv;
       acc[3 * f + 2] = fma(ctr, Dv, acc[3 * f + 2]);

@@ -1,0 +1,331 @@
+// kick_tma.cuh -- the fused drift + kick + lattice-sum stage of (2.47)-(2.48) as a TMA-fed z-march (sm_100a).
+//
+// Same arithmetic as kick_fused (kernels.cuh): per stage phi' = phi + c_drift pi, D = stencil (2.7) of phi',
+// pi' = pi + kD D - kV dV/dphi(phi'), and the three sums of PAPER.md:327-331, 399.  What differs is how the
+// planes reach the SM: one elected thread issues two 4-D tensor-map bulk copies (cp.async.bulk.tensor, SASS
+// UTMALDG) per z-plane -- the (TX + 2G) x (TY + 2) x NF box of phi and of pi, halo included -- into a ring of
+// S shared-memory stages that complete on mbarriers.  The loads in flight therefore live in shared memory, not
+// in registers, and their depth (S - 1 planes ahead) is independent of occupancy.
+//
+// TMA boxes cannot wrap around a periodic lattice (out-of-bounds elements are zero-filled), so the arrays carry
+// ghost images in x and y (Layout, kernels.cuh): every block writes, next to each output on a lattice face, its
+// periodic image(s) into the ghost columns / rows of the output buffer, which the next stage then reads as plain
+// in-bounds box elements.  z wraps through the box coordinate (one plane per box).  DESIGN.md "TMA path".
+//
+// Thread (tx2, ty2) owns the 2 x 2 sites x = 2 tx2 + {0,1}, y = 2 ty2 + {0,1} of the tile for all NF fields.
+#pragma once
+#include <cuda.h>
+
+#include "kernels.cuh"
+
+namespace pycool {
+
+template <typename Real> struct Vec2T;
+template <> struct Vec2T<double> { using type = double2; };
+template <> struct Vec2T<float> { using type = float2; };
+
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+// 4-D tiled tensor-map load global -> shared, completion on an mbarrier (bytes of the whole box)
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2,
+                                            int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::
+          "r"(dst),
+      "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
+
+template <typename Real, int TX_, int TY_, int S_>
+struct TmaTile {
+  static constexpr int TX = TX_, TY = TY_, S = S_;
+  static constexpr int G = 16 / (int)sizeof(Real);      // box halo / ghost columns on each side (16 bytes)
+  static constexpr int PX = TX + 2 * G;                 // box row length
+  static constexpr int RY = TY + 2;                     // box rows
+  static constexpr int PLANE = PX * RY;                 // box elements per field
+  static constexpr int NT = (TX / 2) * (TY / 2);        // threads: 2 x 2 sites each
+  static constexpr int NH = 2 * (TX + 2) + 2 * TY;      // ring of halo sites the stencil reads
+  static_assert(TX % 2 == 0 && TY % 2 == 0, "2 x 2 sites per thread");
+  static_assert(NT % 32 == 0 && NT <= 1024, "block size");
+  static_assert(PX <= 256 && RY <= 256, "TMA box extents");
+};
+
+template <typename Real, class Model, class T>
+struct TmaSmem {
+  static constexpr size_t BOX = (size_t)Model::NF * T::PLANE * sizeof(Real);   // bytes one bulk copy delivers
+  static constexpr size_t BOXA = (BOX + 127) / 128 * 128;                      // 128-byte aligned slot
+  static constexpr size_t RAW = (size_t)T::S * 2 * BOXA;                       // ring: [S][phi, pi]
+  static constexpr size_t PSI = 2 * BOXA;                                      // double-buffered psi planes
+  static constexpr size_t BARS = 128;                                          // S mbarriers
+  static constexpr size_t TOTAL = RAW + PSI + BARS + 128;                      // + slack to align the base
+  static_assert(3 * (T::NT / 32) * sizeof(double) <= PSI, "reduction scratch fits in the psi buffers");
+};
+
+template <typename Real>
+struct TmaArgs {
+  Real* phi_out;
+  Real* pi_out;
+  const Real* phi_in;     // read directly only for the block's reference values
+  const Scalars* sc;
+  double* partials;       // [3][nblocks]: SD, SV, Spi2
+  Layout L;
+  int zc;                 // planes per z-chunk
+  double c1, c2, c3;
+  ModelParams mp;
+};
+
+template <typename Real, class Model, class T>
+__global__ void __launch_bounds__(T::NT)
+kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_pi,
+         const TmaArgs<Real> g) {
+  using R2 = typename Vec2T<Real>::type;
+  using SM = TmaSmem<Real, Model, T>;
+  constexpr int NF = Model::NF, TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT;
+  constexpr int PLANE = T::PLANE;
+
+  extern __shared__ unsigned char smem_dyn[];
+  unsigned char* base = smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u);
+  unsigned char* raw = base;                                   // [S][2][BOXA]
+  Real* psi = reinterpret_cast<Real*>(base + SM::RAW);         // [2][BOXA]
+  const uint32_t bars = smem_addr(base + SM::RAW + SM::PSI);   // S x 8 bytes
+
+  const Layout& L = g.L;
+  const int N = L.N;
+  const int tid = threadIdx.x;
+  const int tx2 = tid % (TX / 2), ty2 = tid / (TX / 2);
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * g.zc;
+  const int nz = min(g.zc, N - z0);
+  const int nload = nz + 2;                                    // planes z0-1 .. z0+nz
+
+  auto zwrap = [&](int p) {
+    int gz = z0 + p;
+    return gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+  };
+  auto issue = [&](int i) {                                    // load index i <-> plane p = i - 1
+    const int s = i % S;
+    const uint32_t bar = bars + 8u * s;
+    const uint32_t dst = smem_addr(raw + (size_t)s * 2 * SM::BOXA);
+    mbar_expect_tx(bar, (uint32_t)(2 * SM::BOX));
+    const int gz = zwrap(i - 1);
+    tma_load_4d(dst, &tm_phi, bar, x0, y0, gz, 0);             // box origin (x0-G, y0-1) in padded coordinates
+    tma_load_4d(dst + (uint32_t)SM::BOXA, &tm_pi, bar, x0, y0, gz, 0);
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) mbar_init(bars + 8u * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    for (int i = 0; i < S && i < nload; ++i) issue(i);
+  }
+
+  const Real cd = Real(g.sc->c_drift), kD = Real(g.sc->kD), kV = Real(g.sc->kV);
+  const Real c1 = Real(g.c1), c2 = Real(g.c2), c3 = Real(g.c3);
+  const Real c0 = -(Real(6) * c1 + Real(12) * c2 + Real(8) * c3);
+  const typename Model::template Coef<Real> coef(g.mp);
+  Real ref[NF];                                                // block-uniform; D annihilates constants
+#pragma unroll
+  for (int f = 0; f < NF; ++f) ref[f] = __ldg(g.phi_in + L.at(f, z0, y0, x0));
+
+  // own sites: global x pair and rows; ghost images (periodic copies on the x / y faces)
+  const int gx = x0 + 2 * tx2;
+  const bool okx = gx < N;
+  int ximg = 0;                                                // element offset of the x image, 0 = none
+  if (gx < L.gx) ximg = N; else if (gx >= N - L.gx) ximg = -N;
+  const bool ximg2 = (gx < L.gx) && (gx >= N - L.gx);          // both images (N <= 2 gx only)
+  bool valid[2];
+  size_t own_off[2];                                           // offset within a (field, z) plane
+  long long yimg[2];                                           // offset of the y image, 0 = none
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const int gy = y0 + 2 * ty2 + j;
+    valid[j] = okx && gy < N;
+    own_off[j] = (size_t)(gy + L.gy) * L.pitch + (gx + L.gx);
+    yimg[j] = 0;
+    if (gy == 0) yimg[j] = (long long)N * L.pitch; else if (gy == N - 1) yimg[j] = -(long long)N * L.pitch;
+    if (N == 1) yimg[j] = 0;
+  }
+  auto store2 = [&](Real* plane, int j, R2 v) {                // one output pair and its periodic images
+    Real* p = plane + own_off[j];
+    *reinterpret_cast<R2*>(p) = v;
+    if (ximg | (yimg[j] != 0)) {
+      if (ximg) {
+        *reinterpret_cast<R2*>(p + ximg) = v;
+        if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
+      }
+      if (yimg[j]) {
+        *reinterpret_cast<R2*>(p + yimg[j]) = v;
+        if (ximg) {
+          *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
+          if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
+        }
+      }
+    }
+  };
+
+  // box offsets: own pair (row j) and the halo ring site(s) of this thread
+  const int own_sm = (2 * ty2 + 1) * PX + G + 2 * tx2;
+  constexpr int NHT = (T::NH + NT - 1) / NT;                   // halo sites per thread (1 or 2)
+  int halo_sm[NHT];
+#pragma unroll
+  for (int k = 0; k < NHT; ++k) {
+    const int h = tid + k * NT;
+    int row, col;
+    if (h < TX + 2) { row = 0; col = G - 1 + h; }
+    else if (h < 2 * (TX + 2)) { row = TY + 1; col = G - 1 + h - (TX + 2); }
+    else { const int r = h - 2 * (TX + 2); row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 1; }
+    halo_sm[k] = h < T::NH ? row * PX + col : -1;
+  }
+
+  R2 pphi[NF][2], ppi[NF][2];                                  // phi', pi of plane p-1 (to be finalised)
+  R2 A[NF][2], B[NF][2];                                       // stencil accumulators
+  double sD = 0.0, sV = 0.0, sP = 0.0;
+#pragma unroll
+  for (int f = 0; f < NF; ++f)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      A[f][j] = B[f][j] = pphi[f][j] = ppi[f][j] = R2{Real(0), Real(0)};
+    }
+
+  __syncthreads();                                             // barriers initialised before anyone waits
+
+#pragma unroll 1
+  for (int p = -1; p <= nz; ++p) {
+    const int i = p + 1, s = i % S;
+    const Real* rphi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA);
+    const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
+    Real* pb = psi + (size_t)(i & 1) * (SM::BOXA / sizeof(Real));
+    mbar_wait(bars + 8u * s, (uint32_t)((i / S) & 1));
+
+    // ---- 1. drift: phi' = phi + c_drift pi (own pairs and halo ring); psi = phi' - ref to shared memory
+    const bool own_plane = (p >= 0) && (p < nz);
+    const size_t zoff = (size_t)zwrap(p) * L.plane;
+    R2 cphi[NF][2], cpi[NF][2];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int o = f * PLANE + own_sm + j * PX;
+        const R2 a = *reinterpret_cast<const R2*>(rphi + o);
+        const R2 b = *reinterpret_cast<const R2*>(rpi + o);
+        R2 ph;
+        ph.x = fma(cd, b.x, a.x);
+        ph.y = fma(cd, b.y, a.y);
+        cphi[f][j] = ph; cpi[f][j] = b;
+        if (own_plane && valid[j]) store2(g.phi_out + f * L.field + zoff, j, ph);
+        *reinterpret_cast<R2*>(pb + o) = R2{ph.x - ref[f], ph.y - ref[f]};
+      }
+#pragma unroll
+      for (int k = 0; k < NHT; ++k)
+        if (halo_sm[k] >= 0) {
+          const int o = f * PLANE + halo_sm[k];
+          pb[o] = fma(cd, rpi[o], rphi[o]) - ref[f];
+        }
+    }
+    __syncthreads();                                           // psi plane complete; raw stage s consumed
+    if (tid == 0 && i + S < nload) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      issue(i + S);
+    }
+
+    // ---- 2. in-plane sums of plane p; 3. finalise plane p-1
+    R2 D[NF][2];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const Real* sp = pb + f * PLANE + own_sm - PX;           // row above the first own row
+      Real Rx[4], Cx[4], Ry[4], Cy[4];                         // x-output 0 and 1: side sums and centres
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const Real l = sp[r * PX - 1];
+        const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
+        const Real rr = sp[r * PX + 2];
+        Rx[r] = l + m.y; Cx[r] = m.x;
+        Ry[r] = m.x + rr; Cy[r] = m.y;
+      }
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        {
+          const Real P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
+          const Real up = c1 * P0 + c2 * P1 + c3 * P2;         // weight of plane p in outputs p-1 and p+1
+          const Real mid = c0 * P0 + c1 * P1 + c2 * P2;        // weight of plane p in output p
+          D[f][j].x = A[f][j].x + up;
+          A[f][j].x = B[f][j].x + mid;
+          B[f][j].x = up;
+        }
+        {
+          const Real P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
+          const Real up = c1 * P0 + c2 * P1 + c3 * P2;
+          const Real mid = c0 * P0 + c1 * P1 + c2 * P2;
+          D[f][j].y = A[f][j].y + up;
+          A[f][j].y = B[f][j].y + mid;
+          B[f][j].y = up;
+        }
+      }
+    }
+    if (p >= 1) {
+      const size_t zq = (size_t)zwrap(p - 1) * L.plane;
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        if (valid[j]) {
+          Real ph[NF], dV[NF];
+          R2 pn[NF];
+#pragma unroll
+          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].x;
+          sV += (double)Model::template eval<Real>(coef, ph, dV);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            pn[f].x = fma(kD, D[f][j].x, fma(-kV, dV[f], ppi[f][j].x));   // pi' = pi + kD D - kV dV
+            sD = fma((double)ph[f], (double)D[f][j].x, sD);
+            sP = fma((double)pn[f].x, (double)pn[f].x, sP);
+          }
+#pragma unroll
+          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].y;
+          sV += (double)Model::template eval<Real>(coef, ph, dV);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            pn[f].y = fma(kD, D[f][j].y, fma(-kV, dV[f], ppi[f][j].y));
+            sD = fma((double)ph[f], (double)D[f][j].y, sD);
+            sP = fma((double)pn[f].y, (double)pn[f].y, sP);
+            store2(g.pi_out + f * L.field + zq, j, pn[f]);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int f = 0; f < NF; ++f)
+#pragma unroll
+      for (int j = 0; j < 2; ++j) { pphi[f][j] = cphi[f][j]; ppi[f][j] = cpi[f][j]; }
+  }
+
+  // ---- per-block partial sums, fixed order
+  __syncthreads();
+  double v[3] = {sD, sV, sP};
+  block_reduce<3, NT>(v, reinterpret_cast<double*>(psi));
+  if (tid == 0) {
+    const size_t nb = (size_t)gridDim.x * gridDim.y * gridDim.z;
+    const size_t b = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    g.partials[b] = v[0];
+    g.partials[nb + b] = v[1];
+    g.partials[2 * nb + b] = v[2];
+  }
+}
+
+}  // namespace pycool

@@ -16,10 +16,12 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "../../include/pycool.h"
 #include "kernels.cuh"
+#include "kick_tma.cuh"
 
 using namespace pycool;
 
@@ -54,9 +56,14 @@ int stage_weights_ld(int order, long double* w) {
 }
 
 constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
-constexpr int kNumTiles = 3;
+constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
+constexpr int kNumTiles = 8;             // + kick_tma variants (ghost layout only)
 
-struct TileInfo { int tx, ty, k, nt; };
+struct TileInfo { int tx, ty, nt, stages; };   // stages > 0: TMA ring depth
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 }  // namespace
 
@@ -69,10 +76,12 @@ struct pycool_ctx {
   ScalarConst kc{};
   int nstages = 0;
   double w[16];
-  // device memory
+  // device memory: two state buffers (ping-pong), each phi and pi in layout L
+  Layout lay{};
   void* phi[2] = {nullptr, nullptr};
   void* pi[2] = {nullptr, nullptr};
   int cur = 0;
+  CUtensorMap tm[2][2];         // [buffer][phi, pi] for the current TMA tile
   double* partials = nullptr;   // max(3 * kick blocks, 13 * kMaxSumBlocks) doubles
   size_t partials_cap = 0;
   double* sums = nullptr;       // 16 doubles: reduced rows
@@ -115,12 +124,45 @@ int fail(pycool_ctx* c, int code, const char* fmt, ...) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-const TileInfo kTiles[kNumTiles] = {{32, 8, 2, 128}, {32, 16, 2, 256}, {64, 16, 2, 512}};
+//                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
+const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
+                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 8, 128, 4}, {32, 32, 256, 3},
+                                    {128, 8, 256, 3}};
 using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 16, 2>;
+template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3>;
+template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3>;
+template <typename Real> using TTile5 = TmaTile<Real, 64, 8, 4>;
+template <typename Real> using TTile6 = TmaTile<Real, 32, 32, 3>;
+template <typename Real> using TTile7 = TmaTile<Real, 128, 8, 3>;
 
-int auto_tile(int N) { return N <= 64 ? 0 : 1; }
+// Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
+Layout make_layout(int N, int nf, size_t esize) {
+  Layout L{};
+  L.N = N;
+  if (N % 2 == 0 && N >= 4) {
+    L.gx = (int)(16 / esize);
+    L.gy = 1;
+    L.pitch = (int)align_up((size_t)N + 2 * L.gx, 32 / esize);     // rows start on 32-byte sectors
+    L.rows = N + 2;
+  } else {
+    L.gx = L.gy = 0;
+    L.pitch = N;
+    L.rows = N;
+  }
+  L.plane = (size_t)L.pitch * L.rows;
+  L.field = L.plane * N;
+  L.total = L.field * nf;
+  return L;
+}
+
+bool tile_allowed(const Layout& L, int tile) { return tile < kNumGeneric || L.gx > 0; }
+
+int auto_tile(const Layout& L) {
+  if (L.gx > 0) return L.N <= 64 ? 4 : 3;
+  return L.N <= 64 ? 0 : 1;
+}
 
 int blocks_xy(int N, int tile) {
   const TileInfo& t = kTiles[tile];
@@ -144,20 +186,62 @@ size_t partials_capacity(int N) {
   return m;
 }
 
-size_t work_layout(int N, int nf, size_t esize, size_t* off_phi1, size_t* off_pi1, size_t* off_part,
-                   size_t* off_sums, size_t* off_sc) {
-  const size_t bytes = align_up((size_t)nf * N * N * N * esize, 256);
-  size_t o = 0;
-  *off_phi1 = o; o += bytes;
-  *off_pi1 = o; o += bytes;
-  *off_part = o; o += align_up(partials_capacity(N) * sizeof(double), 256);
-  *off_sums = o; o += 256;
-  *off_sc = o; o += 256;
-  return o;
+// work memory: [phi0][pi0][phi1][pi1][partials][sums][scalars]
+struct WorkLayout { size_t arr, off_part, off_sums, off_sc, total; };
+WorkLayout work_layout(int N, int nf, size_t esize) {
+  WorkLayout w;
+  const Layout L = make_layout(N, nf, esize);
+  w.arr = align_up(L.total * esize, 256);
+  size_t o = 4 * w.arr;
+  w.off_part = o; o += align_up(partials_capacity(N) * sizeof(double), 256);
+  w.off_sums = o; o += 256;
+  w.off_sc = o; o += 256;
+  w.total = o;
+  return w;
 }
 
 bool valid_shape(int N, int nf, int precision) {
   return N >= 3 && N <= 2048 && nf >= 1 && nf <= 4 && (precision == 0 || precision == 32 || precision == 64);
+}
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+    else
+      cudaGetLastError();
+  }
+  return fn;
+}
+
+// Tensor map over one padded array: dims (x: N + 2 gx, y: N + 2 gy, z: N, f: nf), box (TX + 2 gx, TY + 2, 1, nf)
+int encode_maps(pycool_ctx* c) {
+  const TileInfo& t = kTiles[c->tile];
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return fail(c, PYCOOL_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  const Layout& L = c->lay;
+  const cuuint64_t dims[4] = {(cuuint64_t)(L.N + 2 * L.gx), (cuuint64_t)(L.N + 2 * L.gy), (cuuint64_t)L.N,
+                              (cuuint64_t)c->nf};
+  const cuuint64_t strides[3] = {(cuuint64_t)L.pitch * c->esize, (cuuint64_t)L.plane * c->esize,
+                                 (cuuint64_t)L.field * c->esize};
+  const cuuint32_t box[4] = {(cuuint32_t)(t.tx + 2 * L.gx), (cuuint32_t)(t.ty + 2), 1u, (cuuint32_t)c->nf};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const CUtensorMapDataType dt = c->precision == 32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+  for (int b = 0; b < 2; ++b)
+    for (int a = 0; a < 2; ++a) {
+      void* ptr = a == 0 ? c->phi[b] : c->pi[b];
+      CUresult r = enc(&c->tm[b][a], dt, 4, ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) return fail(c, PYCOOL_ECUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    }
+  return PYCOOL_OK;
 }
 
 // ---- kernel dispatch: <precision, model, nf, tile> -> template instance ----
@@ -177,11 +261,34 @@ int launch_kick_t(pycool_ctx* c) {
   g.pi_out = (Real*)c->pi[c->cur ^ 1];
   g.sc = c->sc;
   g.partials = c->partials;
-  g.N = c->N;
+  g.L = c->lay;
   g.zc = c->zc;
   g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
   g.mp = c->mp;
   kick_fused<Real, Model, T><<<c->grid, T::NT, smem, c->stream>>>(g);
+  CUDA_TRY(c, cudaGetLastError());
+  return PYCOOL_OK;
+}
+template <typename Real, class Model, class T>
+int launch_tma_t(pycool_ctx* c) {
+  static bool attr_done = false;
+  constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
+  if (!attr_done) {
+    CUDA_TRY(c, cudaFuncSetAttribute(kick_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)smem));
+    attr_done = true;
+  }
+  TmaArgs<Real> g;
+  g.phi_in = (const Real*)c->phi[c->cur];
+  g.phi_out = (Real*)c->phi[c->cur ^ 1];
+  g.pi_out = (Real*)c->pi[c->cur ^ 1];
+  g.sc = c->sc;
+  g.partials = c->partials;
+  g.L = c->lay;
+  g.zc = c->zc;
+  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
+  g.mp = c->mp;
+  kick_tma<Real, Model, T><<<c->grid, T::NT, smem, c->stream>>>(c->tm[c->cur][0], c->tm[c->cur][1], g);
   CUDA_TRY(c, cudaGetLastError());
   return PYCOOL_OK;
 }
@@ -190,7 +297,12 @@ int launch_kick_m(pycool_ctx* c) {
   switch (c->tile) {
     case 0: return launch_kick_t<Real, Model, Tile0>(c);
     case 1: return launch_kick_t<Real, Model, Tile1>(c);
-    default: return launch_kick_t<Real, Model, Tile2>(c);
+    case 2: return launch_kick_t<Real, Model, Tile2>(c);
+    case 3: return launch_tma_t<Real, Model, TTile3<Real>>(c);
+    case 4: return launch_tma_t<Real, Model, TTile4<Real>>(c);
+    case 5: return launch_tma_t<Real, Model, TTile5<Real>>(c);
+    case 6: return launch_tma_t<Real, Model, TTile6<Real>>(c);
+    default: return launch_tma_t<Real, Model, TTile7<Real>>(c);
   }
 }
 template <typename Real, class Model>
@@ -198,13 +310,18 @@ size_t kick_smem_m(int tile) {
   switch (tile) {
     case 0: return kick_smem_bytes<Real, Model, Tile0>();
     case 1: return kick_smem_bytes<Real, Model, Tile1>();
-    default: return kick_smem_bytes<Real, Model, Tile2>();
+    case 2: return kick_smem_bytes<Real, Model, Tile2>();
+    case 3: return TmaSmem<Real, Model, TTile3<Real>>::TOTAL;
+    case 4: return TmaSmem<Real, Model, TTile4<Real>>::TOTAL;
+    case 5: return TmaSmem<Real, Model, TTile5<Real>>::TOTAL;
+    case 6: return TmaSmem<Real, Model, TTile6<Real>>::TOTAL;
+    default: return TmaSmem<Real, Model, TTile7<Real>>::TOTAL;
   }
 }
 template <typename Real, class Model>
 int launch_energy_m(pycool_ctx* c, int nb) {
   energy_sums<Real, Model><<<nb, 256, 0, c->stream>>>((const Real*)c->phi[c->cur], (const Real*)c->pi[c->cur],
-                                                      c->N, c->c[1], c->c[2], c->c[3], c->mp, c->partials);
+                                                      c->lay, c->c[1], c->c[2], c->c[3], c->mp, c->partials);
   CUDA_TRY(c, cudaGetLastError());
   return PYCOOL_OK;
 }
@@ -236,7 +353,7 @@ long long dispatch(pycool_ctx* c, Op op, int arg) {
   return c->precision == 32 ? dispatch_model<float>(c, op, arg) : dispatch_model<double>(c, op, arg);
 }
 
-void set_geometry(pycool_ctx* c) {
+int set_geometry(pycool_ctx* c) {
   const TileInfo& t = kTiles[c->tile];
   int zc = c->zc_user > 0 ? c->zc_user : auto_zchunk(c->N, c->tile);
   if (zc > c->N) zc = c->N;
@@ -244,6 +361,8 @@ void set_geometry(pycool_ctx* c) {
   while (3 * (size_t)blocks_xy(c->N, c->tile) * (size_t)((c->N + zc - 1) / zc) > c->partials_cap) ++zc;
   c->zc = zc;
   c->grid = dim3((c->N + t.tx - 1) / t.tx, (c->N + t.ty - 1) / t.ty, (c->N + zc - 1) / zc);
+  if (t.stages > 0) return encode_maps(c);
+  return PYCOOL_OK;
 }
 
 int launch_scalar(pycool_ctx* c, double h, double h_next, int mode) {
@@ -255,7 +374,7 @@ int launch_scalar(pycool_ctx* c, double h, double h_next, int mode) {
 }
 
 int launch_flush(pycool_ctx* c) {
-  const size_t n = c->elems;
+  const size_t n = c->lay.total;
   int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 32);
   if (c->precision == 32)
     drift_flush<float><<<nb, 256, 0, c->stream>>>((float*)c->phi[c->cur], (const float*)c->pi[c->cur], c->sc, n);
@@ -269,14 +388,42 @@ int launch_flush(pycool_ctx* c) {
 int launch_sum_pi2(pycool_ctx* c) {
   const size_t n = c->elems;
   int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)kMaxSumBlocks);
-  if (c->precision == 32) sumsq<float><<<nb, 256, 0, c->stream>>>((const float*)c->pi[c->cur], n, c->partials);
-  else sumsq<double><<<nb, 256, 0, c->stream>>>((const double*)c->pi[c->cur], n, c->partials);
+  if (c->precision == 32) sumsq<float><<<nb, 256, 0, c->stream>>>((const float*)c->pi[c->cur], c->lay, c->nf, c->partials);
+  else sumsq<double><<<nb, 256, 0, c->stream>>>((const double*)c->pi[c->cur], c->lay, c->nf, c->partials);
   CUDA_TRY(c, cudaGetLastError());
   reduce_rows<<<1, kReduceThreads, 0, c->stream>>>(c->partials, nb, c->sums);
   CUDA_TRY(c, cudaGetLastError());
   store_spi2<<<1, 1, 0, c->stream>>>(c->sc, c->sums);
   CUDA_TRY(c, cudaGetLastError());
   c->counts[3] += 3;
+  return PYCOOL_OK;
+}
+
+// Copy between a dense [nf][N][N][N] array (host or device) and a state array in layout L.
+int copy_dense(pycool_ctx* c, void* state, void* dense, bool to_state, cudaMemcpyKind kind) {
+  const Layout& L = c->lay;
+  cudaMemcpy3DParms p;
+  std::memset(&p, 0, sizeof p);
+  const cudaPitchedPtr ps = make_cudaPitchedPtr(state, (size_t)L.pitch * c->esize, (size_t)L.pitch, (size_t)L.rows);
+  const cudaPitchedPtr pd = make_cudaPitchedPtr(dense, (size_t)L.N * c->esize, (size_t)L.N, (size_t)L.N);
+  const cudaPos pos_s = make_cudaPos((size_t)L.gx * c->esize, (size_t)L.gy, 0), pos_d = make_cudaPos(0, 0, 0);
+  if (to_state) { p.srcPtr = pd; p.srcPos = pos_d; p.dstPtr = ps; p.dstPos = pos_s; }
+  else { p.srcPtr = ps; p.srcPos = pos_s; p.dstPtr = pd; p.dstPos = pos_d; }
+  p.extent = make_cudaExtent((size_t)L.N * c->esize, (size_t)L.N, (size_t)L.N * c->nf);
+  p.kind = kind;
+  CUDA_TRY(c, cudaMemcpy3DAsync(&p, c->stream));
+  return PYCOOL_OK;
+}
+
+int launch_fill_ghosts(pycool_ctx* c, void* arr) {
+  const Layout& L = c->lay;
+  if (L.gx == 0) return PYCOOL_OK;
+  const size_t n = (size_t)(L.N + 2 * L.gx) * (L.N + 2 * L.gy) * L.N * c->nf;
+  const int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 32);
+  if (c->precision == 32) fill_ghosts<float><<<nb, 256, 0, c->stream>>>((float*)arr, L, c->nf);
+  else fill_ghosts<double><<<nb, 256, 0, c->stream>>>((double*)arr, L, c->nf);
+  CUDA_TRY(c, cudaGetLastError());
+  c->counts[3]++;
   return PYCOOL_OK;
 }
 
@@ -322,7 +469,7 @@ int averages(pycool_ctx* c, double a, Averages* av) {
 }
 
 int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params* p, int order, double dt,
-                  void* d_phi, void* d_pi, void* d_work, size_t work_bytes, void* stream, bool ext) {
+                  void* d_work, size_t work_bytes, void* stream, bool ext) {
   if (!out) return fail(nullptr, PYCOOL_EINVAL, "out is NULL");
   *out = nullptr;
   if (!p) return fail(nullptr, PYCOOL_EINVAL, "params is NULL");
@@ -345,7 +492,7 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
     if (!(std::fabs(cs[0] + s) <= 1e-12 * (std::fabs(cs[0]) + std::fabs(s))))
       return fail(nullptr, PYCOOL_EINVAL, "stencil must satisfy c0 = -(6 c1 + 12 c2 + 8 c3)");
   }
-  if (ext && (!d_phi || !d_pi || !d_work)) return fail(nullptr, PYCOOL_EINVAL, "device buffers are NULL");
+  if (ext && !d_work) return fail(nullptr, PYCOOL_EINVAL, "work buffer is NULL");
 
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -359,6 +506,7 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
   c->esize = c->precision == 32 ? 4 : 8;
   c->L = L; c->dx = L / N; c->dt = dt; c->mpl = p->mpl; c->rho_g = p->rho_gamma0; c->rho_m = p->rho_m0;
   c->V = (size_t)N * N * N; c->elems = c->V * nf;
+  c->lay = make_layout(N, nf, c->esize);
   if (dflt) { c->c[0] = -128.0 / 30.0; c->c[1] = 14.0 / 30.0; c->c[2] = 3.0 / 30.0; c->c[3] = 1.0 / 30.0; }
   else for (int i = 0; i < 4; ++i) c->c[i] = cs[i];
   for (int i = 0; i < 8; ++i) c->mp.p[i] = p->p[i];
@@ -369,28 +517,23 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
   c->nstages = ns;
   for (int i = 0; i < ns; ++i) c->w[i] = (double)wl[i];
 
-  size_t o_phi1, o_pi1, o_part, o_sums, o_sc;
-  const size_t need = work_layout(N, nf, c->esize, &o_phi1, &o_pi1, &o_part, &o_sums, &o_sc);
-  const size_t state_bytes = align_up(c->elems * c->esize, 256);
+  const WorkLayout w = work_layout(N, nf, c->esize);
   unsigned char* work = nullptr;
   int rc = PYCOOL_OK;
   if (ext) {
-    if (work_bytes < need) { rc = fail(nullptr, PYCOOL_EINVAL, "work buffer too small: need %zu bytes", need); goto bad; }
+    if (work_bytes < w.total) { rc = fail(nullptr, PYCOOL_EINVAL, "work buffer too small: need %zu bytes", w.total); goto bad; }
     if (((uintptr_t)d_work & 255) != 0) { rc = fail(nullptr, PYCOOL_EINVAL, "work buffer must be 256-byte aligned"); goto bad; }
-    c->phi[0] = d_phi; c->pi[0] = d_pi;
     work = (unsigned char*)d_work;
     c->stream = (cudaStream_t)stream;
   } else {
     void* blk = nullptr;
-    if (cudaMalloc(&blk, need + 2 * state_bytes) != cudaSuccess) {
+    if (cudaMalloc(&blk, w.total) != cudaSuccess) {
       cudaGetLastError();
-      rc = fail(nullptr, PYCOOL_ENOMEM, "cudaMalloc of %zu bytes failed", need + 2 * state_bytes);
+      rc = fail(nullptr, PYCOOL_ENOMEM, "cudaMalloc of %zu bytes failed", w.total);
       goto bad;
     }
     c->owned_block = blk; c->own_mem = true;
-    c->phi[0] = blk;
-    c->pi[0] = (unsigned char*)blk + state_bytes;
-    work = (unsigned char*)blk + 2 * state_bytes;
+    work = (unsigned char*)blk;
     if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) {
       cudaGetLastError();
       rc = fail(nullptr, PYCOOL_ECUDA, "cudaStreamCreate failed");
@@ -398,23 +541,27 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
     }
     c->own_stream = true;
   }
-  c->phi[1] = work + o_phi1; c->pi[1] = work + o_pi1;
-  c->partials = (double*)(work + o_part);
+  c->phi[0] = work; c->pi[0] = work + w.arr;
+  c->phi[1] = work + 2 * w.arr; c->pi[1] = work + 3 * w.arr;
+  c->partials = (double*)(work + w.off_part);
   c->partials_cap = partials_capacity(N);
-  c->sums = (double*)(work + o_sums);
-  c->sc = (Scalars*)(work + o_sc);
-  c->tile = auto_tile(N);
-  set_geometry(c);
+  c->sums = (double*)(work + w.off_sums);
+  c->sc = (Scalars*)(work + w.off_sc);
+  c->tile = auto_tile(c->lay);
   {
+    // padding and ghosts start as zeros (the closing drift sweeps the whole padded arrays)
     Scalars s0;
     std::memset(&s0, 0, sizeof s0);
     s0.a = 1.0;
-    if (cudaMemcpyAsync(c->sc, &s0, sizeof s0, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+    if (cudaMemsetAsync(work, 0, 4 * w.arr, c->stream) != cudaSuccess ||
+        cudaMemcpyAsync(c->sc, &s0, sizeof s0, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess) {
-      rc = fail(nullptr, PYCOOL_ECUDA, "initialising device scalars failed: %s", cudaGetErrorString(cudaGetLastError()));
+      rc = fail(nullptr, PYCOOL_ECUDA, "initialising device memory failed: %s", cudaGetErrorString(cudaGetLastError()));
       goto bad;
     }
   }
+  rc = set_geometry(c);
+  if (rc != PYCOOL_OK) { g_create_err = c->err; goto bad; }
   *out = c;
   return PYCOOL_OK;
 bad:
@@ -431,36 +578,36 @@ extern "C" {
 
 int pycool_create(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
                   double dt) {
-  return create_common(out, N, L, nfields, params, order, dt, nullptr, nullptr, nullptr, 0, nullptr, false);
+  return create_common(out, N, L, nfields, params, order, dt, nullptr, 0, nullptr, false);
 }
 
 size_t pycool_work_bytes(int N, int nfields, int precision) {
   if (!valid_shape(N, nfields, precision)) return 0;
-  size_t a, b, c, d, e;
-  return work_layout(N, nfields, precision == 32 ? 4 : 8, &a, &b, &c, &d, &e);
+  return work_layout(N, nfields, precision == 32 ? 4 : 8).total;
 }
 
 int pycool_create_ext(pycool_ctx** out, int N, double L, int nfields, const pycool_params* params, int order,
-                      double dt, void* d_phi, void* d_pi, void* d_work, size_t work_bytes, void* cuda_stream) {
-  return create_common(out, N, L, nfields, params, order, dt, d_phi, d_pi, d_work, work_bytes, cuda_stream, true);
+                      double dt, void* d_work, size_t work_bytes, void* cuda_stream) {
+  return create_common(out, N, L, nfields, params, order, dt, d_work, work_bytes, cuda_stream, true);
 }
 
-static int after_upload(pycool_ctx* c) {
+static int upload(pycool_ctx* c, const void* phi, const void* pi, cudaMemcpyKind kind) {
+  c->cur = 0;
+  int st = copy_dense(c, c->phi[0], const_cast<void*>(phi), true, kind);
+  if (st == PYCOOL_OK) st = copy_dense(c, c->pi[0], const_cast<void*>(pi), true, kind);
+  if (st == PYCOOL_OK) st = launch_fill_ghosts(c, c->phi[0]);
+  if (st == PYCOOL_OK) st = launch_fill_ghosts(c, c->pi[0]);
+  if (st != PYCOOL_OK) return st;
   c->have_fields = true;
   c->nonfinite_seen = false;
-  int zero = 0;
-  CUDA_TRY(c, cudaMemcpyAsync(&c->sc->nonfinite, &zero, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(&c->sc->nonfinite, 0, sizeof(int), c->stream));
   return launch_sum_pi2(c);
 }
 
 int pycool_set_fields(pycool_ctx* c, const void* phi_host, const void* pi_host) {
   if (!c) return PYCOOL_EINVAL;
   if (!phi_host || !pi_host) return fail(c, PYCOOL_EINVAL, "phi_host / pi_host is NULL");
-  c->cur = 0;
-  const size_t bytes = c->elems * c->esize;
-  CUDA_TRY(c, cudaMemcpyAsync(c->phi[0], phi_host, bytes, cudaMemcpyHostToDevice, c->stream));
-  CUDA_TRY(c, cudaMemcpyAsync(c->pi[0], pi_host, bytes, cudaMemcpyHostToDevice, c->stream));
-  int st = after_upload(c);
+  int st = upload(c, phi_host, pi_host, cudaMemcpyHostToDevice);
   if (st != PYCOOL_OK) return st;
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   return PYCOOL_OK;
@@ -469,13 +616,7 @@ int pycool_set_fields(pycool_ctx* c, const void* phi_host, const void* pi_host) 
 int pycool_set_fields_device(pycool_ctx* c, const void* d_phi_src, const void* d_pi_src) {
   if (!c) return PYCOOL_EINVAL;
   if (!d_phi_src || !d_pi_src) return fail(c, PYCOOL_EINVAL, "source pointer is NULL");
-  c->cur = 0;
-  const size_t bytes = c->elems * c->esize;
-  if (d_phi_src != c->phi[0])
-    CUDA_TRY(c, cudaMemcpyAsync(c->phi[0], d_phi_src, bytes, cudaMemcpyDeviceToDevice, c->stream));
-  if (d_pi_src != c->pi[0])
-    CUDA_TRY(c, cudaMemcpyAsync(c->pi[0], d_pi_src, bytes, cudaMemcpyDeviceToDevice, c->stream));
-  return after_upload(c);
+  return upload(c, d_phi_src, d_pi_src, cudaMemcpyDeviceToDevice);
 }
 
 int pycool_set_background(pycool_ctx* c, double a, double p_a) {
@@ -551,17 +692,31 @@ int pycool_sync(pycool_ctx* c) {
 int pycool_read_fields(pycool_ctx* c, void* phi_host, void* pi_host) {
   if (!c) return PYCOOL_EINVAL;
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "read before set_fields");
-  const size_t bytes = c->elems * c->esize;
-  if (phi_host) CUDA_TRY(c, cudaMemcpyAsync(phi_host, c->phi[c->cur], bytes, cudaMemcpyDeviceToHost, c->stream));
-  if (pi_host) CUDA_TRY(c, cudaMemcpyAsync(pi_host, c->pi[c->cur], bytes, cudaMemcpyDeviceToHost, c->stream));
+  int st = PYCOOL_OK;
+  if (phi_host) st = copy_dense(c, c->phi[c->cur], phi_host, false, cudaMemcpyDeviceToHost);
+  if (st == PYCOOL_OK && pi_host) st = copy_dense(c, c->pi[c->cur], pi_host, false, cudaMemcpyDeviceToHost);
+  if (st != PYCOOL_OK) return st;
   Scalars s;
   return read_scalars(c, &s);
 }
 
-int pycool_device_fields(pycool_ctx* c, void** d_phi, void** d_pi) {
+int pycool_read_fields_device(pycool_ctx* c, void* d_phi_dst, void* d_pi_dst) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "read before set_fields");
+  int st = PYCOOL_OK;
+  if (d_phi_dst) st = copy_dense(c, c->phi[c->cur], d_phi_dst, false, cudaMemcpyDeviceToDevice);
+  if (st == PYCOOL_OK && d_pi_dst) st = copy_dense(c, c->pi[c->cur], d_pi_dst, false, cudaMemcpyDeviceToDevice);
+  return st;
+}
+
+int pycool_device_fields(pycool_ctx* c, void** d_phi, void** d_pi, size_t layout[4]) {
   if (!c) return PYCOOL_EINVAL;
   if (d_phi) *d_phi = c->phi[c->cur];
   if (d_pi) *d_pi = c->pi[c->cur];
+  if (layout) {
+    layout[0] = (size_t)c->lay.pitch; layout[1] = (size_t)c->lay.rows;
+    layout[2] = (size_t)c->lay.gx; layout[3] = (size_t)c->lay.gy;
+  }
   return PYCOOL_OK;
 }
 
@@ -640,12 +795,14 @@ int pycool_kick_time_ms(pycool_ctx* c, double* total_ms, unsigned long long* lau
   return PYCOOL_OK;
 }
 
-int pycool_kick_geometry(const pycool_ctx* c, int tile[6]) {
+int pycool_kick_geometry(const pycool_ctx* c, int tile[8]) {
   if (!c || !tile) return PYCOOL_EINVAL;
   const TileInfo& t = kTiles[c->tile];
   tile[0] = t.tx; tile[1] = t.ty; tile[2] = c->zc; tile[3] = t.nt;
   tile[4] = (int)(c->grid.x * c->grid.y * c->grid.z);
   tile[5] = (int)dispatch(const_cast<pycool_ctx*>(c), OP_SMEM, c->tile);
+  tile[6] = c->tile;
+  tile[7] = t.stages;
   return PYCOOL_OK;
 }
 
@@ -653,16 +810,16 @@ int pycool_set_zchunk(pycool_ctx* c, int planes) {
   if (!c) return PYCOOL_EINVAL;
   if (planes < 0) return fail(c, PYCOOL_EINVAL, "planes < 0");
   c->zc_user = planes;
-  set_geometry(c);
-  return PYCOOL_OK;
+  return set_geometry(c);
 }
 
 int pycool_set_tile(pycool_ctx* c, int tile) {
   if (!c) return PYCOOL_EINVAL;
   if (tile < -1 || tile >= kNumTiles) return fail(c, PYCOOL_EINVAL, "tile must be -1 (auto) .. %d", kNumTiles - 1);
-  c->tile = tile < 0 ? auto_tile(c->N) : tile;
-  set_geometry(c);
-  return PYCOOL_OK;
+  if (tile >= 0 && !tile_allowed(c->lay, tile))
+    return fail(c, PYCOOL_EINVAL, "tile %d is a TMA variant: it needs the ghost layout (even N >= 4)", tile);
+  c->tile = tile < 0 ? auto_tile(c->lay) : tile;
+  return set_geometry(c);
 }
 
 }  // extern "C"

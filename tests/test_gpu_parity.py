@@ -139,21 +139,66 @@ def test_all_orders(pc, order):
     assert g.launch_counts()[0] == 3 * {2: 1, 4: 3, 6: 7, 8: 15}[order]
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2])
-@pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32)])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32), (6, 0),
+                                  (70, 9), (136, 50)])
 def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
-    """Several tiles with ragged tails in x, y and z, wrap-around at every face, for each tile variant."""
+    """Several tiles with ragged tails in x, y and z, wrap-around at every face, for each variant of the fused
+    kernel: 0-2 register prefetch (any N), 3-7 TMA ring with ghost images (even N)."""
     cfg = inputs.config("cfg0_chaotic32", N=N, dt=0.002, order=4)
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg)
     g, o = make_pair(pc, cfg)
+    if tile >= 3 and N % 2:
+        with pytest.raises(pc.PycoolError) as ei:
+            g.set_tile(tile)
+        assert ei.value.code == pc.EINVAL
+        return
     g.set_tile(tile)
     g.set_zchunk(zc)
     geo = g.kick_geometry()
-    assert geo["zchunk"] >= 1 and geo["blocks"] >= 1
+    assert geo["zchunk"] >= 1 and geo["blocks"] >= 1 and geo["variant"] == tile
+    assert (geo["tma_stages"] > 0) == (tile >= 3)
     start(g, o, phi, pi)
     g.step(2); o.step(2)
     compare(g, o, 2, 2e-12)
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_variants_agree_and_ghost_images_hold(pc, precision):
+    """Every kernel variant from the same state: results agree to rounding, and the ghost columns / rows of the
+    padded state equal their periodic sources bit for bit after stepping (what the TMA boxes rely on)."""
+    import torch
+    cfg = inputs.config("cfg0_chaotic32", N=36, dt=0.002, order=4)
+    cfg["init"], cfg["amp"] = "white", 1e-3
+    phi, pi = inputs.make_initial(cfg, precision=precision)
+    outs = []
+    for tile in range(8):
+        g = pc.from_config(cfg, precision=precision)
+        g.set_tile(tile)
+        g.set_fields(phi, pi)
+        g.set_background(1.0)
+        g.step(2)
+        g.sync()
+        outs.append(g.read_fields())
+        a, b, lay = pc.C.c_void_p(), pc.C.c_void_p(), (pc.C.c_size_t * 4)()
+        assert pc.lib().pycool_device_fields(g._h, pc.C.byref(a), pc.C.byref(b), lay) == 0
+        pitch, rows, gx, gy = (int(v) for v in lay)
+        assert gx == (2 if precision == 64 else 4) and gy == 1 and rows == 38 and pitch >= 36 + 2 * gx
+        for ptr in (a.value, b.value):
+            off = ptr - g._work.data_ptr()
+            full = g._work[off:off + 2 * 36 * rows * pitch * (precision // 8)].view(g._tdtype).view(2, 36, rows, pitch)
+            inner = full[:, :, gy:gy + 36, gx:gx + 36]
+            want = torch.cat([inner[..., -gx:], inner, inner[..., :gx]], dim=-1)
+            want = torch.cat([want[:, :, -1:, :], want, want[:, :, :1, :]], dim=2)
+            assert torch.equal(full[..., :36 + 2 * gx], want), tile
+        pd, qd = g.read_fields_device()
+        assert np.array_equal(pd.cpu().numpy(), outs[-1][0]) and np.array_equal(qd.cpu().numpy(), outs[-1][1])
+        v1, v2 = g.device_fields()
+        assert torch.equal(v1, pd) and torch.equal(v2, qd)
+    tol = 1e-13 if precision == 64 else 2e-5
+    for p, q in outs[1:]:
+        assert rel_err_per_site(p, outs[0][0]) < tol and rel_err_per_site(q, outs[0][1]) < tol
 
 
 def test_bitwise_reproducible(pc):
@@ -267,11 +312,13 @@ def test_state_errors(pc):
 
 
 # ------------------------------------------------------------------------------------- fp32 option
-def test_fp32_one_step(pc):
+@pytest.mark.parametrize("tile", [-1, 1, 3, 6])
+def test_fp32_one_step(pc, tile):
     cfg = inputs.config("cfg0b_chaotic32_resolved", N=40)
     cfg["amp"] = 1e-3
     phi, pi = inputs.make_initial(cfg, precision=32)
     g, o = make_pair(pc, cfg, precision=32)
+    g.set_tile(tile)
     start(g, o, phi, pi)
     g.step(1); o.step(1)
     pg, qg = g.read_fields()
