@@ -55,16 +55,19 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm,
       : "memory");
 }
 
-template <typename Real, int TX_, int TY_, int S_>
+// Tile traits.  Thread (tx2, tyj) owns the x pair 2 tx2 + {0,1} of rows J tyj .. J tyj + J-1 for all fields;
+// MINB = blocks per SM the register budget is cut for (__launch_bounds__).
+template <typename Real, int TX_, int TY_, int S_, int J_ = 2, int MINB_ = 1>
 struct TmaTile {
-  static constexpr int TX = TX_, TY = TY_, S = S_;
+  static constexpr int TX = TX_, TY = TY_, S = S_, J = J_, MINB = MINB_;
   static constexpr int G = 16 / (int)sizeof(Real);      // box halo / ghost columns on each side (16 bytes)
   static constexpr int PX = TX + 2 * G;                 // box row length
   static constexpr int RY = TY + 2;                     // box rows
   static constexpr int PLANE = PX * RY;                 // box elements per field
-  static constexpr int NT = (TX / 2) * (TY / 2);        // threads: 2 x 2 sites each
-  static constexpr int NH = 2 * (TX + 2) + 2 * TY;      // ring of halo sites the stencil reads
-  static_assert(TX % 2 == 0 && TY % 2 == 0, "2 x 2 sites per thread");
+  static constexpr int NT = (TX / 2) * (TY / J);        // threads: 2 x J sites each
+  static constexpr int HR = (TX + 4) / 2;               // halo pairs in the top (and bottom) box row: x = -2 .. TX+1
+  static constexpr int NHP = 2 * HR + 2 * TY;           // ring of halo pairs the stencil reads (x pairs)
+  static_assert(TX % 2 == 0 && TY % J == 0 && (J == 1 || J == 2), "2 x J sites per thread");
   static_assert(NT % 32 == 0 && NT <= 1024, "block size");
   static_assert(PX <= 256 && RY <= 256, "TMA box extents");
 };
@@ -94,13 +97,14 @@ struct TmaArgs {
 };
 
 template <typename Real, class Model, class T>
-__global__ void __launch_bounds__(T::NT)
+__global__ void __launch_bounds__(T::NT, T::MINB)
 kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_pi,
          const TmaArgs<Real> g) {
   using R2 = typename Vec2T<Real>::type;
   using SM = TmaSmem<Real, Model, T>;
-  constexpr int NF = Model::NF, TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT;
+  constexpr int NF = Model::NF, TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J;
   constexpr int PLANE = T::PLANE;
+  constexpr uint32_t ES = (uint32_t)sizeof(Real);
 
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* base = smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u);
@@ -111,7 +115,7 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   const Layout& L = g.L;
   const int N = L.N;
   const int tid = threadIdx.x;
-  const int tx2 = tid % (TX / 2), ty2 = tid / (TX / 2);
+  const int tx2 = tid % (TX / 2), tyj = tid / (TX / 2);
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * g.zc;
   const int nz = min(g.zc, N - z0);
   const int nload = nz + 2;                                    // planes z0-1 .. z0+nz
@@ -145,84 +149,92 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
 #pragma unroll
   for (int f = 0; f < NF; ++f) ref[f] = __ldg(g.phi_in + L.at(f, z0, y0, x0));
 
-  // own sites: global x pair and rows; ghost images (periodic copies on the x / y faces)
+  // Own sites.  Blocks that touch no lattice face and no ragged edge (block-uniform test) store through a
+  // uniform plane pointer plus a 32-bit per-thread byte offset and nothing else; the others also write the
+  // periodic images of their face sites into the ghost columns / rows and predicate ragged sites.
+  const bool edge_blk = (x0 < L.gx) | (x0 + TX > N - L.gx) | (y0 == 0) | (y0 + TY >= N);
   const int gx = x0 + 2 * tx2;
   const bool okx = gx < N;
   int ximg = 0;                                                // element offset of the x image, 0 = none
   if (gx < L.gx) ximg = N; else if (gx >= N - L.gx) ximg = -N;
   const bool ximg2 = (gx < L.gx) && (gx >= N - L.gx);          // both images (N <= 2 gx only)
-  bool valid[2];
-  size_t own_off[2];                                           // offset within a (field, z) plane
-  long long yimg[2];                                           // offset of the y image, 0 = none
+  bool valid[J];
+  uint32_t own_off[J];                                         // byte offset within a (field, z) plane
+  long long yimg[J];                                           // element offset of the y image, 0 = none
 #pragma unroll
-  for (int j = 0; j < 2; ++j) {
-    const int gy = y0 + 2 * ty2 + j;
+  for (int j = 0; j < J; ++j) {
+    const int gy = y0 + J * tyj + j;
     valid[j] = okx && gy < N;
-    own_off[j] = (size_t)(gy + L.gy) * L.pitch + (gx + L.gx);
+    own_off[j] = ((uint32_t)(gy + L.gy) * (uint32_t)L.pitch + (uint32_t)(gx + L.gx)) * ES;
     yimg[j] = 0;
     if (gy == 0) yimg[j] = (long long)N * L.pitch; else if (gy == N - 1) yimg[j] = -(long long)N * L.pitch;
-    if (N == 1) yimg[j] = 0;
   }
-  auto store2 = [&](Real* plane, int j, R2 v) {                // one output pair and its periodic images
-    Real* p = plane + own_off[j];
-    *reinterpret_cast<R2*>(p) = v;                             // plain store (st.global.cs measured 9 % slower)
-    if (ximg | (yimg[j] != 0)) {
+  auto store_edge = [&](unsigned char* plane, int j, R2 v) {   // one output pair and its periodic images
+    Real* p = reinterpret_cast<Real*>(plane + own_off[j]);
+    *reinterpret_cast<R2*>(p) = v;
+    if (ximg) {
+      *reinterpret_cast<R2*>(p + ximg) = v;
+      if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
+    }
+    if (yimg[j]) {
+      *reinterpret_cast<R2*>(p + yimg[j]) = v;
       if (ximg) {
-        *reinterpret_cast<R2*>(p + ximg) = v;
-        if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
-      }
-      if (yimg[j]) {
-        *reinterpret_cast<R2*>(p + yimg[j]) = v;
-        if (ximg) {
-          *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
-          if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
-        }
+        *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
+        if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
       }
     }
   };
+  auto store_own = [&](unsigned char* plane, int j, R2 v) {    // plain store (st.global.cs measured 9 % slower)
+    if (!edge_blk) *reinterpret_cast<R2*>(plane + own_off[j]) = v;
+    else if (valid[j]) store_edge(plane, j, v);
+  };
 
-  // box offsets: own pair (row j) and the halo ring site(s) of this thread
-  const int own_sm = (2 * ty2 + 1) * PX + G + 2 * tx2;
-  constexpr int NHT = (T::NH + NT - 1) / NT;                   // halo sites per thread (1 or 2)
+  // box offsets: own pair of row j, and the halo pair(s) of this thread (top and bottom box rows x = -2 ..
+  // TX+1, and the pairs left and right of every own row; 16-byte accesses, the outer element is unused)
+  const int own_sm = (J * tyj + 1) * PX + G + 2 * tx2;
+  constexpr int NHT = (T::NHP + NT - 1) / NT;                  // halo pairs per thread
   int halo_sm[NHT];
 #pragma unroll
   for (int k = 0; k < NHT; ++k) {
     const int h = tid + k * NT;
     int row, col;
-    if (h < TX + 2) { row = 0; col = G - 1 + h; }
-    else if (h < 2 * (TX + 2)) { row = TY + 1; col = G - 1 + h - (TX + 2); }
-    else { const int r = h - 2 * (TX + 2); row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 1; }
-    halo_sm[k] = h < T::NH ? row * PX + col : -1;
+    if (h < T::HR) { row = 0; col = G - 2 + 2 * h; }
+    else if (h < 2 * T::HR) { row = TY + 1; col = G - 2 + 2 * (h - T::HR); }
+    else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 2; }
+    halo_sm[k] = h < T::NHP ? row * PX + col : -1;
   }
 
-  R2 pphi[NF][2], ppi[NF][2];                                  // phi', pi of plane p-1 (to be finalised)
-  R2 A[NF][2], B[NF][2];                                       // stencil accumulators
+  R2 qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
+  R2 A[NF][J], B[NF][J];                                       // stencil accumulators
   double sD = 0.0, sV = 0.0, sP = 0.0;
 #pragma unroll
   for (int f = 0; f < NF; ++f)
 #pragma unroll
-    for (int j = 0; j < 2; ++j) {
-      A[f][j] = B[f][j] = pphi[f][j] = ppi[f][j] = R2{Real(0), Real(0)};
+    for (int j = 0; j < J; ++j) {
+      A[f][j] = B[f][j] = qa_phi[f][j] = qa_pi[f][j] = qb_phi[f][j] = qb_pi[f][j] = R2{Real(0), Real(0)};
     }
+
+  // uniform output plane pointers, advanced by one plane per step of the march (z wraps at most once per end)
+  const size_t plane_b = L.plane * ES, field_b = L.field * ES;
 
   __syncthreads();                                             // barriers initialised before anyone waits
 
-#pragma unroll 1
-  for (int p = -1; p <= nz; ++p) {
+  // One plane of the march: cphi/cpi receive plane p, pphi/ppi hold plane p-1 (finalised here).
+  auto step = [&](const int p, const int par, R2 (&cphi)[NF][J], R2 (&cpi)[NF][J], const R2 (&pphi)[NF][J],
+                  const R2 (&ppi)[NF][J]) {
     const int i = p + 1, s = i % S;
     const Real* rphi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA);
     const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
-    Real* pb = psi + (size_t)(i & 1) * (SM::BOXA / sizeof(Real));
+    Real* pb = psi + (size_t)par * (SM::BOXA / sizeof(Real));
     mbar_wait(bars + 8u * s, (uint32_t)((i / S) & 1));
 
     // ---- 1. drift: phi' = phi + c_drift pi (own pairs and halo ring); psi = phi' - ref to shared memory
     const bool own_plane = (p >= 0) && (p < nz);
-    const size_t zoff = (size_t)zwrap(p) * L.plane;
-    R2 cphi[NF][2], cpi[NF][2];
+    unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)zwrap(p) * plane_b;
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < J; ++j) {
         const int o = f * PLANE + own_sm + j * PX;
         const R2 a = *reinterpret_cast<const R2*>(rphi + o);
         const R2 b = *reinterpret_cast<const R2*>(rpi + o);
@@ -230,14 +242,16 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
         ph.x = fma(cd, b.x, a.x);
         ph.y = fma(cd, b.y, a.y);
         cphi[f][j] = ph; cpi[f][j] = b;
-        if (own_plane && valid[j]) store2(g.phi_out + f * L.field + zoff, j, ph);
+        if (own_plane) store_own(ophi + f * field_b, j, ph);
         *reinterpret_cast<R2*>(pb + o) = R2{ph.x - ref[f], ph.y - ref[f]};
       }
 #pragma unroll
       for (int k = 0; k < NHT; ++k)
         if (halo_sm[k] >= 0) {
           const int o = f * PLANE + halo_sm[k];
-          pb[o] = fma(cd, rpi[o], rphi[o]) - ref[f];
+          const R2 a = *reinterpret_cast<const R2*>(rphi + o);
+          const R2 b = *reinterpret_cast<const R2*>(rpi + o);
+          *reinterpret_cast<R2*>(pb + o) = R2{fma(cd, b.x, a.x) - ref[f], fma(cd, b.y, a.y) - ref[f]};
         }
     }
     __syncthreads();                                           // psi plane complete; raw stage s consumed
@@ -247,13 +261,13 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     }
 
     // ---- 2. in-plane sums of plane p; 3. finalise plane p-1
-    R2 D[NF][2];
+    R2 D[NF][J];
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       const Real* sp = pb + f * PLANE + own_sm - PX;           // row above the first own row
-      Real Rx[4], Cx[4], Ry[4], Cy[4];                         // x-output 0 and 1: side sums and centres
+      Real Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];         // x-output 0 and 1: side sums and centres
 #pragma unroll
-      for (int r = 0; r < 4; ++r) {
+      for (int r = 0; r < J + 2; ++r) {
         const Real l = sp[r * PX - 1];
         const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
         const Real rr = sp[r * PX + 2];
@@ -261,30 +275,28 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
         Ry[r] = m.x + rr; Cy[r] = m.y;
       }
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < J; ++j) {
         {
           const Real P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
-          const Real up = c1 * P0 + c2 * P1 + c3 * P2;         // weight of plane p in outputs p-1 and p+1
-          const Real mid = c0 * P0 + c1 * P1 + c2 * P2;        // weight of plane p in output p
-          D[f][j].x = A[f][j].x + up;
-          A[f][j].x = B[f][j].x + mid;
+          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));   // weight of plane p in outputs p-1 and p+1
+          D[f][j].x = A[f][j].x + up;                          // output p-1 complete
+          A[f][j].x = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].x)));   // + weight of plane p in output p
           B[f][j].x = up;
         }
         {
           const Real P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
-          const Real up = c1 * P0 + c2 * P1 + c3 * P2;
-          const Real mid = c0 * P0 + c1 * P1 + c2 * P2;
+          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));
           D[f][j].y = A[f][j].y + up;
-          A[f][j].y = B[f][j].y + mid;
+          A[f][j].y = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].y)));
           B[f][j].y = up;
         }
       }
     }
     if (p >= 1) {
-      const size_t zq = (size_t)zwrap(p - 1) * L.plane;
+      unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)zwrap(p - 1) * plane_b;
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        if (valid[j]) {
+      for (int j = 0; j < J; ++j) {
+        if (!edge_blk || valid[j]) {
           Real ph[NF], dV[NF];
           R2 pn[NF];
 #pragma unroll
@@ -304,15 +316,17 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
             pn[f].y = fma(kD, D[f][j].y, fma(-kV, dV[f], ppi[f][j].y));
             sD = fma((double)ph[f], (double)D[f][j].y, sD);
             sP = fma((double)pn[f].y, (double)pn[f].y, sP);
-            store2(g.pi_out + f * L.field + zq, j, pn[f]);
+            store_own(opi + f * field_b, j, pn[f]);
           }
         }
       }
     }
-#pragma unroll
-    for (int f = 0; f < NF; ++f)
-#pragma unroll
-      for (int j = 0; j < 2; ++j) { pphi[f][j] = cphi[f][j]; ppi[f][j] = cpi[f][j]; }
+  };
+
+#pragma unroll 1
+  for (int p = -1; p <= nz; p += 2) {                          // two planes per trip: the p / p-1 roles swap
+    step(p, 0, qa_phi, qa_pi, qb_phi, qb_pi);
+    if (p + 1 <= nz) step(p + 1, 1, qb_phi, qb_pi, qa_phi, qa_pi);
   }
 
   // ---- per-block partial sums, fixed order

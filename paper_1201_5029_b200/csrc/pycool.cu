@@ -126,16 +126,17 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 //                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
 const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
-                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 8, 128, 4}, {32, 32, 256, 3},
-                                    {64, 16, 256, 4}};
+                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 16, 512, 3}, {32, 16, 256, 3},
+                                    {64, 8, 256, 3}};
 using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 16, 2>;
-template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3>;
-template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3>;
-template <typename Real> using TTile5 = TmaTile<Real, 64, 8, 4>;
-template <typename Real> using TTile6 = TmaTile<Real, 32, 32, 3>;
-template <typename Real> using TTile7 = TmaTile<Real, 64, 16, 4>;
+// kick_tma variants: <TX, TY, ring stages, rows per thread J, blocks per SM the registers are cut for>
+template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, 1>;   // 256 threads x (2 x 2 sites)
+template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3, 2, 1>;   // 128 threads x (2 x 2 sites)
+template <typename Real> using TTile5 = TmaTile<Real, 64, 16, 3, 1, 1>;   // 512 threads x (2 x 1 sites)
+template <typename Real> using TTile6 = TmaTile<Real, 32, 16, 3, 1, 2>;   // 256 threads x (2 x 1), 2 blocks / SM
+template <typename Real> using TTile7 = TmaTile<Real, 64, 8, 3, 1, 2>;    // 256 threads x (2 x 1), 2 blocks / SM
 
 // Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
 Layout make_layout(int N, int nf, size_t esize) {
