@@ -167,7 +167,7 @@ int pycool_kick_geometry(const pycool_ctx*, int tile[8]);
 int pycool_set_zchunk(pycool_ctx*, int planes);
 /* Select the variant of the fused kernel; -1 = automatic.
  *   0..2: register-prefetch kernel, tiles 32x8, 32x16, 64x16 sites (any N);
- *   3..7: TMA-fed kernel (even N only, else PYCOOL_EINVAL), tiles 64x16, 32x16 (2 x 2 sites per thread),
+ *   3..9: TMA-fed kernel (even N only, else PYCOOL_EINVAL), tiles 64x16, 32x16 (2 x 2 sites per thread),
  *         64x16, 32x16, 64x8 (2 x 1 sites per thread, more warps per SM). */
 int pycool_set_tile(pycool_ctx*, int tile);
 

@@ -57,7 +57,7 @@ int stage_weights_ld(int order, long double* w) {
 
 constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
 constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
-constexpr int kNumTiles = 8;             // + kick_tma variants (ghost layout only)
+constexpr int kNumTiles = 10;            // + kick_tma variants (ghost layout only)
 
 struct TileInfo { int tx, ty, nt, stages; };   // stages > 0: TMA ring depth
 
@@ -126,8 +126,8 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 //                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
 const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
-                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 16, 512, 3}, {32, 16, 256, 3},
-                                    {64, 8, 256, 3}};
+                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 16, 512, 3}, {64, 16, 256, 4},
+                                    {64, 16, 512, 4}, {128, 8, 256, 3}, {128, 8, 512, 3}};
 using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 16, 2>;
@@ -135,8 +135,10 @@ using Tile2 = Tile<64, 16, 2>;
 template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, 1>;   // 256 threads x (2 x 2 sites)
 template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3, 2, 1>;   // 128 threads x (2 x 2 sites)
 template <typename Real> using TTile5 = TmaTile<Real, 64, 16, 3, 1, 1>;   // 512 threads x (2 x 1 sites)
-template <typename Real> using TTile6 = TmaTile<Real, 32, 16, 3, 1, 2>;   // 256 threads x (2 x 1), 2 blocks / SM
-template <typename Real> using TTile7 = TmaTile<Real, 64, 8, 3, 1, 2>;    // 256 threads x (2 x 1), 2 blocks / SM
+template <typename Real> using TTile6 = TmaTile<Real, 64, 16, 4, 2, 1>;   // as 3, ring of 4
+template <typename Real> using TTile7 = TmaTile<Real, 64, 16, 4, 1, 1>;   // as 5, ring of 4
+template <typename Real> using TTile8 = TmaTile<Real, 128, 8, 3, 2, 1>;   // 256 threads x (2 x 2 sites), 1 KB rows
+template <typename Real> using TTile9 = TmaTile<Real, 128, 8, 3, 1, 1>;   // 512 threads x (2 x 1 sites), 1 KB rows
 
 // Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
 Layout make_layout(int N, int nf, size_t esize) {
@@ -303,7 +305,9 @@ int launch_kick_m(pycool_ctx* c) {
     case 4: return launch_tma_t<Real, Model, TTile4<Real>>(c);
     case 5: return launch_tma_t<Real, Model, TTile5<Real>>(c);
     case 6: return launch_tma_t<Real, Model, TTile6<Real>>(c);
-    default: return launch_tma_t<Real, Model, TTile7<Real>>(c);
+    case 7: return launch_tma_t<Real, Model, TTile7<Real>>(c);
+    case 8: return launch_tma_t<Real, Model, TTile8<Real>>(c);
+    default: return launch_tma_t<Real, Model, TTile9<Real>>(c);
   }
 }
 template <typename Real, class Model>
@@ -316,7 +320,9 @@ size_t kick_smem_m(int tile) {
     case 4: return TmaSmem<Real, Model, TTile4<Real>>::TOTAL;
     case 5: return TmaSmem<Real, Model, TTile5<Real>>::TOTAL;
     case 6: return TmaSmem<Real, Model, TTile6<Real>>::TOTAL;
-    default: return TmaSmem<Real, Model, TTile7<Real>>::TOTAL;
+    case 7: return TmaSmem<Real, Model, TTile7<Real>>::TOTAL;
+    case 8: return TmaSmem<Real, Model, TTile8<Real>>::TOTAL;
+    default: return TmaSmem<Real, Model, TTile9<Real>>::TOTAL;
   }
 }
 template <typename Real, class Model>

@@ -139,7 +139,7 @@ def test_all_orders(pc, order):
     assert g.launch_counts()[0] == 3 * {2: 1, 4: 3, 6: 7, 8: 15}[order]
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9])
 @pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32), (6, 0),
                                   (70, 9), (136, 50)])
 def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
@@ -173,7 +173,7 @@ def test_variants_agree_and_ghost_images_hold(pc, precision):
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg, precision=precision)
     outs = []
-    for tile in range(8):
+    for tile in range(10):
         g = pc.from_config(cfg, precision=precision)
         g.set_tile(tile)
         g.set_fields(phi, pi)
