@@ -115,6 +115,24 @@ class ClockSampler:
         return {"sm_mhz": med, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def max_over_ranks(x, world, device):
+    """MAX over ranks of one host float (the slowest rank's time); identity at world 1.  Needs an initialised
+    process group (NCCL on GPUs; the CPU tests drive it over gloo)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(N, nf, steps, world, seconds):
+    """Replicas only: every rank steps its own lattice, so the job's units are world x one rank's,
+    over the slowest rank's time."""
+    return float(N) ** 3 * nf * steps * world / seconds
+
+
 def time_oracle(cfg, order, steps, warmup, precision):
     """The oracle on an ORACLE_SAMPLE_N^3 sub-lattice with the workload's dx, dt, model and order."""
     import oracle
@@ -215,12 +233,8 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     lat.sync()
     launches = sum(c1) - sum(c0)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    units = float(N) ** 3 * nf * a.steps * world
-    value = units / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, dev)
+    value = whole_job_value(N, nf, a.steps, world, ms * 1e-3)
 
     # ---- end to end: host buffers -> host buffers
     e2e = None
@@ -235,11 +249,8 @@ def main():
         lat.read_fields(h_phi, h_pi)
         barrier()
         te = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([te], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            te = float(t.item())
-        e2e = {"value": units / te, "unit": UNIT, "h2d_bytes_per_step": 2 * nf * N ** 3 * esz / a.steps,
+        te = max_over_ranks(te, world, dev)
+        e2e = {"value": whole_job_value(N, nf, a.steps, world, te), "unit": UNIT, "h2d_bytes_per_step": 2 * nf * N ** 3 * esz / a.steps,
                "d2h_bytes_per_step": (2 * nf * N ** 3 * esz + 208) / a.steps,
                "what": "set_fields(H2D) + set_background + %d steps + energies + read_fields(D2H), pinned host buffers, "
                        "wall clock; bytes are per step of the %d-step job" % (a.steps, a.steps),
