@@ -165,6 +165,15 @@ int pycool_kick_time_ms(pycool_ctx*, double* total_ms, unsigned long long* launc
 int pycool_kick_geometry(const pycool_ctx*, int tile[8]);
 /* Override the z-chunk length (planes per block; 0 = automatic) before the next step. */
 int pycool_set_zchunk(pycool_ctx*, int planes);
+/* Fused stage tail (default on): the block of a drift+kick launch that finishes last adds the per-block partial
+ * sums in block-index order and advances a, p_a and the next stage's coefficients,
+ * so a stage is ONE launch.  Off: a separate reduce + scalar-update launch follows every kick.  Both orders of
+ * summation are fixed; they differ from each other in the last bits only. */
+int pycool_set_fused_tail(pycool_ctx*, int on);
+/* Persistent launch of the TMA-fed kernel (default on): as many blocks as fit on the device at once, each
+ * taking work items (x-y tile, z-chunk) round-robin with its TMA ring running on across item boundaries.
+ * Off: one block per work item.  Partial sums are indexed by work item, so results are bitwise the same. */
+int pycool_set_persistent(pycool_ctx*, int on);
 /* Select the variant of the fused kernel; -1 = automatic.
  *   0..2: register-prefetch kernel, tiles 32x8, 32x16, 64x16 sites (any N);
  *   3..9: TMA-fed kernel (even N only, else PYCOOL_EINVAL), tiles 64x16, 32x16 (2 x 2 sites per thread),

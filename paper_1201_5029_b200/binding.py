@@ -21,7 +21,8 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_set_fields_device", "pycool_set_background", "pycool_set_dt", "pycool_step", "pycool_sync",
            "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
-           "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile")
+           "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
+           "pycool_set_fused_tail", "pycool_set_persistent")
 
 
 class Params(C.Structure):
@@ -87,6 +88,8 @@ def lib():
         L.pycool_kick_geometry.argtypes = [vp, C.POINTER(ip)]
         L.pycool_set_zchunk.argtypes = [vp, ip]
         L.pycool_set_tile.argtypes = [vp, ip]
+        L.pycool_set_fused_tail.argtypes = [vp, ip]
+        L.pycool_set_persistent.argtypes = [vp, ip]
         _lib = L
     return _lib
 
@@ -242,6 +245,12 @@ class Lattice:
 
     def set_zchunk(self, planes):
         self._chk(lib().pycool_set_zchunk(self._h, planes))
+
+    def set_persistent(self, on):
+        self._chk(lib().pycool_set_persistent(self._h, 1 if on else 0))
+
+    def set_fused_tail(self, on):
+        self._chk(lib().pycool_set_fused_tail(self._h, 1 if on else 0))
 
     def set_tile(self, tile):
         self._chk(lib().pycool_set_tile(self._h, tile))

@@ -100,14 +100,17 @@ __device__ __forceinline__ void kick_coefs(Scalars& s, const ScalarConst& k, dou
 
 constexpr int kReduceThreads = 1024;
 
-// Fixed-order sum of v[0..n) by one block: thread t adds elements t, t+T, t+2T, ... in order, then a
-// shared-memory tree whose shape depends only on T.  Result valid in thread 0.
-__device__ __forceinline__ double block_sum_fixed(const double* __restrict__ v, int n, double* sh) {
+// Fixed-order sum of v[0..n) by one block of T threads: thread t adds elements t, t+T, t+2T, ... in order, then
+// a shared-memory tree whose shape depends only on T.  Result valid in every thread.  Loads bypass L1 (the
+// fused tail reads partial sums other blocks wrote during the same launch).
+template <int T>
+__device__ __forceinline__ double block_sum_fixed(const double* v, int n, double* sh /* T doubles */) {
+  static_assert((T & (T - 1)) == 0, "tree shape: power of two");
   double acc = 0.0;
-  for (int i = threadIdx.x; i < n; i += kReduceThreads) acc += v[i];
+  for (int i = threadIdx.x; i < n; i += T) acc += __ldcg(v + i);
   sh[threadIdx.x] = acc;
   __syncthreads();
-  for (int s = kReduceThreads / 2; s > 0; s >>= 1) {
+  for (int s = T / 2; s > 0; s >>= 1) {
     if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
     __syncthreads();
   }
@@ -116,22 +119,13 @@ __device__ __forceinline__ double block_sum_fixed(const double* __restrict__ v, 
   return r;
 }
 
+// The scalar side of the step, one thread.
 // mode 0: opening of a pycool_step call: H1(h_next/2), H2(h_next/2) scalar part, coefficients of the first kick.
-// mode 1: after the kick of a stage of length h: reduce partials [3][nblocks] -> (SD, SV, Spi2); H3 p_a;
-//         H2(h/2) p_a; H1(h/2); and, if h_next != 0, the opening of the next stage merged in:
-//         H1(h_next/2), H2(h_next/2) p_a, c_drift = h/(2 a_i^2) + h_next/(2 a_{i+1}^2).
-__global__ void __launch_bounds__(kReduceThreads)
-scalar_update(Scalars* __restrict__ sc, const double* __restrict__ partials, int nblocks, ScalarConst k,
-              double h, double h_next, int mode) {
-  __shared__ double sh[kReduceThreads];
-  double SD = 0, SV = 0, SP = 0;
-  if (mode == 1) {
-    SD = block_sum_fixed(partials, nblocks, sh);
-    SV = block_sum_fixed(partials + nblocks, nblocks, sh);
-    SP = block_sum_fixed(partials + 2 * (size_t)nblocks, nblocks, sh);
-  }
-  if (threadIdx.x != 0) return;
-  Scalars s = *sc;
+// mode 1: after the kick of a stage of length h, given its reduced sums (SD, SV, Spi2): H3 p_a; H2(h/2) p_a;
+//         H1(h/2); and, if h_next != 0, the opening of the next stage merged in: H1(h_next/2), H2(h_next/2) p_a,
+//         c_drift = h/(2 a_i^2) + h_next/(2 a_{i+1}^2).
+__device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k, double h, double h_next, int mode,
+                                               double SD, double SV, double SP) {
   double c1 = 0.0;
   if (mode == 1) {
     s.SD = SD; s.SV = SV; s.Spi2 = SP;
@@ -151,7 +145,77 @@ scalar_update(Scalars* __restrict__ sc, const double* __restrict__ partials, int
   } else {
     s.c_drift = c1;
   }
+}
+
+// Stand-alone form: reduces partials [3][nblocks] (mode 1) and advances the scalars.  Used for the opening of a
+// call (mode 0) and when the fused tail is switched off.
+__global__ void __launch_bounds__(kReduceThreads)
+scalar_update(Scalars* __restrict__ sc, const double* __restrict__ partials, int nblocks, ScalarConst k,
+              double h, double h_next, int mode) {
+  __shared__ double sh[kReduceThreads];
+  double SD = 0, SV = 0, SP = 0;
+  if (mode == 1) {
+    SD = block_sum_fixed<kReduceThreads>(partials, nblocks, sh);
+    SV = block_sum_fixed<kReduceThreads>(partials + nblocks, nblocks, sh);
+    SP = block_sum_fixed<kReduceThreads>(partials + 2 * (size_t)nblocks, nblocks, sh);
+  }
+  if (threadIdx.x != 0) return;
+  Scalars s = *sc;
+  scalar_advance(s, k, h, h_next, mode, SD, SV, SP);
   *sc = s;
+}
+
+// Tail of a kick kernel.  Thread 0 of every block publishes the block's three partial sums (index = linear
+// block id, so the final order does not depend on arrival).  With a ticket counter (fused mode) the block that
+// arrives last -- every other block has published by then -- reduces all partials in index order and advances
+// the scalars: the stage needs no second launch.  The kernel's own reads of *sc all precede its ticket.
+struct StageTail {
+  Scalars* sc;
+  unsigned int* ticket;   // nullptr: partials only (scalar_update follows as its own launch)
+  ScalarConst k;
+  double h, h_next;
+};
+
+// Thread 0: the three partial sums of work item `idx` of `nparts` (the order of the final sum is the index
+// order, whichever block computed the item and whenever).
+__device__ __forceinline__ void publish_partials(double* partials, unsigned nparts, unsigned idx,
+                                                 const double (&v)[3]) {
+  partials[idx] = v[0];
+  partials[(size_t)nparts + idx] = v[1];
+  partials[2 * (size_t)nparts + idx] = v[2];
+}
+
+// All threads, once per block, after thread 0 published the block's last partials.
+template <int NT>
+__device__ __forceinline__ void stage_finish(const StageTail& t, const double* partials, unsigned nparts,
+                                             double* sh /* >= NT doubles, free to overwrite */) {
+  if (!t.ticket) return;                        // grid-uniform
+  __shared__ int is_last;
+  if (threadIdx.x == 0) {
+    __threadfence();
+    is_last = atomicAdd(t.ticket, 1u) == gridDim.x * gridDim.y * gridDim.z - 1;
+  }
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  const double SD = block_sum_fixed<NT>(partials, (int)nparts, sh);
+  const double SV = block_sum_fixed<NT>(partials + nparts, (int)nparts, sh);
+  const double SP = block_sum_fixed<NT>(partials + 2 * (size_t)nparts, (int)nparts, sh);
+  if (threadIdx.x == 0) {
+    Scalars s = *t.sc;
+    scalar_advance(s, t.k, t.h, t.h_next, 1, SD, SV, SP);
+    *t.sc = s;
+    *t.ticket = 0u;                            // ready for the next launch (stream order)
+  }
+}
+
+// One work item per block (kick_fused): publish, then finish.
+template <int NT>
+__device__ __forceinline__ void stage_tail(const StageTail& t, double* partials, const double (&v)[3], double* sh) {
+  const unsigned nb = gridDim.x * gridDim.y * gridDim.z;
+  const unsigned b = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+  if (threadIdx.x == 0) publish_partials(partials, nb, b, v);
+  stage_finish<NT>(t, partials, nb, sh);
 }
 
 // ------------------------------------------------------------------------------------------------ block reduce
@@ -187,6 +251,7 @@ struct KickArgs {
   Real* pi_out;
   const Scalars* sc;
   double* partials;      // [3][nblocks]: SD, SV, Spi2
+  StageTail tail;        // fused reduction + scalar update by the last block
   Layout L;
   int zc;                // planes per z-chunk
   double c1, c2, c3;     // stencil weights by neighbour class (c0 = -(6c1+12c2+8c3))
@@ -207,7 +272,7 @@ struct Tile {
 template <typename Real, class Model, class T>
 constexpr size_t kick_smem_bytes() {
   size_t tile = 2 * (size_t)Model::NF * T::PLANE * sizeof(Real);
-  size_t red = 3 * (T::NT / 32) * sizeof(double);
+  size_t red = (size_t)T::NT * sizeof(double);          // block_reduce scratch, then the tail's tree
   return tile > red ? tile : red;
 }
 
@@ -385,13 +450,7 @@ kick_fused(const KickArgs<Real> g) {
   __syncthreads();
   double v[3] = {sD, sV, sP};
   block_reduce<3, NT>(v, reinterpret_cast<double*>(smem_raw));
-  if (tid == 0) {
-    const size_t nb = (size_t)gridDim.x * gridDim.y * gridDim.z;
-    const size_t b = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-    g.partials[b] = v[0];
-    g.partials[nb + b] = v[1];
-    g.partials[2 * nb + b] = v[2];
-  }
+  stage_tail<NT>(g.tail, g.partials, v, reinterpret_cast<double*>(smem_raw));
 }
 
 // ------------------------------------------------------------------------------------------------ pointwise
@@ -450,7 +509,7 @@ __global__ void __launch_bounds__(256) sumsq(const Real* __restrict__ v, Layout 
 __global__ void __launch_bounds__(kReduceThreads) reduce_rows(const double* __restrict__ partials, int nb,
                                                              double* __restrict__ out) {
   __shared__ double sh[kReduceThreads];
-  const double r = block_sum_fixed(partials + (size_t)blockIdx.x * nb, nb, sh);
+  const double r = block_sum_fixed<kReduceThreads>(partials + (size_t)blockIdx.x * nb, nb, sh);
   if (threadIdx.x == 0) out[blockIdx.x] = r;
 }
 

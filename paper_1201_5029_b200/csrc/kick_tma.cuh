@@ -79,23 +79,30 @@ struct TmaSmem {
   static constexpr size_t RAW = (size_t)T::S * 2 * BOXA;                       // ring: [S][phi, pi]
   static constexpr size_t PSI = 2 * BOXA;                                      // double-buffered psi planes
   static constexpr size_t BARS = 128;                                          // S mbarriers
-  static constexpr size_t TOTAL = RAW + PSI + BARS + 128;                      // + slack to align the base
-  static_assert(3 * (T::NT / 32) * sizeof(double) <= PSI, "reduction scratch fits in the psi buffers");
+  static constexpr size_t RED = 3 * (T::NT / 32) * sizeof(double);             // per-item block reduction
+  static constexpr size_t TOTAL = RAW + PSI + BARS + RED + 128;                // + slack to align the base
+  static_assert(T::S * 8 <= BARS, "mbarriers fit");
+  static_assert(T::NT * sizeof(double) <= PSI, "the stage tail's tree fits in the psi buffers");
 };
 
 template <typename Real>
 struct TmaArgs {
   Real* phi_out;
   Real* pi_out;
-  const Real* phi_in;     // read directly only for the block's reference values
   const Scalars* sc;
-  double* partials;       // [3][nblocks]: SD, SV, Spi2
+  double* partials;       // [3][nitems]: SD, SV, Spi2
+  StageTail tail;         // fused reduction + scalar update by the last block
   Layout L;
   int zc;                 // planes per z-chunk
+  int nbx, nby, nitems;   // work items = (x tile, y tile, z chunk), x fastest: nitems = nbx nby nbz
   double c1, c2, c3;
   ModelParams mp;
 };
 
+// Work items are dealt round-robin: block b takes items b, b + gridDim.x, ...  With gridDim.x = nitems every
+// block has one item; with gridDim.x = (blocks resident on the GPU) the kernel is persistent and the TMA ring
+// runs on across item boundaries -- the first planes of the next item are in flight while the last planes of
+// the current one are computed, so no block ever waits for a cold pipeline except at the start of the launch.
 template <typename Real, class Model, class T>
 __global__ void __launch_bounds__(T::NT, T::MINB)
 kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_pi,
@@ -111,83 +118,51 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   unsigned char* raw = base;                                   // [S][2][BOXA]
   Real* psi = reinterpret_cast<Real*>(base + SM::RAW);         // [2][BOXA]
   const uint32_t bars = smem_addr(base + SM::RAW + SM::PSI);   // S x 8 bytes
+  double* red = reinterpret_cast<double*>(base + SM::RAW + SM::PSI + SM::BARS);
 
   const Layout& L = g.L;
   const int N = L.N;
   const int tid = threadIdx.x;
   const int tx2 = tid % (TX / 2), tyj = tid / (TX / 2);
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * g.zc;
-  const int nz = min(g.zc, N - z0);
-  const int nload = nz + 2;                                    // planes z0-1 .. z0+nz
+  const int nbxy = g.nbx * g.nby;
 
-  auto zwrap = [&](int p) {
-    int gz = z0 + p;
-    return gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+  // ---- producer (thread 0): the stream of loads, item after item, plane z0-1 .. z0+nz of each
+  int pr_item = blockIdx.x, pr_i = 0, pr_x0 = 0, pr_y0 = 0, pr_z0 = 0, pr_nload = 0;
+  auto pr_decode = [&]() {
+    if (pr_item < g.nitems) {
+      const int bz = pr_item / nbxy, r = pr_item - bz * nbxy, by = r / g.nbx;
+      pr_x0 = (r - by * g.nbx) * TX; pr_y0 = by * TY; pr_z0 = bz * g.zc;
+      pr_nload = min(g.zc, N - pr_z0) + 2;
+    }
+    pr_i = 0;
   };
-  auto issue = [&](int i) {                                    // load index i <-> plane p = i - 1
-    const int s = i % S;
-    const uint32_t bar = bars + 8u * s;
-    const uint32_t dst = smem_addr(raw + (size_t)s * 2 * SM::BOXA);
-    mbar_expect_tx(bar, (uint32_t)(2 * SM::BOX));
-    const int gz = zwrap(i - 1);
-    tma_load_4d(dst, &tm_phi, bar, x0, y0, gz, 0);             // box origin (x0-G, y0-1) in padded coordinates
-    tma_load_4d(dst + (uint32_t)SM::BOXA, &tm_pi, bar, x0, y0, gz, 0);
+  // Every thread keeps the (block-uniform) bookkeeping; only thread 0 touches the barrier and the TMA unit.
+  auto issue_next = [&](int s) {                               // next load of the stream into ring slot s
+    if (pr_item >= g.nitems) return;
+    if (tid == 0) {
+      const uint32_t bar = bars + 8u * s;
+      const uint32_t dst = smem_addr(raw + (size_t)s * 2 * SM::BOXA);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(bar, (uint32_t)(2 * SM::BOX));
+      int gz = pr_z0 + pr_i - 1;
+      gz = gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+      tma_load_4d(dst, &tm_phi, bar, pr_x0, pr_y0, gz, 0);     // box origin (x0-G, y0-1) in padded coordinates
+      tma_load_4d(dst + (uint32_t)SM::BOXA, &tm_pi, bar, pr_x0, pr_y0, gz, 0);
+    }
+    if (++pr_i == pr_nload) { pr_item += gridDim.x; pr_decode(); }
   };
 
   if (tid == 0) {
     for (int s = 0; s < S; ++s) mbar_init(bars + 8u * s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    for (int i = 0; i < S && i < nload; ++i) issue(i);
   }
+  pr_decode();
+  for (int s = 0; s < S; ++s) issue_next(s);
 
   const Real cd = Real(g.sc->c_drift), kD = Real(g.sc->kD), kV = Real(g.sc->kV);
   const Real c1 = Real(g.c1), c2 = Real(g.c2), c3 = Real(g.c3);
   const Real c0 = -(Real(6) * c1 + Real(12) * c2 + Real(8) * c3);
   const typename Model::template Coef<Real> coef(g.mp);
-  Real ref[NF];                                                // block-uniform; D annihilates constants
-#pragma unroll
-  for (int f = 0; f < NF; ++f) ref[f] = __ldg(g.phi_in + L.at(f, z0, y0, x0));
-
-  // Own sites.  Blocks that touch no lattice face and no ragged edge (block-uniform test) store through a
-  // uniform plane pointer plus a 32-bit per-thread byte offset and nothing else; the others also write the
-  // periodic images of their face sites into the ghost columns / rows and predicate ragged sites.
-  const bool edge_blk = (x0 < L.gx) | (x0 + TX > N - L.gx) | (y0 == 0) | (y0 + TY >= N);
-  const int gx = x0 + 2 * tx2;
-  const bool okx = gx < N;
-  int ximg = 0;                                                // element offset of the x image, 0 = none
-  if (gx < L.gx) ximg = N; else if (gx >= N - L.gx) ximg = -N;
-  const bool ximg2 = (gx < L.gx) && (gx >= N - L.gx);          // both images (N <= 2 gx only)
-  bool valid[J];
-  uint32_t own_off[J];                                         // byte offset within a (field, z) plane
-  long long yimg[J];                                           // element offset of the y image, 0 = none
-#pragma unroll
-  for (int j = 0; j < J; ++j) {
-    const int gy = y0 + J * tyj + j;
-    valid[j] = okx && gy < N;
-    own_off[j] = ((uint32_t)(gy + L.gy) * (uint32_t)L.pitch + (uint32_t)(gx + L.gx)) * ES;
-    yimg[j] = 0;
-    if (gy == 0) yimg[j] = (long long)N * L.pitch; else if (gy == N - 1) yimg[j] = -(long long)N * L.pitch;
-  }
-  auto store_edge = [&](unsigned char* plane, int j, R2 v) {   // one output pair and its periodic images
-    Real* p = reinterpret_cast<Real*>(plane + own_off[j]);
-    *reinterpret_cast<R2*>(p) = v;
-    if (ximg) {
-      *reinterpret_cast<R2*>(p + ximg) = v;
-      if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
-    }
-    if (yimg[j]) {
-      *reinterpret_cast<R2*>(p + yimg[j]) = v;
-      if (ximg) {
-        *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
-        if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
-      }
-    }
-  };
-  auto store_own = [&](unsigned char* plane, int j, R2 v) {    // plain store (st.global.cs measured 9 % slower)
-    if (!edge_blk) *reinterpret_cast<R2*>(plane + own_off[j]) = v;
-    else if (valid[j]) store_edge(plane, j, v);
-  };
 
   // box offsets: own pair of row j, and the halo pair(s) of this thread (top and bottom box rows x = -2 ..
   // TX+1, and the pairs left and right of every own row; 16-byte accesses, the outer element is unused)
@@ -203,143 +178,200 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 2; }
     halo_sm[k] = h < T::NHP ? row * PX + col : -1;
   }
-
-  R2 qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
-  R2 A[NF][J], B[NF][J];                                       // stencil accumulators
-  double sD = 0.0, sV = 0.0, sP = 0.0;
-#pragma unroll
-  for (int f = 0; f < NF; ++f)
-#pragma unroll
-    for (int j = 0; j < J; ++j) {
-      A[f][j] = B[f][j] = qa_phi[f][j] = qa_pi[f][j] = qb_phi[f][j] = qb_pi[f][j] = R2{Real(0), Real(0)};
-    }
-
-  // uniform output plane pointers, advanced by one plane per step of the march (z wraps at most once per end)
   const size_t plane_b = L.plane * ES, field_b = L.field * ES;
+
+  int slot = 0;                                                // ring slot and phase of the next plane to consume
+  uint32_t phase = 0;
 
   __syncthreads();                                             // barriers initialised before anyone waits
 
-  // One plane of the march: cphi/cpi receive plane p, pphi/ppi hold plane p-1 (finalised here).
-  auto step = [&](const int p, const int par, R2 (&cphi)[NF][J], R2 (&cpi)[NF][J], const R2 (&pphi)[NF][J],
-                  const R2 (&ppi)[NF][J]) {
-    const int i = p + 1, s = i % S;
-    const Real* rphi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA);
-    const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
-    Real* pb = psi + (size_t)par * (SM::BOXA / sizeof(Real));
-    mbar_wait(bars + 8u * s, (uint32_t)((i / S) & 1));
+#pragma unroll 1
+  for (int item = blockIdx.x; item < g.nitems; item += gridDim.x) {
+    const int bz = item / nbxy, rr_ = item - bz * nbxy, by = rr_ / g.nbx;
+    const int x0 = (rr_ - by * g.nbx) * TX, y0 = by * TY, z0 = bz * g.zc;
+    const int nz = min(g.zc, N - z0);
+    auto zwrap = [&](int p) {
+      int gz = z0 + p;
+      return gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+    };
 
-    // ---- 1. drift: phi' = phi + c_drift pi (own pairs and halo ring); psi = phi' - ref to shared memory
-    const bool own_plane = (p >= 0) && (p < nz);
-    unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)zwrap(p) * plane_b;
+    // Own sites.  Items that touch no lattice face and no ragged edge (block-uniform test) store through a
+    // uniform plane pointer plus a 32-bit per-thread byte offset and nothing else; the others also write the
+    // periodic images of their face sites into the ghost columns / rows and predicate ragged sites.
+    const bool edge_blk = (x0 < L.gx) | (x0 + TX > N - L.gx) | (y0 == 0) | (y0 + TY >= N);
+    const int gx = x0 + 2 * tx2;
+    const bool okx = gx < N;
+    int ximg = 0;                                              // element offset of the x image, 0 = none
+    if (gx < L.gx) ximg = N; else if (gx >= N - L.gx) ximg = -N;
+    const bool ximg2 = (gx < L.gx) && (gx >= N - L.gx);        // both images (N <= 2 gx only)
+    bool valid[J];
+    uint32_t own_off[J];                                       // byte offset within a (field, z) plane
+    long long yimg[J];                                         // element offset of the y image, 0 = none
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const int gy = y0 + J * tyj + j;
+      valid[j] = okx && gy < N;
+      own_off[j] = ((uint32_t)(gy + L.gy) * (uint32_t)L.pitch + (uint32_t)(gx + L.gx)) * ES;
+      yimg[j] = 0;
+      if (gy == 0) yimg[j] = (long long)N * L.pitch; else if (gy == N - 1) yimg[j] = -(long long)N * L.pitch;
+    }
+    auto store_edge = [&](unsigned char* plane, int j, R2 v) { // one output pair and its periodic images
+      Real* p = reinterpret_cast<Real*>(plane + own_off[j]);
+      *reinterpret_cast<R2*>(p) = v;
+      if (ximg) {
+        *reinterpret_cast<R2*>(p + ximg) = v;
+        if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
+      }
+      if (yimg[j]) {
+        *reinterpret_cast<R2*>(p + yimg[j]) = v;
+        if (ximg) {
+          *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
+          if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
+        }
+      }
+    };
+    auto store_own = [&](unsigned char* plane, int j, R2 v) {  // plain store (st.global.cs measured 9 % slower)
+      if (!edge_blk) *reinterpret_cast<R2*>(plane + own_off[j]) = v;
+      else if (valid[j]) store_edge(plane, j, v);
+    };
+
+    R2 qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
+    R2 A[NF][J], B[NF][J];                                     // stencil accumulators
+    Real ref[NF];                                              // item-uniform; D annihilates constants
+    double sD = 0.0, sV = 0.0, sP = 0.0;
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
+      ref[f] = Real(0);
 #pragma unroll
       for (int j = 0; j < J; ++j) {
-        const int o = f * PLANE + own_sm + j * PX;
-        const R2 a = *reinterpret_cast<const R2*>(rphi + o);
-        const R2 b = *reinterpret_cast<const R2*>(rpi + o);
-        R2 ph;
-        ph.x = fma(cd, b.x, a.x);
-        ph.y = fma(cd, b.y, a.y);
-        cphi[f][j] = ph; cpi[f][j] = b;
-        if (own_plane) store_own(ophi + f * field_b, j, ph);
-        *reinterpret_cast<R2*>(pb + o) = R2{ph.x - ref[f], ph.y - ref[f]};
+        A[f][j] = B[f][j] = qa_phi[f][j] = qa_pi[f][j] = qb_phi[f][j] = qb_pi[f][j] = R2{Real(0), Real(0)};
       }
+    }
+
+    // One plane of the march: cphi/cpi receive plane p, pphi/ppi hold plane p-1 (finalised here).
+    auto step = [&](const int p, const int par, R2 (&cphi)[NF][J], R2 (&cpi)[NF][J], const R2 (&pphi)[NF][J],
+                    const R2 (&ppi)[NF][J]) {
+      const int s = slot;
+      const Real* rphi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA);
+      const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
+      Real* pb = psi + (size_t)par * (SM::BOXA / sizeof(Real));
+      mbar_wait(bars + 8u * s, phase);
+      if (++slot == S) { slot = 0; phase ^= 1u; }
+
+      // reference value of each field: phi at the item's first site one plane below (any item-uniform value
+      // near the field does; it is the same for every thread because it is read from the shared box)
+      if (p == -1) {
 #pragma unroll
-      for (int k = 0; k < NHT; ++k)
-        if (halo_sm[k] >= 0) {
-          const int o = f * PLANE + halo_sm[k];
+        for (int f = 0; f < NF; ++f) ref[f] = rphi[f * PLANE + PX + G];
+      }
+
+      // ---- 1. drift: phi' = phi + c_drift pi (own pairs and halo ring); psi = phi' - ref to shared memory
+      const bool own_plane = (p >= 0) && (p < nz);
+      unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)zwrap(p) * plane_b;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+          const int o = f * PLANE + own_sm + j * PX;
           const R2 a = *reinterpret_cast<const R2*>(rphi + o);
           const R2 b = *reinterpret_cast<const R2*>(rpi + o);
-          *reinterpret_cast<R2*>(pb + o) = R2{fma(cd, b.x, a.x) - ref[f], fma(cd, b.y, a.y) - ref[f]};
+          R2 ph;
+          ph.x = fma(cd, b.x, a.x);
+          ph.y = fma(cd, b.y, a.y);
+          cphi[f][j] = ph; cpi[f][j] = b;
+          if (own_plane) store_own(ophi + f * field_b, j, ph);
+          *reinterpret_cast<R2*>(pb + o) = R2{ph.x - ref[f], ph.y - ref[f]};
         }
-    }
-    __syncthreads();                                           // psi plane complete; raw stage s consumed
-    if (tid == 0 && i + S < nload) {
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      issue(i + S);
-    }
+#pragma unroll
+        for (int k = 0; k < NHT; ++k)
+          if (halo_sm[k] >= 0) {
+            const int o = f * PLANE + halo_sm[k];
+            const R2 a = *reinterpret_cast<const R2*>(rphi + o);
+            const R2 b = *reinterpret_cast<const R2*>(rpi + o);
+            *reinterpret_cast<R2*>(pb + o) = R2{fma(cd, b.x, a.x) - ref[f], fma(cd, b.y, a.y) - ref[f]};
+          }
+      }
+      __syncthreads();                                         // psi plane complete; raw stage s consumed
+      issue_next(s);
 
-    // ---- 2. in-plane sums of plane p; 3. finalise plane p-1
-    R2 D[NF][J];
+      // ---- 2. in-plane sums of plane p; 3. finalise plane p-1
+      R2 D[NF][J];
 #pragma unroll
-    for (int f = 0; f < NF; ++f) {
-      const Real* sp = pb + f * PLANE + own_sm - PX;           // row above the first own row
-      Real Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];         // x-output 0 and 1: side sums and centres
+      for (int f = 0; f < NF; ++f) {
+        const Real* sp = pb + f * PLANE + own_sm - PX;         // row above the first own row
+        Real Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];       // x-output 0 and 1: side sums and centres
 #pragma unroll
-      for (int r = 0; r < J + 2; ++r) {
-        const Real l = sp[r * PX - 1];
-        const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
-        const Real rr = sp[r * PX + 2];
-        Rx[r] = l + m.y; Cx[r] = m.x;
-        Ry[r] = m.x + rr; Cy[r] = m.y;
-      }
-#pragma unroll
-      for (int j = 0; j < J; ++j) {
-        {
-          const Real P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
-          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));   // weight of plane p in outputs p-1 and p+1
-          D[f][j].x = A[f][j].x + up;                          // output p-1 complete
-          A[f][j].x = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].x)));   // + weight of plane p in output p
-          B[f][j].x = up;
+        for (int r = 0; r < J + 2; ++r) {
+          const Real l = sp[r * PX - 1];
+          const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
+          const Real rr = sp[r * PX + 2];
+          Rx[r] = l + m.y; Cx[r] = m.x;
+          Ry[r] = m.x + rr; Cy[r] = m.y;
         }
-        {
-          const Real P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
-          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));
-          D[f][j].y = A[f][j].y + up;
-          A[f][j].y = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].y)));
-          B[f][j].y = up;
-        }
-      }
-    }
-    if (p >= 1) {
-      unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)zwrap(p - 1) * plane_b;
 #pragma unroll
-      for (int j = 0; j < J; ++j) {
-        if (!edge_blk || valid[j]) {
-          Real ph[NF], dV[NF];
-          R2 pn[NF];
-#pragma unroll
-          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].x;
-          sV += (double)Model::template eval<Real>(coef, ph, dV);
-#pragma unroll
-          for (int f = 0; f < NF; ++f) {
-            pn[f].x = fma(kD, D[f][j].x, fma(-kV, dV[f], ppi[f][j].x));   // pi' = pi + kD D - kV dV
-            sD = fma((double)ph[f], (double)D[f][j].x, sD);
-            sP = fma((double)pn[f].x, (double)pn[f].x, sP);
+        for (int j = 0; j < J; ++j) {
+          {
+            const Real P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
+            const Real up = fma(c3, P2, fma(c2, P1, c1 * P0)); // weight of plane p in outputs p-1 and p+1
+            D[f][j].x = A[f][j].x + up;                        // output p-1 complete
+            A[f][j].x = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].x)));   // + weight of plane p in output p
+            B[f][j].x = up;
           }
-#pragma unroll
-          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].y;
-          sV += (double)Model::template eval<Real>(coef, ph, dV);
-#pragma unroll
-          for (int f = 0; f < NF; ++f) {
-            pn[f].y = fma(kD, D[f][j].y, fma(-kV, dV[f], ppi[f][j].y));
-            sD = fma((double)ph[f], (double)D[f][j].y, sD);
-            sP = fma((double)pn[f].y, (double)pn[f].y, sP);
-            store_own(opi + f * field_b, j, pn[f]);
+          {
+            const Real P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
+            const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));
+            D[f][j].y = A[f][j].y + up;
+            A[f][j].y = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].y)));
+            B[f][j].y = up;
           }
         }
       }
-    }
-  };
+      if (p >= 1) {
+        unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)zwrap(p - 1) * plane_b;
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+          if (!edge_blk || valid[j]) {
+            Real ph[NF], dV[NF];
+            R2 pn[NF];
+#pragma unroll
+            for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].x;
+            sV += (double)Model::template eval<Real>(coef, ph, dV);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+              pn[f].x = fma(kD, D[f][j].x, fma(-kV, dV[f], ppi[f][j].x));   // pi' = pi + kD D - kV dV
+              sD = fma((double)ph[f], (double)D[f][j].x, sD);
+              sP = fma((double)pn[f].x, (double)pn[f].x, sP);
+            }
+#pragma unroll
+            for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].y;
+            sV += (double)Model::template eval<Real>(coef, ph, dV);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+              pn[f].y = fma(kD, D[f][j].y, fma(-kV, dV[f], ppi[f][j].y));
+              sD = fma((double)ph[f], (double)D[f][j].y, sD);
+              sP = fma((double)pn[f].y, (double)pn[f].y, sP);
+              store_own(opi + f * field_b, j, pn[f]);
+            }
+          }
+        }
+      }
+    };
 
 #pragma unroll 1
-  for (int p = -1; p <= nz; p += 2) {                          // two planes per trip: the p / p-1 roles swap
-    step(p, 0, qa_phi, qa_pi, qb_phi, qb_pi);
-    if (p + 1 <= nz) step(p + 1, 1, qb_phi, qb_pi, qa_phi, qa_pi);
+    for (int p = -1; p <= nz; p += 2) {                        // two planes per trip: the p / p-1 roles swap
+      step(p, 0, qa_phi, qa_pi, qb_phi, qb_pi);
+      if (p + 1 <= nz) step(p + 1, 1, qb_phi, qb_pi, qa_phi, qa_pi);
+    }
+
+    // ---- the item's partial sums, fixed order.  The barrier inside block_reduce also separates this item's
+    // last reads of the psi planes from the next item's first writes.
+    double v[3] = {sD, sV, sP};
+    block_reduce<3, NT>(v, red);
+    if (tid == 0) publish_partials(g.partials, (unsigned)g.nitems, (unsigned)item, v);
   }
 
-  // ---- per-block partial sums, fixed order
-  __syncthreads();
-  double v[3] = {sD, sV, sP};
-  block_reduce<3, NT>(v, reinterpret_cast<double*>(psi));
-  if (tid == 0) {
-    const size_t nb = (size_t)gridDim.x * gridDim.y * gridDim.z;
-    const size_t b = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-    g.partials[b] = v[0];
-    g.partials[nb + b] = v[1];
-    g.partials[2 * nb + b] = v[2];
-  }
+  __syncthreads();                                             // psi is free: the tail's tree uses it
+  stage_finish<NT>(g.tail, g.partials, (unsigned)g.nitems, reinterpret_cast<double*>(psi));
 }
 
 }  // namespace pycool

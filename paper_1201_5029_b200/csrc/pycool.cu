@@ -56,8 +56,9 @@ int stage_weights_ld(int order, long double* w) {
 }
 
 constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
+constexpr size_t kMaxSmem = 227 * 1024;  // dynamic shared memory one block may opt in to on sm_100
 constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
-constexpr int kNumTiles = 10;            // + kick_tma variants (ghost layout only)
+constexpr int kNumTiles = 12;            // + kick_tma variants (ghost layout only)
 
 struct TileInfo { int tx, ty, nt, stages; };   // stages > 0: TMA ring depth
 
@@ -86,6 +87,11 @@ struct pycool_ctx {
   size_t partials_cap = 0;
   double* sums = nullptr;       // 16 doubles: reduced rows
   Scalars* sc = nullptr;
+  unsigned int* ticket = nullptr;   // blocks-done counter of the fused stage tail (zero between launches)
+  bool persistent = true;           // kick_tma: one block per resident slot, the TMA ring runs on across items
+  int blocks_launched = 0;          // grid size of the latest kick launch
+  bool fused_tail = true;           // last block of a kick reduces the partials and advances the scalars
+  double h_cur = 0, h_next = 0;     // stage lengths handed to the next kick launch
   bool own_mem = false, own_stream = false;
   void* owned_block = nullptr;  // one allocation when own_mem
   cudaStream_t stream = nullptr;
@@ -127,18 +133,21 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 //                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
 const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
                                     {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 16, 512, 3}, {64, 16, 256, 4},
-                                    {64, 16, 512, 4}, {128, 8, 256, 3}, {128, 8, 512, 3}};
+                                    {64, 16, 512, 4}, {128, 8, 256, 3}, {128, 8, 512, 3},
+                                    {128, 16, 512, 3}, {64, 32, 512, 3}};
 using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 16, 2>;
 // kick_tma variants: <TX, TY, ring stages, rows per thread J, blocks per SM the registers are cut for>
-template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, 1>;   // 256 threads x (2 x 2 sites)
+template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 256 threads x (2 x 2 sites)
 template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3, 2, 1>;   // 128 threads x (2 x 2 sites)
 template <typename Real> using TTile5 = TmaTile<Real, 64, 16, 3, 1, 1>;   // 512 threads x (2 x 1 sites)
 template <typename Real> using TTile6 = TmaTile<Real, 64, 16, 4, 2, 1>;   // as 3, ring of 4
 template <typename Real> using TTile7 = TmaTile<Real, 64, 16, 4, 1, 1>;   // as 5, ring of 4
-template <typename Real> using TTile8 = TmaTile<Real, 128, 8, 3, 2, 1>;   // 256 threads x (2 x 2 sites), 1 KB rows
+template <typename Real> using TTile8 = TmaTile<Real, 128, 8, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 256 threads x (2 x 2 sites), 1 KB rows
 template <typename Real> using TTile9 = TmaTile<Real, 128, 8, 3, 1, 1>;   // 512 threads x (2 x 1 sites), 1 KB rows
+template <typename Real> using TTile10 = TmaTile<Real, 128, 16, 3, 2, 1>; // 512 threads x (2 x 2 sites): twice the
+template <typename Real> using TTile11 = TmaTile<Real, 64, 32, 3, 2, 1>;  //   bytes per plane (fp32, one field)
 
 // Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
 Layout make_layout(int N, int nf, size_t esize) {
@@ -162,10 +171,7 @@ Layout make_layout(int N, int nf, size_t esize) {
 
 bool tile_allowed(const Layout& L, int tile) { return tile < kNumGeneric || L.gx > 0; }
 
-int auto_tile(const Layout& L) {
-  if (L.gx > 0) return L.N <= 64 ? 4 : 3;
-  return L.N <= 64 ? 0 : 1;
-}
+int auto_tile(pycool_ctx* c);   // after dispatch(): needs the shared-memory size of a variant
 
 int blocks_xy(int N, int tile) {
   const TileInfo& t = kTiles[tile];
@@ -264,6 +270,11 @@ int launch_kick_t(pycool_ctx* c) {
   g.pi_out = (Real*)c->pi[c->cur ^ 1];
   g.sc = c->sc;
   g.partials = c->partials;
+  g.tail.sc = c->sc;
+  g.tail.ticket = c->fused_tail ? c->ticket : nullptr;
+  g.tail.k = c->kc;
+  g.tail.h = c->h_cur;
+  g.tail.h_next = c->h_next;
   g.L = c->lay;
   g.zc = c->zc;
   g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
@@ -275,23 +286,37 @@ int launch_kick_t(pycool_ctx* c) {
 template <typename Real, class Model, class T>
 int launch_tma_t(pycool_ctx* c) {
   static bool attr_done = false;
+  static int resident = 0;            // blocks of this instance that fit on the device at once
   constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
   if (!attr_done) {
     CUDA_TRY(c, cudaFuncSetAttribute(kick_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)smem));
+    int per_sm = 0, dev = 0, sms = 0;
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kick_tma<Real, Model, T>, T::NT, smem));
+    CUDA_TRY(c, cudaGetDevice(&dev));
+    CUDA_TRY(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    resident = per_sm * sms;
+    if (resident < 1) return fail(c, PYCOOL_ECUDA, "kick_tma does not fit on an SM (%zu bytes of shared memory)", smem);
     attr_done = true;
   }
   TmaArgs<Real> g;
-  g.phi_in = (const Real*)c->phi[c->cur];
   g.phi_out = (Real*)c->phi[c->cur ^ 1];
   g.pi_out = (Real*)c->pi[c->cur ^ 1];
   g.sc = c->sc;
   g.partials = c->partials;
+  g.tail.sc = c->sc;
+  g.tail.ticket = c->fused_tail ? c->ticket : nullptr;
+  g.tail.k = c->kc;
+  g.tail.h = c->h_cur;
+  g.tail.h_next = c->h_next;
   g.L = c->lay;
   g.zc = c->zc;
-  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
-  g.mp = c->mp;
-  kick_tma<Real, Model, T><<<c->grid, T::NT, smem, c->stream>>>(c->tm[c->cur][0], c->tm[c->cur][1], g);
+  g.nbx = (int)c->grid.x; g.nby = (int)c->grid.y;
+  g.nitems = (int)(c->grid.x * c->grid.y * c->grid.z);
+  // persistent: one block per resident slot, items dealt round-robin; else one block per item
+  const int nblocks = c->persistent && resident < g.nitems ? resident : g.nitems;
+  c->blocks_launched = nblocks;
+  kick_tma<Real, Model, T><<<nblocks, T::NT, smem, c->stream>>>(c->tm[c->cur][0], c->tm[c->cur][1], g);
   CUDA_TRY(c, cudaGetLastError());
   return PYCOOL_OK;
 }
@@ -307,7 +332,9 @@ int launch_kick_m(pycool_ctx* c) {
     case 6: return launch_tma_t<Real, Model, TTile6<Real>>(c);
     case 7: return launch_tma_t<Real, Model, TTile7<Real>>(c);
     case 8: return launch_tma_t<Real, Model, TTile8<Real>>(c);
-    default: return launch_tma_t<Real, Model, TTile9<Real>>(c);
+    case 9: return launch_tma_t<Real, Model, TTile9<Real>>(c);
+    case 10: return launch_tma_t<Real, Model, TTile10<Real>>(c);
+    default: return launch_tma_t<Real, Model, TTile11<Real>>(c);
   }
 }
 template <typename Real, class Model>
@@ -322,7 +349,9 @@ size_t kick_smem_m(int tile) {
     case 6: return TmaSmem<Real, Model, TTile6<Real>>::TOTAL;
     case 7: return TmaSmem<Real, Model, TTile7<Real>>::TOTAL;
     case 8: return TmaSmem<Real, Model, TTile8<Real>>::TOTAL;
-    default: return TmaSmem<Real, Model, TTile9<Real>>::TOTAL;
+    case 9: return TmaSmem<Real, Model, TTile9<Real>>::TOTAL;
+    case 10: return TmaSmem<Real, Model, TTile10<Real>>::TOTAL;
+    default: return TmaSmem<Real, Model, TTile11<Real>>::TOTAL;
   }
 }
 template <typename Real, class Model>
@@ -358,6 +387,18 @@ long long dispatch_model(pycool_ctx* c, Op op, int arg) {
 }
 long long dispatch(pycool_ctx* c, Op op, int arg) {
   return c->precision == 32 ? dispatch_model<float>(c, op, arg) : dispatch_model<double>(c, op, arg);
+}
+
+// Automatic variant: the register-prefetch kernel where the layout has no ghosts (odd N); else the first TMA
+// variant of a measured preference list whose ring fits in shared memory for this model and precision.
+int auto_tile(pycool_ctx* c) {
+  const Layout& L = c->lay;
+  if (L.gx == 0) return L.N <= 64 ? 0 : 1;
+  if (L.N <= 64) return 4;
+  static const int pref[] = {3, 4};
+  for (int t : pref)
+    if ((size_t)dispatch(c, OP_SMEM, t) <= kMaxSmem) return t;
+  return 1;
 }
 
 int set_geometry(pycool_ctx* c) {
@@ -554,13 +595,15 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
   c->partials_cap = partials_capacity(N);
   c->sums = (double*)(work + w.off_sums);
   c->sc = (Scalars*)(work + w.off_sc);
-  c->tile = auto_tile(c->lay);
+  c->ticket = (unsigned int*)(work + w.off_sc + 128);
+  c->tile = auto_tile(c);
   {
     // padding and ghosts start as zeros (the closing drift sweeps the whole padded arrays)
     Scalars s0;
     std::memset(&s0, 0, sizeof s0);
     s0.a = 1.0;
     if (cudaMemsetAsync(work, 0, 4 * w.arr, c->stream) != cudaSuccess ||
+        cudaMemsetAsync(work + w.off_sc, 0, 256, c->stream) != cudaSuccess ||
         cudaMemcpyAsync(c->sc, &s0, sizeof s0, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess) {
       rc = fail(nullptr, PYCOOL_ECUDA, "initialising device memory failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -676,13 +719,17 @@ int pycool_step(pycool_ctx* c, int nsteps) {
     const double h = c->w[i % ns] * c->dt;
     const double h_next = (i + 1 < S) ? c->w[(i + 1) % ns] * c->dt : 0.0;
     if (c->profiling) CUDA_TRY(c, cudaEventRecord(c->ev[c->ev_used++], c->stream));
+    c->h_cur = h;
+    c->h_next = h_next;
     st = (int)dispatch(c, OP_KICK, 0);
     if (st != PYCOOL_OK) return st;
     if (c->profiling) CUDA_TRY(c, cudaEventRecord(c->ev[c->ev_used++], c->stream));
     c->counts[0]++;
     c->cur ^= 1;
-    st = launch_scalar(c, h, h_next, 1);
-    if (st != PYCOOL_OK) return st;
+    if (!c->fused_tail) {
+      st = launch_scalar(c, h, h_next, 1);
+      if (st != PYCOOL_OK) return st;
+    }
   }
   st = launch_flush(c);
   if (st != PYCOOL_OK) return st;
@@ -820,12 +867,27 @@ int pycool_set_zchunk(pycool_ctx* c, int planes) {
   return set_geometry(c);
 }
 
+int pycool_set_persistent(pycool_ctx* c, int on) {
+  if (!c) return PYCOOL_EINVAL;
+  c->persistent = on != 0;
+  return PYCOOL_OK;
+}
+
+int pycool_set_fused_tail(pycool_ctx* c, int on) {
+  if (!c) return PYCOOL_EINVAL;
+  c->fused_tail = on != 0;
+  return PYCOOL_OK;
+}
+
 int pycool_set_tile(pycool_ctx* c, int tile) {
   if (!c) return PYCOOL_EINVAL;
   if (tile < -1 || tile >= kNumTiles) return fail(c, PYCOOL_EINVAL, "tile must be -1 (auto) .. %d", kNumTiles - 1);
   if (tile >= 0 && !tile_allowed(c->lay, tile))
     return fail(c, PYCOOL_EINVAL, "tile %d is a TMA variant: it needs the ghost layout (even N >= 4)", tile);
-  c->tile = tile < 0 ? auto_tile(c->lay) : tile;
+  if (tile >= 0 && (size_t)dispatch(c, OP_SMEM, tile) > kMaxSmem)
+    return fail(c, PYCOOL_EINVAL, "tile %d needs %zu bytes of shared memory for this model and precision (limit %zu)",
+                tile, (size_t)dispatch(c, OP_SMEM, tile), kMaxSmem);
+  c->tile = tile < 0 ? auto_tile(c) : tile;
   return set_geometry(c);
 }
 
