@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--precision", type=int, default=64, choices=[32, 64])
     ap.add_argument("--tile", type=int, default=-1)
     ap.add_argument("--zchunk", type=int, default=0)
+    ap.add_argument("--persistent", type=int, default=-1, help="1/0: persistent launch of the TMA kernel on/off (default: library's)")
+    ap.add_argument("--fused-tail", type=int, default=-1, help="1/0: fused stage tail on/off (default: library's)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -204,6 +206,10 @@ def main():
         lat.set_tile(a.tile)
     if a.zchunk > 0:
         lat.set_zchunk(a.zchunk)
+    if a.persistent >= 0:
+        lat.set_persistent(a.persistent)
+    if a.fused_tail >= 0:
+        lat.set_fused_tail(a.fused_tail)
     lat.set_fields(h_phi, h_pi)
     lat.set_background(1.0)
     lat.step(a.warmup)
@@ -224,6 +230,7 @@ def main():
     barrier()
     ev0.record(lat.stream)
     lat.step(a.steps)
+    lat.flush()                  # the deferred closing half drift belongs to these steps: inside the timed region
     ev1.record(lat.stream)
     barrier()
     ms = ev0.elapsed_time(ev1)

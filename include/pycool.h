@@ -122,7 +122,15 @@ int pycool_set_dt(pycool_ctx*, double dt);
  * sticky flag set and it has been observed by a synchronising call. */
 int pycool_step(pycool_ctx*, int nsteps);
 
-/* Wait for the context stream; returns PYCOOL_ENONFINITE / PYCOOL_ECUDA if the enqueued work failed. */
+/* The closing half drift H2(h_s/2) of a pycool_step call ((2.48)) is deferred: a following
+ * pycool_step merges it with its own opening half drift exactly as between two stages of one call, so
+ * step(1) x n and step(n) give bitwise the same state; every call that looks at the fields (read_fields*,
+ * device_fields, energies, set_background, sync) applies it first.  pycool_flush applies it now (asynchronous,
+ * one pointwise pass over phi); a no-op when nothing is pending. */
+int pycool_flush(pycool_ctx*);
+
+/* Apply a pending closing drift and wait for the context stream; returns PYCOOL_ENONFINITE / PYCOOL_ECUDA if
+ * the enqueued work failed. */
 int pycool_sync(pycool_ctx*);
 
 /* Download phi and/or pi (either may be NULL) to host memory.  Synchronises. */

@@ -22,7 +22,7 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
-           "pycool_set_fused_tail", "pycool_set_persistent")
+           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush")
 
 
 class Params(C.Structure):
@@ -90,6 +90,7 @@ def lib():
         L.pycool_set_tile.argtypes = [vp, ip]
         L.pycool_set_fused_tail.argtypes = [vp, ip]
         L.pycool_set_persistent.argtypes = [vp, ip]
+        L.pycool_flush.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -245,6 +246,10 @@ class Lattice:
 
     def set_zchunk(self, planes):
         self._chk(lib().pycool_set_zchunk(self._h, planes))
+
+    def flush(self):
+        """Apply the deferred closing half drift of the last step call now (asynchronous)."""
+        self._chk(lib().pycool_flush(self._h))
 
     def set_persistent(self, on):
         self._chk(lib().pycool_set_persistent(self._h, 1 if on else 0))

@@ -121,12 +121,14 @@ __device__ __forceinline__ double block_sum_fixed(const double* v, int n, double
 
 // The scalar side of the step, one thread.
 // mode 0: opening of a pycool_step call: H1(h_next/2), H2(h_next/2) scalar part, coefficients of the first kick.
+// mode 2: the same, continuing from a call whose closing half drift h/(2 a^2) has not been applied yet
+//         (s.c_drift): it merges with the opening half drift exactly as between two stages of one call.
 // mode 1: after the kick of a stage of length h, given its reduced sums (SD, SV, Spi2): H3 p_a; H2(h/2) p_a;
 //         H1(h/2); and, if h_next != 0, the opening of the next stage merged in: H1(h_next/2), H2(h_next/2) p_a,
 //         c_drift = h/(2 a_i^2) + h_next/(2 a_{i+1}^2).
 __device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k, double h, double h_next, int mode,
                                                double SD, double SV, double SP) {
-  double c1 = 0.0;
+  double c1 = mode == 2 ? s.c_drift : 0.0;     // mode 2: the previous call's closing half drift is still pending
   if (mode == 1) {
     s.SD = SD; s.SV = SV; s.Spi2 = SP;
     if (!(isfinite(SD) && isfinite(SV) && isfinite(SP))) s.nonfinite = 1;
@@ -171,7 +173,9 @@ scalar_update(Scalars* __restrict__ sc, const double* __restrict__ partials, int
 // the scalars: the stage needs no second launch.  The kernel's own reads of *sc all precede its ticket.
 struct StageTail {
   Scalars* sc;
-  unsigned int* ticket;   // nullptr: partials only (scalar_update follows as its own launch)
+  unsigned int* ticket;   // blocks-done counter, zero between launches
+  unsigned int* work;     // work-item claim counter of a persistent launch (kick_tma), zero between launches
+  int fused;              // 0: partials only (scalar_update follows as its own launch)
   ScalarConst k;
   double h, h_next;
 };
@@ -189,7 +193,6 @@ __device__ __forceinline__ void publish_partials(double* partials, unsigned npar
 template <int NT>
 __device__ __forceinline__ void stage_finish(const StageTail& t, const double* partials, unsigned nparts,
                                              double* sh /* >= NT doubles, free to overwrite */) {
-  if (!t.ticket) return;                        // grid-uniform
   __shared__ int is_last;
   if (threadIdx.x == 0) {
     __threadfence();
@@ -197,6 +200,11 @@ __device__ __forceinline__ void stage_finish(const StageTail& t, const double* p
   }
   __syncthreads();
   if (!is_last) return;
+  if (threadIdx.x == 0) {                      // every block is done: counters ready for the next launch
+    *t.ticket = 0u;
+    *t.work = 0u;
+  }
+  if (!t.fused) return;
   __threadfence();
   const double SD = block_sum_fixed<NT>(partials, (int)nparts, sh);
   const double SV = block_sum_fixed<NT>(partials + nparts, (int)nparts, sh);
@@ -205,7 +213,6 @@ __device__ __forceinline__ void stage_finish(const StageTail& t, const double* p
     Scalars s = *t.sc;
     scalar_advance(s, t.k, t.h, t.h_next, 1, SD, SV, SP);
     *t.sc = s;
-    *t.ticket = 0u;                            // ready for the next launch (stream order)
   }
 }
 

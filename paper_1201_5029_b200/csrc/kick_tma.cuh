@@ -99,10 +99,15 @@ struct TmaArgs {
   ModelParams mp;
 };
 
-// Work items are dealt round-robin: block b takes items b, b + gridDim.x, ...  With gridDim.x = nitems every
-// block has one item; with gridDim.x = (blocks resident on the GPU) the kernel is persistent and the TMA ring
-// runs on across item boundaries -- the first planes of the next item are in flight while the last planes of
-// the current one are computed, so no block ever waits for a cold pipeline except at the start of the launch.
+// Work items.  With gridDim.x = nitems every block has one item.  With fewer blocks (as many as are resident on
+// the GPU at once) the launch is persistent: a block's first item is its index, every further one is claimed
+// from a device counter a few planes before the current item's loads run out -- the order in which a hardware
+// block scheduler would hand them out, so the blocks in flight stay x-y neighbours within a few planes of each
+// other (their halo rows hit L2), however unequal the SMs' speeds.  (A fixed round-robin deal loses that: blocks
+// drift apart over ~28 items and DRAM reads grow 1.35x, measured.)  The TMA ring runs on across item
+// boundaries: the first planes of the next item are in flight while the last planes of the current one are
+// computed, so a block waits for a cold pipeline only once per launch.  Partial sums are indexed by item, so
+// results do not depend on which block computed what.
 template <typename Real, class Model, class T>
 __global__ void __launch_bounds__(T::NT, T::MINB)
 kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_pi,
@@ -126,8 +131,13 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   const int tx2 = tid % (TX / 2), tyj = tid / (TX / 2);
   const int nbxy = g.nbx * g.nby;
 
-  // ---- producer (thread 0): the stream of loads, item after item, plane z0-1 .. z0+nz of each
-  int pr_item = blockIdx.x, pr_i = 0, pr_x0 = 0, pr_y0 = 0, pr_z0 = 0, pr_nload = 0;
+  // ---- producer: the stream of loads, item after item, planes z0-1 .. z0+nz of each.  Every thread keeps the
+  // (block-uniform) bookkeeping; only thread 0 touches the barriers, the TMA unit and the claim counter.
+  __shared__ int item_ring[4];                                 // items of this block by sequence number (mod 4)
+  const bool dyn = (int)gridDim.x < g.nitems;
+  int pr_item = blockIdx.x, pr_seq = 0, pr_i = 0, pr_x0 = 0, pr_y0 = 0, pr_z0 = 0, pr_nload = 0;
+  bool pr_switch = false;                                      // current item's loads all issued
+  int claimed = 0x7fffffff;                                    // thread 0: the next item (none unless dyn)
   auto pr_decode = [&]() {
     if (pr_item < g.nitems) {
       const int bz = pr_item / nbxy, r = pr_item - bz * nbxy, by = r / g.nbx;
@@ -136,8 +146,14 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     }
     pr_i = 0;
   };
-  // Every thread keeps the (block-uniform) bookkeeping; only thread 0 touches the barrier and the TMA unit.
-  auto issue_next = [&](int s) {                               // next load of the stream into ring slot s
+  // Next load of the stream into ring slot s.  Call only after a block-wide barrier that follows the previous
+  // call (the item switch reads what thread 0 wrote during that call).
+  auto issue_next = [&](int s) {
+    if (pr_switch) {
+      pr_switch = false;
+      pr_item = item_ring[++pr_seq & 3];
+      pr_decode();
+    }
     if (pr_item >= g.nitems) return;
     if (tid == 0) {
       const uint32_t bar = bars + 8u * s;
@@ -148,8 +164,13 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
       gz = gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
       tma_load_4d(dst, &tm_phi, bar, pr_x0, pr_y0, gz, 0);     // box origin (x0-G, y0-1) in padded coordinates
       tma_load_4d(dst + (uint32_t)SM::BOXA, &tm_pi, bar, pr_x0, pr_y0, gz, 0);
+      // claim the next item a few planes ahead, so the counter's round trip is over when the value is needed
+      if (dyn && pr_i == max(pr_nload - 4, 0)) claimed = (int)(gridDim.x + atomicAdd(g.tail.work, 1u));
     }
-    if (++pr_i == pr_nload) { pr_item += gridDim.x; pr_decode(); }
+    if (++pr_i == pr_nload) {
+      if (tid == 0) item_ring[(pr_seq + 1) & 3] = claimed;     // INT_MAX ends the stream
+      pr_switch = true;
+    }
   };
 
   if (tid == 0) {
@@ -157,7 +178,10 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   pr_decode();
-  for (int s = 0; s < S; ++s) issue_next(s);
+  for (int s = 0; s < S; ++s) {
+    issue_next(s);
+    __syncthreads();                                           // also: barriers initialised before anyone waits
+  }
 
   const Real cd = Real(g.sc->c_drift), kD = Real(g.sc->kD), kV = Real(g.sc->kV);
   const Real c1 = Real(g.c1), c2 = Real(g.c2), c3 = Real(g.c3);
@@ -183,10 +207,9 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   int slot = 0;                                                // ring slot and phase of the next plane to consume
   uint32_t phase = 0;
 
-  __syncthreads();                                             // barriers initialised before anyone waits
-
+  int cs_seq = 0;
 #pragma unroll 1
-  for (int item = blockIdx.x; item < g.nitems; item += gridDim.x) {
+  for (int item = blockIdx.x; item < g.nitems; item = item_ring[++cs_seq & 3]) {
     const int bz = item / nbxy, rr_ = item - bz * nbxy, by = rr_ / g.nbx;
     const int x0 = (rr_ - by * g.nbx) * TX, y0 = by * TY, z0 = bz * g.zc;
     const int nz = min(g.zc, N - z0);

@@ -58,7 +58,7 @@ int stage_weights_ld(int order, long double* w) {
 constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
 constexpr size_t kMaxSmem = 227 * 1024;  // dynamic shared memory one block may opt in to on sm_100
 constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
-constexpr int kNumTiles = 12;            // + kick_tma variants (ghost layout only)
+constexpr int kNumTiles = 14;            // + kick_tma variants (ghost layout only)
 
 struct TileInfo { int tx, ty, nt, stages; };   // stages > 0: TMA ring depth
 
@@ -100,6 +100,7 @@ struct pycool_ctx {
   dim3 grid;
   // state
   bool have_fields = false, nonfinite_seen = false;
+  bool pending_drift = false;   // the closing half drift of the last step call is still to be applied to phi
   unsigned long long counts[4] = {0, 0, 0, 0};
   bool profiling = false;
   std::vector<cudaEvent_t> ev;   // pairs
@@ -134,7 +135,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
                                     {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 16, 512, 3}, {64, 16, 256, 4},
                                     {64, 16, 512, 4}, {128, 8, 256, 3}, {128, 8, 512, 3},
-                                    {128, 16, 512, 3}, {64, 32, 512, 3}};
+                                    {128, 16, 512, 3}, {64, 32, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}};
 using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 16, 2>;
@@ -148,6 +149,8 @@ template <typename Real> using TTile8 = TmaTile<Real, 128, 8, 3, 2, sizeof(Real)
 template <typename Real> using TTile9 = TmaTile<Real, 128, 8, 3, 1, 1>;   // 512 threads x (2 x 1 sites), 1 KB rows
 template <typename Real> using TTile10 = TmaTile<Real, 128, 16, 3, 2, 1>; // 512 threads x (2 x 2 sites): twice the
 template <typename Real> using TTile11 = TmaTile<Real, 64, 32, 3, 2, 1>;  //   bytes per plane (fp32, one field)
+template <typename Real> using TTile12 = TmaTile<Real, 32, 16, 3, 1, 2>;  // 256 threads x (2 x 1 sites), two blocks
+template <typename Real> using TTile13 = TmaTile<Real, 64, 8, 3, 1, 2>;   //   per SM: one fills its ring while the other runs
 
 // Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
 Layout make_layout(int N, int nf, size_t esize) {
@@ -271,7 +274,9 @@ int launch_kick_t(pycool_ctx* c) {
   g.sc = c->sc;
   g.partials = c->partials;
   g.tail.sc = c->sc;
-  g.tail.ticket = c->fused_tail ? c->ticket : nullptr;
+  g.tail.ticket = c->ticket;
+  g.tail.work = c->ticket + 1;
+  g.tail.fused = c->fused_tail ? 1 : 0;
   g.tail.k = c->kc;
   g.tail.h = c->h_cur;
   g.tail.h_next = c->h_next;
@@ -305,7 +310,9 @@ int launch_tma_t(pycool_ctx* c) {
   g.sc = c->sc;
   g.partials = c->partials;
   g.tail.sc = c->sc;
-  g.tail.ticket = c->fused_tail ? c->ticket : nullptr;
+  g.tail.ticket = c->ticket;
+  g.tail.work = c->ticket + 1;
+  g.tail.fused = c->fused_tail ? 1 : 0;
   g.tail.k = c->kc;
   g.tail.h = c->h_cur;
   g.tail.h_next = c->h_next;
@@ -313,6 +320,8 @@ int launch_tma_t(pycool_ctx* c) {
   g.zc = c->zc;
   g.nbx = (int)c->grid.x; g.nby = (int)c->grid.y;
   g.nitems = (int)(c->grid.x * c->grid.y * c->grid.z);
+  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
+  g.mp = c->mp;
   // persistent: one block per resident slot, items dealt round-robin; else one block per item
   const int nblocks = c->persistent && resident < g.nitems ? resident : g.nitems;
   c->blocks_launched = nblocks;
@@ -334,7 +343,9 @@ int launch_kick_m(pycool_ctx* c) {
     case 8: return launch_tma_t<Real, Model, TTile8<Real>>(c);
     case 9: return launch_tma_t<Real, Model, TTile9<Real>>(c);
     case 10: return launch_tma_t<Real, Model, TTile10<Real>>(c);
-    default: return launch_tma_t<Real, Model, TTile11<Real>>(c);
+    case 11: return launch_tma_t<Real, Model, TTile11<Real>>(c);
+    case 12: return launch_tma_t<Real, Model, TTile12<Real>>(c);
+    default: return launch_tma_t<Real, Model, TTile13<Real>>(c);
   }
 }
 template <typename Real, class Model>
@@ -351,7 +362,9 @@ size_t kick_smem_m(int tile) {
     case 8: return TmaSmem<Real, Model, TTile8<Real>>::TOTAL;
     case 9: return TmaSmem<Real, Model, TTile9<Real>>::TOTAL;
     case 10: return TmaSmem<Real, Model, TTile10<Real>>::TOTAL;
-    default: return TmaSmem<Real, Model, TTile11<Real>>::TOTAL;
+    case 11: return TmaSmem<Real, Model, TTile11<Real>>::TOTAL;
+    case 12: return TmaSmem<Real, Model, TTile12<Real>>::TOTAL;
+    default: return TmaSmem<Real, Model, TTile13<Real>>::TOTAL;
   }
 }
 template <typename Real, class Model>
@@ -431,6 +444,15 @@ int launch_flush(pycool_ctx* c) {
   CUDA_TRY(c, cudaGetLastError());
   c->counts[2]++;
   return PYCOOL_OK;
+}
+
+// The closing half drift of a pycool_step call is deferred: a following pycool_step merges it with its own
+// opening half drift (exactly as between two stages of one call, so step(1) x n == step(n) bit for bit); anything
+// that looks at phi applies it first.
+int ensure_flushed(pycool_ctx* c) {
+  if (!c->pending_drift) return PYCOOL_OK;
+  c->pending_drift = false;
+  return launch_flush(c);
 }
 
 int launch_sum_pi2(pycool_ctx* c) {
@@ -643,6 +665,7 @@ int pycool_create_ext(pycool_ctx** out, int N, double L, int nfields, const pyco
 
 static int upload(pycool_ctx* c, const void* phi, const void* pi, cudaMemcpyKind kind) {
   c->cur = 0;
+  c->pending_drift = false;
   int st = copy_dense(c, c->phi[0], const_cast<void*>(phi), true, kind);
   if (st == PYCOOL_OK) st = copy_dense(c, c->pi[0], const_cast<void*>(pi), true, kind);
   if (st == PYCOOL_OK) st = launch_fill_ghosts(c, c->phi[0]);
@@ -672,6 +695,7 @@ int pycool_set_fields_device(pycool_ctx* c, const void* d_phi_src, const void* d
 int pycool_set_background(pycool_ctx* c, double a, double p_a) {
   if (!c) return PYCOOL_EINVAL;
   if (!(a > 0) || !std::isfinite(a)) return fail(c, PYCOOL_EINVAL, "a must be finite and > 0");
+  if (int st = ensure_flushed(c)) return st;
   if (std::isnan(p_a)) {                                   // reading G10: (2.18), expanding branch
     if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "p_a = NaN needs fields (call set_fields first)");
     if (std::isinf(c->mpl)) return fail(c, PYCOOL_EINVAL, "p_a = NaN with a static background (mpl = INF)");
@@ -705,7 +729,7 @@ int pycool_step(pycool_ctx* c, int nsteps) {
   if (nsteps == 0) return PYCOOL_OK;
   const int ns = c->nstages;
   const long long S = (long long)nsteps * ns;
-  int st = launch_scalar(c, 0.0, c->w[0] * c->dt, 0);
+  int st = launch_scalar(c, 0.0, c->w[0] * c->dt, c->pending_drift ? 2 : 0);
   if (st != PYCOOL_OK) return st;
   if (c->profiling && c->ev.size() < c->ev_used + 2 * (size_t)S) {
     const size_t want = c->ev_used + 2 * (size_t)S;
@@ -731,14 +755,19 @@ int pycool_step(pycool_ctx* c, int nsteps) {
       if (st != PYCOOL_OK) return st;
     }
   }
-  st = launch_flush(c);
-  if (st != PYCOOL_OK) return st;
+  c->pending_drift = true;
   for (int i = 0; i < nsteps; ++i) c->eta += c->dt;
   return PYCOOL_OK;
 }
 
+int pycool_flush(pycool_ctx* c) {
+  if (!c) return PYCOOL_EINVAL;
+  return ensure_flushed(c);
+}
+
 int pycool_sync(pycool_ctx* c) {
   if (!c) return PYCOOL_EINVAL;
+  if (int st = ensure_flushed(c)) return st;
   Scalars s;
   return read_scalars(c, &s);
 }
@@ -746,7 +775,8 @@ int pycool_sync(pycool_ctx* c) {
 int pycool_read_fields(pycool_ctx* c, void* phi_host, void* pi_host) {
   if (!c) return PYCOOL_EINVAL;
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "read before set_fields");
-  int st = PYCOOL_OK;
+  int st = ensure_flushed(c);
+  if (st != PYCOOL_OK) return st;
   if (phi_host) st = copy_dense(c, c->phi[c->cur], phi_host, false, cudaMemcpyDeviceToHost);
   if (st == PYCOOL_OK && pi_host) st = copy_dense(c, c->pi[c->cur], pi_host, false, cudaMemcpyDeviceToHost);
   if (st != PYCOOL_OK) return st;
@@ -757,7 +787,8 @@ int pycool_read_fields(pycool_ctx* c, void* phi_host, void* pi_host) {
 int pycool_read_fields_device(pycool_ctx* c, void* d_phi_dst, void* d_pi_dst) {
   if (!c) return PYCOOL_EINVAL;
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "read before set_fields");
-  int st = PYCOOL_OK;
+  int st = ensure_flushed(c);
+  if (st != PYCOOL_OK) return st;
   if (d_phi_dst) st = copy_dense(c, c->phi[c->cur], d_phi_dst, false, cudaMemcpyDeviceToDevice);
   if (st == PYCOOL_OK && d_pi_dst) st = copy_dense(c, c->pi[c->cur], d_pi_dst, false, cudaMemcpyDeviceToDevice);
   return st;
@@ -765,6 +796,7 @@ int pycool_read_fields_device(pycool_ctx* c, void* d_phi_dst, void* d_pi_dst) {
 
 int pycool_device_fields(pycool_ctx* c, void** d_phi, void** d_pi, size_t layout[4]) {
   if (!c) return PYCOOL_EINVAL;
+  if (int st = ensure_flushed(c)) return st;
   if (d_phi) *d_phi = c->phi[c->cur];
   if (d_pi) *d_pi = c->pi[c->cur];
   if (layout) {
@@ -778,8 +810,10 @@ int pycool_energies(pycool_ctx* c, pycool_energy* o) {
   if (!c) return PYCOOL_EINVAL;
   if (!o) return fail(c, PYCOOL_EINVAL, "out is NULL");
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "energies before set_fields");
+  int st = ensure_flushed(c);
+  if (st != PYCOOL_OK) return st;
   Scalars s;
-  int st = read_scalars(c, &s);
+  st = read_scalars(c, &s);
   if (st != PYCOOL_OK) return st;
   Averages av;
   st = averages(c, s.a, &av);

@@ -144,12 +144,12 @@ def set_tile_or_skip(pc, g, tile):
     try:
         g.set_tile(tile)
     except pc.PycoolError as e:
-        assert e.code == pc.EINVAL and tile >= 10 and "shared memory" in str(e)
+        assert e.code == pc.EINVAL and tile in (10, 11) and "shared memory" in str(e)
         return False
     return True
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13])
 @pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32), (6, 0),
                                   (70, 9), (136, 50)])
 def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
@@ -184,7 +184,7 @@ def test_variants_agree_and_ghost_images_hold(pc, precision):
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg, precision=precision)
     outs = []
-    for tile in range(12):
+    for tile in range(14):
         g = pc.from_config(cfg, precision=precision)
         if not set_tile_or_skip(pc, g, tile):
             assert precision == 64
@@ -231,7 +231,7 @@ def test_fused_tail_equals_separate_scalar_update(pc, tile, N):
         g.step(2); g.step(1); o.step(3)
         compare(g, o, 2, 5e-12)
         kicks, scalars, flushes, _ = g.launch_counts()
-        assert kicks == 9 and flushes == 2 and scalars == (2 if fused else 2 + 9)
+        assert kicks == 9 and flushes == 1 and scalars == (2 if fused else 2 + 9)   # one deferred closing drift
         outs.append((g.read_fields(), g.energies()))
     (pa, qa), ea = outs[0]
     (pb, qb), eb = outs[1]
@@ -239,7 +239,7 @@ def test_fused_tail_equals_separate_scalar_update(pc, tile, N):
     assert rel(ea.a, eb.a) < 1e-14 and rel(ea.p_a, eb.p_a) < 1e-13
 
 
-@pytest.mark.parametrize("tile,N,zc", [(3, 136, 5), (4, 70, 3), (8, 260, 4), (5, 136, 1), (4, 40, 1)])
+@pytest.mark.parametrize("tile,N,zc", [(3, 136, 5), (4, 70, 1), (8, 260, 4), (5, 136, 1), (13, 72, 1)])
 def test_persistent_launch_is_bitwise_the_one_block_per_item_launch(pc, tile, N, zc):
     """More work items than resident blocks (short z-chunks): every block walks several items with its TMA ring
     running on across them (ragged tiles, lattice faces and z-wrap included).  Partial sums are indexed by work
@@ -256,7 +256,7 @@ def test_persistent_launch_is_bitwise_the_one_block_per_item_launch(pc, tile, N,
         e = g.energies()
         outs.append((g.read_fields(), (e.a, e.p_a, e.pot, e.kin[0], e.grad[1])))
         if persistent:
-            assert g.kick_geometry()["blocks"] > 148 * 2       # really more items than any B200 holds at once
+            assert g.kick_geometry()["blocks"] > 148 * 3       # really more items than a B200 holds at once
     assert np.array_equal(outs[0][0][0], outs[1][0][0]) and np.array_equal(outs[0][0][1], outs[1][0][1])
     assert outs[0][1] == outs[1][1]
     if N <= 136:
@@ -300,7 +300,9 @@ def test_bitwise_reproducible(pc):
 
 
 def test_step_split_equals_one_call(pc):
-    """pycool_step(3) and three pycool_step(1) calls agree to rounding (merged vs separate half drifts)."""
+    """pycool_step(3) and three pycool_step(1) calls are bitwise the same: the closing half drift of a call is
+    deferred and merges with the next call's opening drift like two stages of one call; pycool_flush in between
+    applies it separately instead (agreement to rounding)."""
     cfg = inputs.config("cfg0_chaotic32", N=24)
     phi, pi = inputs.make_initial(cfg)
     a, b = pc.from_config(cfg), pc.from_config(cfg)
@@ -310,10 +312,21 @@ def test_step_split_equals_one_call(pc):
     a.step(3)
     for _ in range(3):
         b.step(1)
+    c = pc.from_config(cfg)
+    c.set_fields(phi, pi)
+    c.set_background(1.0)
+    for _ in range(3):
+        c.step(1)
+        c.flush()
+    assert a.launch_counts()[2] == 0 and b.launch_counts()[2] == 0 and c.launch_counts()[2] == 3
     pa, qa = a.read_fields()
     pb, qb = b.read_fields()
-    assert rel_err_per_site(pa, pb) < 1e-14 and rel_err_per_site(qa, qb) < 1e-14
-    assert rel(a.energies().a, b.energies().a) < 1e-14 and abs(a.energies().eta - 3 * cfg["dt"]) < 1e-15
+    pc_, qc = c.read_fields()
+    assert a.launch_counts()[2] == 1 and c.launch_counts()[2] == 3
+    assert np.array_equal(pa, pb) and np.array_equal(qa, qb)
+    assert a.energies().a == b.energies().a and a.energies().p_a == b.energies().p_a
+    assert rel_err_per_site(pa, pc_) < 1e-14 and rel_err_per_site(qa, qc) < 1e-14
+    assert rel(a.energies().a, c.energies().a) < 1e-14 and abs(a.energies().eta - 3 * cfg["dt"]) < 1e-15
 
 
 # ------------------------------------------------------------------------------------- free model, stencils
