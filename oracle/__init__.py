@@ -47,6 +47,7 @@ def lib():
         L.oracle_set_fields.argtypes = [vp, vp, vp]
         L.oracle_set_background.argtypes = [vp, C.c_double, C.c_double]
         L.oracle_set_dt.argtypes = [vp, C.c_double]
+        L.oracle_set_adaptive.argtypes = [vp, C.c_int]
         L.oracle_step.argtypes = [vp, ip]
         L.oracle_read_fields.argtypes = [vp, vp, vp]
         L.oracle_energies.argtypes = [vp, C.POINTER(Energy)]
@@ -118,6 +119,10 @@ class Oracle:
 
     def set_dt(self, dt):
         self._chk(lib().oracle_set_dt(self._h, dt))
+
+    def set_adaptive(self, on=True):
+        """dt becomes a physical-time increment: step n has conformal length dt / a_n."""
+        self._chk(lib().oracle_set_adaptive(self._h, 1 if on else 0))
 
     def step(self, n=1):
         self._chk(lib().oracle_step(self._h, n))

@@ -89,6 +89,7 @@ struct Base {
   virtual int set_fields(const void*, const void*) = 0;
   virtual int set_background(double, double) = 0;
   virtual int set_dt(double) = 0;
+  virtual int set_adaptive(int) = 0;
   virtual int step(int) = 0;
   virtual int read_fields(void*, void*) = 0;
   virtual int energies(oracle_energy*) = 0;
@@ -109,6 +110,7 @@ struct Stepper : Base {
   S c[4];               /* stencil weights by neighbour class d = 0..3 */
   std::vector<T> phi, pi;
   bool have_fields = false, nonfinite = false;
+  bool adaptive = false;  /* dt is a physical-time increment: each step uses d eta = dt / a */
 
   size_t idx(int f, int x, int y, int z) const {
     return (size_t)f * V + ((size_t)z * N + (size_t)y) * N + (size_t)x;
@@ -231,8 +233,11 @@ struct Stepper : Base {
     long double w[16];
     int s = stage_weights(order, w);
     for (int it = 0; it < n; ++it) {
-      for (int i = 0; i < s; ++i) phi2(S(w[i]) * dt);                       /* (2.43)/(2.45) */
-      eta += dt;
+      /* "adaptive conformal step with constant increases in physical time": dt_phys = a d eta,
+         so the conformal length of this step is dt / a with a taken at the start of the step (reading G20) */
+      const S de = adaptive ? dt / a : dt;
+      for (int i = 0; i < s; ++i) phi2(S(w[i]) * de);                       /* (2.43)/(2.45) */
+      eta += de;
     }
     if (nonfinite) { err = "non-finite lattice sum"; return ORACLE_ENONFINITE; }
     return ORACLE_OK;
@@ -332,6 +337,8 @@ struct Stepper : Base {
     return ORACLE_OK;
   }
 
+  int set_adaptive(int on) override { adaptive = on != 0; return ORACLE_OK; }
+
   int laplacian(int f, double* out) override {
     if (f < 0 || f >= nf || !out) { err = "bad field index"; return ORACLE_EINVAL; }
     for (int z = 0; z < N; ++z) for (int y = 0; y < N; ++y) for (int x = 0; x < N; ++x)
@@ -417,6 +424,7 @@ int oracle_create(oracle_ctx** out, int N, double L, int nfields, const oracle_p
 int oracle_set_fields(oracle_ctx* c, const void* phi, const void* pi) { return c ? c->impl->set_fields(phi, pi) : ORACLE_EINVAL; }
 int oracle_set_background(oracle_ctx* c, double a, double p_a) { return c ? c->impl->set_background(a, p_a) : ORACLE_EINVAL; }
 int oracle_set_dt(oracle_ctx* c, double dt) { return c ? c->impl->set_dt(dt) : ORACLE_EINVAL; }
+int oracle_set_adaptive(oracle_ctx* c, int on) { return c ? c->impl->set_adaptive(on) : ORACLE_EINVAL; }
 int oracle_step(oracle_ctx* c, int n) { return c ? c->impl->step(n) : ORACLE_EINVAL; }
 int oracle_read_fields(oracle_ctx* c, void* phi, void* pi) { return c ? c->impl->read_fields(phi, pi) : ORACLE_EINVAL; }
 int oracle_energies(oracle_ctx* c, oracle_energy* o) { return c ? c->impl->energies(o) : ORACLE_EINVAL; }

@@ -53,6 +53,9 @@ int oracle_set_fields(oracle_ctx*, const void* phi, const void* pi);
 /* p_a = NaN => solve the first Friedmann equation (2.18) on the current lattice (expanding branch). */
 int oracle_set_background(oracle_ctx*, double a, double p_a);
 int oracle_set_dt(oracle_ctx*, double dt);
+/* on: dt is a constant PHYSICAL-time increment; step n has conformal length dt / a_n, a_n the scale factor at
+ * the start of the step ("adaptive conformal step with constant increases in physical time"). */
+int oracle_set_adaptive(oracle_ctx*, int on);
 int oracle_step(oracle_ctx*, int nsteps);
 int oracle_read_fields(oracle_ctx*, void* phi, void* pi);
 int oracle_energies(oracle_ctx*, oracle_energy* out);

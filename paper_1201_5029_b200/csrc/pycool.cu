@@ -180,13 +180,7 @@ int blocks_xy(int N, int tile) {
   const TileInfo& t = kTiles[tile];
   return ((N + t.tx - 1) / t.tx) * ((N + t.ty - 1) / t.ty);
 }
-// z-chunk: enough blocks to fill 148 SMs several times over, chunks not shorter than 16 planes unless N is
-int auto_zchunk(int N, int tile) {
-  const int bxy = blocks_xy(N, tile);
-  int zc = N;
-  while (zc > 16 && (long long)bxy * ((N + zc - 1) / zc) < 148LL * 16) zc = (zc + 1) / 2;
-  return zc < 1 ? 1 : zc;
-}
+int auto_zchunk(pycool_ctx* c);
 // partial-sum capacity actually reserved: automatic geometry of every tile with zc >= min(N, 4)
 size_t partials_capacity(int N) {
   size_t m = 13 * (size_t)kMaxSumBlocks;
@@ -288,22 +282,32 @@ int launch_kick_t(pycool_ctx* c) {
   CUDA_TRY(c, cudaGetLastError());
   return PYCOOL_OK;
 }
+// Blocks of this kick_tma instance that fit on the device at once (0 on error, message in c->err); the first
+// call also opts the instance in to its dynamic shared memory.
+template <typename Real, class Model, class T>
+int tma_resident(pycool_ctx* c) {
+  static int resident = -1;
+  if (resident >= 0) return resident;
+  constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
+  int per_sm = 0, dev = 0, sms = 0;
+  cudaError_t e = cudaFuncSetAttribute(kick_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kick_tma<Real, Model, T>, T::NT, smem);
+  if (e == cudaSuccess) e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess || per_sm * sms < 1) {
+    fail(c, PYCOOL_ECUDA, "kick_tma does not fit on an SM (%zu bytes of shared memory): %s", smem, cudaGetErrorString(e));
+    cudaGetLastError();
+    return 0;
+  }
+  resident = per_sm * sms;
+  return resident;
+}
+
 template <typename Real, class Model, class T>
 int launch_tma_t(pycool_ctx* c) {
-  static bool attr_done = false;
-  static int resident = 0;            // blocks of this instance that fit on the device at once
   constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
-  if (!attr_done) {
-    CUDA_TRY(c, cudaFuncSetAttribute(kick_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)smem));
-    int per_sm = 0, dev = 0, sms = 0;
-    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kick_tma<Real, Model, T>, T::NT, smem));
-    CUDA_TRY(c, cudaGetDevice(&dev));
-    CUDA_TRY(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    resident = per_sm * sms;
-    if (resident < 1) return fail(c, PYCOOL_ECUDA, "kick_tma does not fit on an SM (%zu bytes of shared memory)", smem);
-    attr_done = true;
-  }
+  const int resident = tma_resident<Real, Model, T>(c);
+  if (resident < 1) return PYCOOL_ECUDA;
   TmaArgs<Real> g;
   g.phi_out = (Real*)c->phi[c->cur ^ 1];
   g.pi_out = (Real*)c->pi[c->cur ^ 1];
@@ -368,6 +372,23 @@ size_t kick_smem_m(int tile) {
   }
 }
 template <typename Real, class Model>
+int kick_resident_m(pycool_ctx* c, int tile) {
+  switch (tile) {
+    case 0: case 1: case 2: return 2 * 148;             // register-prefetch kernel: not persistent, a guess does
+    case 3: return tma_resident<Real, Model, TTile3<Real>>(c);
+    case 4: return tma_resident<Real, Model, TTile4<Real>>(c);
+    case 5: return tma_resident<Real, Model, TTile5<Real>>(c);
+    case 6: return tma_resident<Real, Model, TTile6<Real>>(c);
+    case 7: return tma_resident<Real, Model, TTile7<Real>>(c);
+    case 8: return tma_resident<Real, Model, TTile8<Real>>(c);
+    case 9: return tma_resident<Real, Model, TTile9<Real>>(c);
+    case 10: return tma_resident<Real, Model, TTile10<Real>>(c);
+    case 11: return tma_resident<Real, Model, TTile11<Real>>(c);
+    case 12: return tma_resident<Real, Model, TTile12<Real>>(c);
+    default: return tma_resident<Real, Model, TTile13<Real>>(c);
+  }
+}
+template <typename Real, class Model>
 int launch_energy_m(pycool_ctx* c, int nb) {
   energy_sums<Real, Model><<<nb, 256, 0, c->stream>>>((const Real*)c->phi[c->cur], (const Real*)c->pi[c->cur],
                                                       c->lay, c->c[1], c->c[2], c->c[3], c->mp, c->partials);
@@ -375,13 +396,14 @@ int launch_energy_m(pycool_ctx* c, int nb) {
   return PYCOOL_OK;
 }
 
-enum Op { OP_KICK, OP_ENERGY, OP_SMEM };
+enum Op { OP_KICK, OP_ENERGY, OP_SMEM, OP_RESIDENT };
 template <typename Real>
 long long dispatch_model(pycool_ctx* c, Op op, int arg) {
 #define PYCOOL_CASE(M)                                                    \
   do {                                                                    \
     if (op == OP_KICK) return launch_kick_m<Real, M>(c);                  \
     if (op == OP_ENERGY) return launch_energy_m<Real, M>(c, arg);         \
+    if (op == OP_RESIDENT) return kick_resident_m<Real, M>(c, arg);       \
     return (long long)kick_smem_m<Real, M>(arg);                          \
   } while (0)
   switch (c->model) {
@@ -402,21 +424,50 @@ long long dispatch(pycool_ctx* c, Op op, int arg) {
   return c->precision == 32 ? dispatch_model<float>(c, op, arg) : dispatch_model<double>(c, op, arg);
 }
 
-// Automatic variant: the register-prefetch kernel where the layout has no ghosts (odd N); else the first TMA
-// variant of a measured preference list whose ring fits in shared memory for this model and precision.
+// Automatic variant (measured on B200, profiles/): the register-prefetch kernel where the layout has no ghosts
+// (odd N); else the first TMA variant of a preference list whose ring fits in shared memory.
+//   two fields fp64 / anything fp32: 64 x 16 tile (fp32 instances are cut for two blocks per SM);
+//   one field fp64: 128 x 16 (a plane of a 64 x 16 box is too few bytes in flight);
+//   Q-ball (the logarithm makes it ALU-heavy): 32 x 16 with 2 x 1 sites per thread, two blocks per SM.
 int auto_tile(pycool_ctx* c) {
   const Layout& L = c->lay;
   if (L.gx == 0) return L.N <= 64 ? 0 : 1;
   if (L.N <= 64) return 4;
-  static const int pref[] = {3, 4};
-  for (int t : pref)
-    if ((size_t)dispatch(c, OP_SMEM, t) <= kMaxSmem) return t;
+  static const int pref_default[] = {3, 4}, pref_one[] = {10, 3, 4}, pref_alu[] = {12, 4};
+  const int* pref = pref_default;
+  int n = 2;
+  if (c->model == PYCOOL_QBALL) { pref = pref_alu; n = 2; }
+  else if (c->nf == 1 && c->precision == 64) { pref = pref_one; n = 3; }
+  for (int i = 0; i < n; ++i)
+    if ((size_t)dispatch(c, OP_SMEM, pref[i]) <= kMaxSmem) return pref[i];
   return 1;
+}
+
+// Automatic z-chunk.  Short chunks keep the blocks in flight (x-y neighbours) within a few planes of each other,
+// so their halo rows hit L2; each chunk re-reads two halo planes.  Measured optimum for lattices with many
+// items per resident block: 16 planes (32 at N >= 1024).  Small lattices: the chunk length that minimises
+// rounds x (planes + 2 halo planes) + pipeline fill over the resident blocks.
+int auto_zchunk(pycool_ctx* c) {
+  const int N = c->N, bxy = blocks_xy(N, c->tile);
+  if (N <= 16) return N;
+  int R = (int)dispatch(c, OP_RESIDENT, c->tile);
+  if (R < 1) R = 148;
+  const int cap = N >= 1024 ? 32 : 16;
+  auto items = [&](int zc) { return (long long)bxy * ((N + zc - 1) / zc); };
+  if (items(cap) >= 4LL * R) return cap;
+  int best = cap;
+  long long best_cost = -1;
+  for (int zc = cap; zc <= N; zc += 8) {
+    const long long rounds = (items(zc) + R - 1) / R;
+    const long long cost = rounds * (zc + 2) + 4;
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = zc; }
+  }
+  return best;
 }
 
 int set_geometry(pycool_ctx* c) {
   const TileInfo& t = kTiles[c->tile];
-  int zc = c->zc_user > 0 ? c->zc_user : auto_zchunk(c->N, c->tile);
+  int zc = c->zc_user > 0 ? c->zc_user : auto_zchunk(c);
   if (zc > c->N) zc = c->N;
   // never exceed the reserved partial-sum capacity
   while (3 * (size_t)blocks_xy(c->N, c->tile) * (size_t)((c->N + zc - 1) / zc) > c->partials_cap) ++zc;

@@ -202,6 +202,71 @@ def test_p8_matter_only_quadratic_a():
     assert e.residual < 1e-13                                    # a'^2 = a rho_m0/(3 mpl^2) holds exactly
 
 
+# ---------------------------------------------------------------- P14: adaptive conformal step
+@pytest.mark.parametrize("order", [2, 4, 6])
+def test_p14_adaptive_step_radiation_only_recurrence(order):
+    """Constant physical-time increments: step n has conformal length dt / a_n.  Radiation only: a' = C is
+    constant, so a_{n+1} = a_n + C dt / a_n and eta_{n+1} = eta_n + dt / a_n exactly, whatever the order; the
+    continuum law is a^2 = a_0^2 + 2 C t (radiation domination), which the recurrence follows to O(dt)."""
+    N, mpl, rg, dt, n = 3, 1.5, 3.0, 0.02, 50
+    o = Oracle(N, 1.0, 1, FREE, [0.0], order=order, dt=dt, mpl=mpl, rho_gamma0=rg)
+    o.set_fields(np.zeros((1, N, N, N)), np.zeros((1, N, N, N)))
+    o.set_background(1.0)
+    o.set_adaptive(True)
+    o.step(n)
+    C = math.sqrt(rg / 3) / mpl
+    a, eta = np.longdouble(1), np.longdouble(0)
+    for _ in range(n):
+        h = np.longdouble(dt) / a
+        a, eta = a + np.longdouble(C) * h, eta + h
+    e = o.energies()
+    assert abs(e.a - float(a)) < 1e-13 and abs(e.eta - float(eta)) < 1e-13
+    assert abs(e.a ** 2 - (1 + 2 * C * n * dt)) < 2 * C * C * n * dt * dt        # a^2 = a0^2 + 2 C t + O(dt)
+    assert e.residual < 1e-13
+
+
+def test_p14_adaptive_step_matter_only_uses_a_at_step_start():
+    """Matter only: p_a' = -V_L rho_m0 is a constant force, the leapfrog is exact within a step of conformal
+    length h_n = dt / a_n: a_{n+1} = a_n + a'_n h_n + F h_n^2 / 2, a'_{n+1} = a'_n + F h_n, F = rho_m0/(6 mpl^2).
+    Taking a at mid-step or at the end instead of at the start of the step fails this at the 1e-4 level."""
+    N, mpl, rm, dt, n = 3, 0.8, 2.0, 0.05, 20
+    o = Oracle(N, 1.0, 1, FREE, [0.0], order=4, dt=dt, mpl=mpl, rho_m0=rm)
+    o.set_fields(np.zeros((1, N, N, N)), np.zeros((1, N, N, N)))
+    o.set_background(1.0)
+    o.set_adaptive(True)
+    o.step(n)
+    LD = np.longdouble
+    a, ap, F, eta = LD(1), LD(math.sqrt(rm / 3) / mpl), LD(rm) / (6 * LD(mpl) ** 2), LD(0)
+    a_end_rule = a
+    for _ in range(n):
+        h = LD(dt) / a
+        a, ap, eta = a + ap * h + F * h * h / 2, ap + F * h, eta + h
+    e = o.energies()
+    assert abs(e.a - float(a)) < 1e-13 and abs(e.eta - float(eta)) < 1e-13
+    assert abs(e.hubble - float(ap / (a * a))) < 1e-13
+    # the wrong reading (h from the a at the END of the previous update but one step late) is far outside
+    b, bp = LD(1), LD(math.sqrt(rm / 3) / mpl)
+    for _ in range(n):
+        h = LD(dt) / (b + bp * LD(dt) / b / 2)                   # mid-step a
+        b, bp = b + bp * h + F * h * h / 2, bp + F * h
+    assert abs(float(b) - e.a) > 1e-5
+
+
+def test_p14_adaptive_off_is_the_fixed_step():
+    cfg_kw = dict(order=4, dt=0.01, mpl=1.0)
+    rng = np.random.default_rng(3)
+    phi = 0.3 + 0.01 * rng.standard_normal((1, 6, 6, 6)); pi = 0.01 * rng.standard_normal((1, 6, 6, 6))
+    outs = []
+    for mode in (None, False):
+        o = Oracle(6, 2.0, 1, FREE, [1.0], **cfg_kw)
+        o.set_fields(phi, pi); o.set_background(1.0)
+        if mode is not None:
+            o.set_adaptive(mode)
+        o.step(5)
+        outs.append(o.read_fields())
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
 # ---------------------------------------------------------------- P9: homogeneous FRW + field vs ODE solver
 def test_p9_homogeneous_frw_against_ode_solver():
     from scipy.integrate import solve_ivp
