@@ -116,6 +116,11 @@ int pycool_set_background(pycool_ctx*, double a, double p_a);
 
 int pycool_set_dt(pycool_ctx*, double dt);
 
+/* on != 0: dt becomes a constant PHYSICAL-time increment: step n has conformal length dt / a_n, a_n the scale
+ * factor at the start of that step, computed on the device ("adaptive conformal step with constant increases in
+ * physical time").  pycool_energy.eta is the sum of the lengths.  Default off. */
+int pycool_set_adaptive(pycool_ctx*, int on);
+
 /* Advance nsteps >= 0 whole steps of length dt.  Asynchronous: kernels are enqueued on the context stream
  * (no host synchronisation inside, a and p_a live on the device).  On return from a later synchronising call
  * the state is time-synchronised at eta + nsteps*dt.  Returns PYCOOL_ENONFINITE if an EARLIER call left the

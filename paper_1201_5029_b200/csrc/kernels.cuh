@@ -65,6 +65,8 @@ struct Scalars {          // device-resident; one per context
   double Spi2, SD, SV;    // sum pi^2 (current pi), sum_f phi_f D[phi_f], sum V of the latest kick
   double c_drift;         // pending drift coefficient: phi += c_drift * pi before the next kick
   double kD, kV;          // a^2 h/dx^2 and a^4 h of the next kick
+  double dt_cur;          // conformal length of the current step (= dt, or dt / a at its start when adaptive)
+  double eta;             // conformal time: sum of the completed steps' lengths
   int nonfinite;          // sticky: a lattice sum was NaN/Inf
   int pad;
 };
@@ -119,6 +121,15 @@ __device__ __forceinline__ double block_sum_fixed(const double* v, int n, double
   return r;
 }
 
+// Lengths of a stage and of the one after it, as weights of the step length.
+struct StageLen {
+  double w, w_next;   // stage weights (2.42)-(2.45), Table 1; w_next = 0: the call ends after this stage
+  double dt;          // the fixed conformal step, or the physical-time increment when adaptive
+  int adaptive;       // step length = dt / a(start of the step): "adaptive conformal step with constant
+                      // increases in physical time"
+  int ends_step;      // this stage is the last of its step
+};
+
 // The scalar side of the step, one thread.
 // mode 0: opening of a pycool_step call: H1(h_next/2), H2(h_next/2) scalar part, coefficients of the first kick.
 // mode 2: the same, continuing from a call whose closing half drift h/(2 a^2) has not been applied yet
@@ -126,10 +137,12 @@ __device__ __forceinline__ double block_sum_fixed(const double* v, int n, double
 // mode 1: after the kick of a stage of length h, given its reduced sums (SD, SV, Spi2): H3 p_a; H2(h/2) p_a;
 //         H1(h/2); and, if h_next != 0, the opening of the next stage merged in: H1(h_next/2), H2(h_next/2) p_a,
 //         c_drift = h/(2 a_i^2) + h_next/(2 a_{i+1}^2).
-__device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k, double h, double h_next, int mode,
+__device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k, const StageLen& len, int mode,
                                                double SD, double SV, double SP) {
+  const double step_len = len.adaptive ? s.dt_cur : len.dt;
   double c1 = mode == 2 ? s.c_drift : 0.0;     // mode 2: the previous call's closing half drift is still pending
   if (mode == 1) {
+    const double h = __dmul_rn(len.w, step_len);
     s.SD = SD; s.SV = SV; s.Spi2 = SP;
     if (!(isfinite(SD) && isfinite(SV) && isfinite(SP))) s.nonfinite = 1;
     flow_H3_pa(s, k, h);                       // H3(h), scalar part
@@ -137,8 +150,15 @@ __device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k,
     flow_H2_pa(s, k, e);                       // H2(h/2), scalar part (pi is constant in H2: post-kick sum)
     c1 = drift_coef(s, e);                     //          field part, applied by the next kernel
     flow_H1(s, k, e);                          // H1(h/2)
+    if (len.ends_step) s.eta = __dadd_rn(s.eta, step_len);
   }
-  if (h_next != 0.0) {
+  if (len.w_next != 0.0) {
+    double next_len = step_len;
+    if (mode != 1 || len.ends_step) {          // a new step begins: its length from the a it starts with
+      next_len = len.adaptive ? __ddiv_rn(len.dt, s.a) : len.dt;
+      s.dt_cur = next_len;
+    }
+    const double h_next = __dmul_rn(len.w_next, next_len);
     const double e = __ddiv_rn(h_next, 2.0);
     flow_H1(s, k, e);                          // H1(h_next/2)
     flow_H2_pa(s, k, e);                       // H2(h_next/2), scalar part
@@ -153,7 +173,7 @@ __device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k,
 // call (mode 0) and when the fused tail is switched off.
 __global__ void __launch_bounds__(kReduceThreads)
 scalar_update(Scalars* __restrict__ sc, const double* __restrict__ partials, int nblocks, ScalarConst k,
-              double h, double h_next, int mode) {
+              StageLen len, int mode) {
   __shared__ double sh[kReduceThreads];
   double SD = 0, SV = 0, SP = 0;
   if (mode == 1) {
@@ -163,7 +183,7 @@ scalar_update(Scalars* __restrict__ sc, const double* __restrict__ partials, int
   }
   if (threadIdx.x != 0) return;
   Scalars s = *sc;
-  scalar_advance(s, k, h, h_next, mode, SD, SV, SP);
+  scalar_advance(s, k, len, mode, SD, SV, SP);
   *sc = s;
 }
 
@@ -177,7 +197,7 @@ struct StageTail {
   unsigned int* work;     // work-item claim counter of a persistent launch (kick_tma), zero between launches
   int fused;              // 0: partials only (scalar_update follows as its own launch)
   ScalarConst k;
-  double h, h_next;
+  StageLen len;
 };
 
 // Thread 0: the three partial sums of work item `idx` of `nparts` (the order of the final sum is the index
@@ -211,7 +231,7 @@ __device__ __forceinline__ void stage_finish(const StageTail& t, const double* p
   const double SP = block_sum_fixed<NT>(partials + 2 * (size_t)nparts, (int)nparts, sh);
   if (threadIdx.x == 0) {
     Scalars s = *t.sc;
-    scalar_advance(s, t.k, t.h, t.h_next, 1, SD, SV, SP);
+    scalar_advance(s, t.k, t.len, 1, SD, SV, SP);
     *t.sc = s;
   }
 }

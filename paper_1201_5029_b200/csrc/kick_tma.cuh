@@ -16,6 +16,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "kernels.cuh"
 
 namespace pycool {
@@ -98,6 +100,203 @@ struct TmaArgs {
   double c1, c2, c3;
   ModelParams mp;
 };
+
+// The z-march of one work item.  EDGE (compile time) = the item touches a lattice face or a ragged edge: only
+// that copy carries the periodic-image stores and the validity predicates; interior items run branch-free.
+template <bool EDGE, typename Real, class Model, class T, class IssueF>
+__device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue_next, int& slot, uint32_t& phase,
+                                           unsigned char* raw, Real* psi, const uint32_t bars, const int x0,
+                                           const int y0, const int z0, const int nz, const int own_sm,
+                                           const int (&halo_sm)[(T::NHP + T::NT - 1) / T::NT], const Real cd,
+                                           const Real kD, const Real kV, const Real c0, const Real c1, const Real c2,
+                                           const Real c3, const typename Model::template Coef<Real>& coef,
+                                           double& sD, double& sV, double& sP) {
+  using R2 = typename Vec2T<Real>::type;
+  using SM = TmaSmem<Real, Model, T>;
+  constexpr int NF = Model::NF, TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J;
+  constexpr int PLANE = T::PLANE;
+  constexpr uint32_t ES = (uint32_t)sizeof(Real);
+  constexpr int NHT = (T::NHP + NT - 1) / NT;
+  const Layout& L = g.L;
+  const int N = L.N;
+  const int tid = threadIdx.x;
+  const int tx2 = tid % (TX / 2), tyj = tid / (TX / 2);
+  const size_t plane_b = L.plane * ES, field_b = L.field * ES;
+  (void)TY; (void)S; (void)tyj;
+
+  auto zwrap = [&](int p) {
+    int gz = z0 + p;
+    return gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+  };
+
+  // Own sites.  Items that touch no lattice face and no ragged edge (block-uniform test) store through a
+  // uniform plane pointer plus a 32-bit per-thread byte offset and nothing else; the others also write the
+  // periodic images of their face sites into the ghost columns / rows and predicate ragged sites.
+  const int gx = x0 + 2 * tx2;
+  const bool okx = gx < N;
+  int ximg = 0;                                              // element offset of the x image, 0 = none
+  if (gx < L.gx) ximg = N; else if (gx >= N - L.gx) ximg = -N;
+  const bool ximg2 = (gx < L.gx) && (gx >= N - L.gx);        // both images (N <= 2 gx only)
+  bool valid[J];
+  uint32_t own_off[J];                                       // byte offset within a (field, z) plane
+  long long yimg[J];                                         // element offset of the y image, 0 = none
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    const int gy = y0 + J * tyj + j;
+    valid[j] = okx && gy < N;
+    own_off[j] = ((uint32_t)(gy + L.gy) * (uint32_t)L.pitch + (uint32_t)(gx + L.gx)) * ES;
+    yimg[j] = 0;
+    if (gy == 0) yimg[j] = (long long)N * L.pitch; else if (gy == N - 1) yimg[j] = -(long long)N * L.pitch;
+  }
+  auto store_edge = [&](unsigned char* plane, int j, R2 v) { // one output pair and its periodic images
+    Real* p = reinterpret_cast<Real*>(plane + own_off[j]);
+    *reinterpret_cast<R2*>(p) = v;
+    if (ximg) {
+      *reinterpret_cast<R2*>(p + ximg) = v;
+      if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
+    }
+    if (yimg[j]) {
+      *reinterpret_cast<R2*>(p + yimg[j]) = v;
+      if (ximg) {
+        *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
+        if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
+      }
+    }
+  };
+  auto store_own = [&](unsigned char* plane, int j, R2 v) {  // plain store (st.global.cs measured 9 % slower)
+    if constexpr (!EDGE) *reinterpret_cast<R2*>(plane + own_off[j]) = v;
+    else if (valid[j]) store_edge(plane, j, v);
+  };
+
+  R2 qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
+  R2 A[NF][J], B[NF][J];                                     // stencil accumulators
+  Real ref[NF];                                              // item-uniform; D annihilates constants
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    ref[f] = Real(0);
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      A[f][j] = B[f][j] = qa_phi[f][j] = qa_pi[f][j] = qb_phi[f][j] = qb_pi[f][j] = R2{Real(0), Real(0)};
+    }
+  }
+
+  // One plane of the march: cphi/cpi receive plane p, pphi/ppi hold plane p-1 (finalised here).
+  // EDGE (compile-time) = the item touches a lattice face or a ragged edge; interior items run a copy of the
+  // march without any of the image / validity branches.
+  auto step = [&](const int p, const int par, R2 (&cphi)[NF][J], R2 (&cpi)[NF][J], const R2 (&pphi)[NF][J],
+                  const R2 (&ppi)[NF][J]) {
+    const int s = slot;
+    const Real* rphi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA);
+    const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
+    Real* pb = psi + (size_t)par * (SM::BOXA / sizeof(Real));
+    mbar_wait(bars + 8u * s, phase);
+    if (++slot == S) { slot = 0; phase ^= 1u; }
+
+    // reference value of each field: phi at the item's first site one plane below (any item-uniform value
+    // near the field does; it is the same for every thread because it is read from the shared box)
+    if (p == -1) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) ref[f] = rphi[f * PLANE + PX + G];
+    }
+
+    // ---- 1. drift: phi' = phi + c_drift pi (own pairs and halo ring); psi = phi' - ref to shared memory
+    const bool own_plane = (p >= 0) && (p < nz);
+    unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)zwrap(p) * plane_b;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        const int o = f * PLANE + own_sm + j * PX;
+        const R2 a = *reinterpret_cast<const R2*>(rphi + o);
+        const R2 b = *reinterpret_cast<const R2*>(rpi + o);
+        R2 ph;
+        ph.x = fma(cd, b.x, a.x);
+        ph.y = fma(cd, b.y, a.y);
+        cphi[f][j] = ph; cpi[f][j] = b;
+        if (own_plane) store_own(ophi + f * field_b, j, ph);
+        *reinterpret_cast<R2*>(pb + o) = R2{ph.x - ref[f], ph.y - ref[f]};
+      }
+#pragma unroll
+      for (int k = 0; k < NHT; ++k)
+        if (halo_sm[k] >= 0) {
+          const int o = f * PLANE + halo_sm[k];
+          const R2 a = *reinterpret_cast<const R2*>(rphi + o);
+          const R2 b = *reinterpret_cast<const R2*>(rpi + o);
+          *reinterpret_cast<R2*>(pb + o) = R2{fma(cd, b.x, a.x) - ref[f], fma(cd, b.y, a.y) - ref[f]};
+        }
+    }
+    __syncthreads();                                         // psi plane complete; raw stage s consumed
+    issue_next(s);
+
+    // ---- 2. in-plane sums of plane p; 3. finalise plane p-1
+    R2 D[NF][J];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const Real* sp = pb + f * PLANE + own_sm - PX;         // row above the first own row
+      Real Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];       // x-output 0 and 1: side sums and centres
+#pragma unroll
+      for (int r = 0; r < J + 2; ++r) {
+        const Real l = sp[r * PX - 1];
+        const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
+        const Real rr = sp[r * PX + 2];
+        Rx[r] = l + m.y; Cx[r] = m.x;
+        Ry[r] = m.x + rr; Cy[r] = m.y;
+      }
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        {
+          const Real P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
+          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0)); // weight of plane p in outputs p-1 and p+1
+          D[f][j].x = A[f][j].x + up;                        // output p-1 complete
+          A[f][j].x = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].x)));   // + weight of plane p in output p
+          B[f][j].x = up;
+        }
+        {
+          const Real P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
+          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));
+          D[f][j].y = A[f][j].y + up;
+          A[f][j].y = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].y)));
+          B[f][j].y = up;
+        }
+      }
+    }
+    if (p >= 1) {
+      unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)zwrap(p - 1) * plane_b;
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        if (!EDGE || valid[j]) {
+          Real ph[NF], dV[NF];
+          R2 pn[NF];
+#pragma unroll
+          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].x;
+          sV += (double)Model::template eval<Real>(coef, ph, dV);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            pn[f].x = fma(kD, D[f][j].x, fma(-kV, dV[f], ppi[f][j].x));   // pi' = pi + kD D - kV dV
+            sD = fma((double)ph[f], (double)D[f][j].x, sD);
+            sP = fma((double)pn[f].x, (double)pn[f].x, sP);
+          }
+#pragma unroll
+          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].y;
+          sV += (double)Model::template eval<Real>(coef, ph, dV);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            pn[f].y = fma(kD, D[f][j].y, fma(-kV, dV[f], ppi[f][j].y));
+            sD = fma((double)ph[f], (double)D[f][j].y, sD);
+            sP = fma((double)pn[f].y, (double)pn[f].y, sP);
+            store_own(opi + f * field_b, j, pn[f]);
+          }
+        }
+      }
+    }
+  };
+
+#pragma unroll 1
+  for (int p = -1; p <= nz; p += 2) {                        // two planes per trip: the p / p-1 roles swap
+    step(p, 0, qa_phi, qa_pi, qb_phi, qb_pi);
+    if (p + 1 <= nz) step(p + 1, 1, qb_phi, qb_pi, qa_phi, qa_pi);
+  }
+}
 
 // Work items.  With gridDim.x = nitems every block has one item.  With fewer blocks (as many as are resident on
 // the GPU at once) the launch is persistent: a block's first item is its index, every further one is claimed
@@ -202,8 +401,6 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 2; }
     halo_sm[k] = h < T::NHP ? row * PX + col : -1;
   }
-  const size_t plane_b = L.plane * ES, field_b = L.field * ES;
-
   int slot = 0;                                                // ring slot and phase of the next plane to consume
   uint32_t phase = 0;
 
@@ -213,178 +410,14 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     const int bz = item / nbxy, rr_ = item - bz * nbxy, by = rr_ / g.nbx;
     const int x0 = (rr_ - by * g.nbx) * TX, y0 = by * TY, z0 = bz * g.zc;
     const int nz = min(g.zc, N - z0);
-    auto zwrap = [&](int p) {
-      int gz = z0 + p;
-      return gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
-    };
-
-    // Own sites.  Items that touch no lattice face and no ragged edge (block-uniform test) store through a
-    // uniform plane pointer plus a 32-bit per-thread byte offset and nothing else; the others also write the
-    // periodic images of their face sites into the ghost columns / rows and predicate ragged sites.
     const bool edge_blk = (x0 < L.gx) | (x0 + TX > N - L.gx) | (y0 == 0) | (y0 + TY >= N);
-    const int gx = x0 + 2 * tx2;
-    const bool okx = gx < N;
-    int ximg = 0;                                              // element offset of the x image, 0 = none
-    if (gx < L.gx) ximg = N; else if (gx >= N - L.gx) ximg = -N;
-    const bool ximg2 = (gx < L.gx) && (gx >= N - L.gx);        // both images (N <= 2 gx only)
-    bool valid[J];
-    uint32_t own_off[J];                                       // byte offset within a (field, z) plane
-    long long yimg[J];                                         // element offset of the y image, 0 = none
-#pragma unroll
-    for (int j = 0; j < J; ++j) {
-      const int gy = y0 + J * tyj + j;
-      valid[j] = okx && gy < N;
-      own_off[j] = ((uint32_t)(gy + L.gy) * (uint32_t)L.pitch + (uint32_t)(gx + L.gx)) * ES;
-      yimg[j] = 0;
-      if (gy == 0) yimg[j] = (long long)N * L.pitch; else if (gy == N - 1) yimg[j] = -(long long)N * L.pitch;
-    }
-    auto store_edge = [&](unsigned char* plane, int j, R2 v) { // one output pair and its periodic images
-      Real* p = reinterpret_cast<Real*>(plane + own_off[j]);
-      *reinterpret_cast<R2*>(p) = v;
-      if (ximg) {
-        *reinterpret_cast<R2*>(p + ximg) = v;
-        if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
-      }
-      if (yimg[j]) {
-        *reinterpret_cast<R2*>(p + yimg[j]) = v;
-        if (ximg) {
-          *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
-          if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
-        }
-      }
-    };
-    auto store_own = [&](unsigned char* plane, int j, R2 v) {  // plain store (st.global.cs measured 9 % slower)
-      if (!edge_blk) *reinterpret_cast<R2*>(plane + own_off[j]) = v;
-      else if (valid[j]) store_edge(plane, j, v);
-    };
-
-    R2 qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
-    R2 A[NF][J], B[NF][J];                                     // stencil accumulators
-    Real ref[NF];                                              // item-uniform; D annihilates constants
     double sD = 0.0, sV = 0.0, sP = 0.0;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) {
-      ref[f] = Real(0);
-#pragma unroll
-      for (int j = 0; j < J; ++j) {
-        A[f][j] = B[f][j] = qa_phi[f][j] = qa_pi[f][j] = qb_phi[f][j] = qb_pi[f][j] = R2{Real(0), Real(0)};
-      }
-    }
-
-    // One plane of the march: cphi/cpi receive plane p, pphi/ppi hold plane p-1 (finalised here).
-    auto step = [&](const int p, const int par, R2 (&cphi)[NF][J], R2 (&cpi)[NF][J], const R2 (&pphi)[NF][J],
-                    const R2 (&ppi)[NF][J]) {
-      const int s = slot;
-      const Real* rphi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA);
-      const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
-      Real* pb = psi + (size_t)par * (SM::BOXA / sizeof(Real));
-      mbar_wait(bars + 8u * s, phase);
-      if (++slot == S) { slot = 0; phase ^= 1u; }
-
-      // reference value of each field: phi at the item's first site one plane below (any item-uniform value
-      // near the field does; it is the same for every thread because it is read from the shared box)
-      if (p == -1) {
-#pragma unroll
-        for (int f = 0; f < NF; ++f) ref[f] = rphi[f * PLANE + PX + G];
-      }
-
-      // ---- 1. drift: phi' = phi + c_drift pi (own pairs and halo ring); psi = phi' - ref to shared memory
-      const bool own_plane = (p >= 0) && (p < nz);
-      unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)zwrap(p) * plane_b;
-#pragma unroll
-      for (int f = 0; f < NF; ++f) {
-#pragma unroll
-        for (int j = 0; j < J; ++j) {
-          const int o = f * PLANE + own_sm + j * PX;
-          const R2 a = *reinterpret_cast<const R2*>(rphi + o);
-          const R2 b = *reinterpret_cast<const R2*>(rpi + o);
-          R2 ph;
-          ph.x = fma(cd, b.x, a.x);
-          ph.y = fma(cd, b.y, a.y);
-          cphi[f][j] = ph; cpi[f][j] = b;
-          if (own_plane) store_own(ophi + f * field_b, j, ph);
-          *reinterpret_cast<R2*>(pb + o) = R2{ph.x - ref[f], ph.y - ref[f]};
-        }
-#pragma unroll
-        for (int k = 0; k < NHT; ++k)
-          if (halo_sm[k] >= 0) {
-            const int o = f * PLANE + halo_sm[k];
-            const R2 a = *reinterpret_cast<const R2*>(rphi + o);
-            const R2 b = *reinterpret_cast<const R2*>(rpi + o);
-            *reinterpret_cast<R2*>(pb + o) = R2{fma(cd, b.x, a.x) - ref[f], fma(cd, b.y, a.y) - ref[f]};
-          }
-      }
-      __syncthreads();                                         // psi plane complete; raw stage s consumed
-      issue_next(s);
-
-      // ---- 2. in-plane sums of plane p; 3. finalise plane p-1
-      R2 D[NF][J];
-#pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        const Real* sp = pb + f * PLANE + own_sm - PX;         // row above the first own row
-        Real Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];       // x-output 0 and 1: side sums and centres
-#pragma unroll
-        for (int r = 0; r < J + 2; ++r) {
-          const Real l = sp[r * PX - 1];
-          const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
-          const Real rr = sp[r * PX + 2];
-          Rx[r] = l + m.y; Cx[r] = m.x;
-          Ry[r] = m.x + rr; Cy[r] = m.y;
-        }
-#pragma unroll
-        for (int j = 0; j < J; ++j) {
-          {
-            const Real P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
-            const Real up = fma(c3, P2, fma(c2, P1, c1 * P0)); // weight of plane p in outputs p-1 and p+1
-            D[f][j].x = A[f][j].x + up;                        // output p-1 complete
-            A[f][j].x = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].x)));   // + weight of plane p in output p
-            B[f][j].x = up;
-          }
-          {
-            const Real P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
-            const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));
-            D[f][j].y = A[f][j].y + up;
-            A[f][j].y = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].y)));
-            B[f][j].y = up;
-          }
-        }
-      }
-      if (p >= 1) {
-        unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)zwrap(p - 1) * plane_b;
-#pragma unroll
-        for (int j = 0; j < J; ++j) {
-          if (!edge_blk || valid[j]) {
-            Real ph[NF], dV[NF];
-            R2 pn[NF];
-#pragma unroll
-            for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].x;
-            sV += (double)Model::template eval<Real>(coef, ph, dV);
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-              pn[f].x = fma(kD, D[f][j].x, fma(-kV, dV[f], ppi[f][j].x));   // pi' = pi + kD D - kV dV
-              sD = fma((double)ph[f], (double)D[f][j].x, sD);
-              sP = fma((double)pn[f].x, (double)pn[f].x, sP);
-            }
-#pragma unroll
-            for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].y;
-            sV += (double)Model::template eval<Real>(coef, ph, dV);
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-              pn[f].y = fma(kD, D[f][j].y, fma(-kV, dV[f], ppi[f][j].y));
-              sD = fma((double)ph[f], (double)D[f][j].y, sD);
-              sP = fma((double)pn[f].y, (double)pn[f].y, sP);
-              store_own(opi + f * field_b, j, pn[f]);
-            }
-          }
-        }
-      }
-    };
-
-#pragma unroll 1
-    for (int p = -1; p <= nz; p += 2) {                        // two planes per trip: the p / p-1 roles swap
-      step(p, 0, qa_phi, qa_pi, qb_phi, qb_pi);
-      if (p + 1 <= nz) step(p + 1, 1, qb_phi, qb_pi, qa_phi, qa_pi);
-    }
+    if (edge_blk)
+      march_item<true, Real, Model, T>(g, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz, own_sm, halo_sm, cd,
+                                       kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
+    else
+      march_item<false, Real, Model, T>(g, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz, own_sm, halo_sm,
+                                        cd, kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
 
     // ---- the item's partial sums, fixed order.  The barrier inside block_reduce also separates this item's
     // last reads of the psi planes from the next item's first writes.

@@ -70,7 +70,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 struct pycool_ctx {
   int N = 0, nf = 0, order = 0, model = 0, precision = 64;
-  double L = 0, dx = 0, dt = 0, eta = 0, mpl = 1, rho_g = 0, rho_m = 0;
+  double L = 0, dx = 0, dt = 0, mpl = 1, rho_g = 0, rho_m = 0;
   size_t V = 0, elems = 0, esize = 8;
   double c[4] = {0, 0, 0, 0};
   ModelParams mp{};
@@ -91,7 +91,8 @@ struct pycool_ctx {
   bool persistent = true;           // kick_tma: one block per resident slot, the TMA ring runs on across items
   int blocks_launched = 0;          // grid size of the latest kick launch
   bool fused_tail = true;           // last block of a kick reduces the partials and advances the scalars
-  double h_cur = 0, h_next = 0;     // stage lengths handed to the next kick launch
+  StageLen len{};                   // stage weights handed to the next kick launch
+  bool adaptive = false;            // dt is a physical-time increment (pycool_set_adaptive)
   bool own_mem = false, own_stream = false;
   void* owned_block = nullptr;  // one allocation when own_mem
   cudaStream_t stream = nullptr;
@@ -272,8 +273,7 @@ int launch_kick_t(pycool_ctx* c) {
   g.tail.work = c->ticket + 1;
   g.tail.fused = c->fused_tail ? 1 : 0;
   g.tail.k = c->kc;
-  g.tail.h = c->h_cur;
-  g.tail.h_next = c->h_next;
+  g.tail.len = c->len;
   g.L = c->lay;
   g.zc = c->zc;
   g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
@@ -318,8 +318,7 @@ int launch_tma_t(pycool_ctx* c) {
   g.tail.work = c->ticket + 1;
   g.tail.fused = c->fused_tail ? 1 : 0;
   g.tail.k = c->kc;
-  g.tail.h = c->h_cur;
-  g.tail.h_next = c->h_next;
+  g.tail.len = c->len;
   g.L = c->lay;
   g.zc = c->zc;
   g.nbx = (int)c->grid.x; g.nby = (int)c->grid.y;
@@ -477,9 +476,9 @@ int set_geometry(pycool_ctx* c) {
   return PYCOOL_OK;
 }
 
-int launch_scalar(pycool_ctx* c, double h, double h_next, int mode) {
+int launch_scalar(pycool_ctx* c, const StageLen& len, int mode) {
   const int nb = (int)(c->grid.x * c->grid.y * c->grid.z);
-  scalar_update<<<1, kReduceThreads, 0, c->stream>>>(c->sc, c->partials, nb, c->kc, h, h_next, mode);
+  scalar_update<<<1, kReduceThreads, 0, c->stream>>>(c->sc, c->partials, nb, c->kc, len, mode);
   CUDA_TRY(c, cudaGetLastError());
   c->counts[1]++;
   return PYCOOL_OK;
@@ -780,7 +779,11 @@ int pycool_step(pycool_ctx* c, int nsteps) {
   if (nsteps == 0) return PYCOOL_OK;
   const int ns = c->nstages;
   const long long S = (long long)nsteps * ns;
-  int st = launch_scalar(c, 0.0, c->w[0] * c->dt, c->pending_drift ? 2 : 0);
+  StageLen len;
+  len.dt = c->dt;
+  len.adaptive = c->adaptive ? 1 : 0;
+  len.w = 0.0; len.w_next = c->w[0]; len.ends_step = 0;
+  int st = launch_scalar(c, len, c->pending_drift ? 2 : 0);
   if (st != PYCOOL_OK) return st;
   if (c->profiling && c->ev.size() < c->ev_used + 2 * (size_t)S) {
     const size_t want = c->ev_used + 2 * (size_t)S;
@@ -791,23 +794,28 @@ int pycool_step(pycool_ctx* c, int nsteps) {
     }
   }
   for (long long i = 0; i < S; ++i) {
-    const double h = c->w[i % ns] * c->dt;
-    const double h_next = (i + 1 < S) ? c->w[(i + 1) % ns] * c->dt : 0.0;
+    len.w = c->w[i % ns];
+    len.w_next = (i + 1 < S) ? c->w[(i + 1) % ns] : 0.0;      // stage weights are never zero
+    len.ends_step = (i % ns) == ns - 1;
     if (c->profiling) CUDA_TRY(c, cudaEventRecord(c->ev[c->ev_used++], c->stream));
-    c->h_cur = h;
-    c->h_next = h_next;
+    c->len = len;
     st = (int)dispatch(c, OP_KICK, 0);
     if (st != PYCOOL_OK) return st;
     if (c->profiling) CUDA_TRY(c, cudaEventRecord(c->ev[c->ev_used++], c->stream));
     c->counts[0]++;
     c->cur ^= 1;
     if (!c->fused_tail) {
-      st = launch_scalar(c, h, h_next, 1);
+      st = launch_scalar(c, len, 1);
       if (st != PYCOOL_OK) return st;
     }
   }
   c->pending_drift = true;
-  for (int i = 0; i < nsteps; ++i) c->eta += c->dt;
+  return PYCOOL_OK;
+}
+
+int pycool_set_adaptive(pycool_ctx* c, int on) {
+  if (!c) return PYCOOL_EINVAL;
+  c->adaptive = on != 0;
   return PYCOOL_OK;
 }
 
@@ -880,7 +888,7 @@ int pycool_energies(pycool_ctx* c, pycool_energy* o) {
   }
   const double ap = -s.p_a / (6.0 * (double)c->V * c->mpl * c->mpl);               // (2.14)
   const double H = ap / a2;
-  o->a = a; o->p_a = s.p_a; o->eta = c->eta;
+  o->a = a; o->p_a = s.p_a; o->eta = s.eta;
   o->pot = av.Vbar; o->rho = rho; o->pressure = P; o->hubble = H;
   o->residual = std::isinf(c->mpl) ? 0.0 : std::fabs(rho / (3.0 * c->mpl * c->mpl * H * H) - 1.0);   // (3.1)
   return PYCOOL_OK;

@@ -49,8 +49,8 @@ def rel(a, b):
     return abs(a - b) / max(abs(b), 1e-300)
 
 
-def check_scalars(eg, eo, nf, tol=1e-10, static=False):
-    assert rel(eg.a, eo.a) <= tol and rel(eg.eta, eo.eta) <= 1e-14
+def check_scalars(eg, eo, nf, tol=1e-10, static=False, tol_eta=1e-14):
+    assert rel(eg.a, eo.a) <= tol and rel(eg.eta, eo.eta) <= tol_eta
     if not static:
         assert rel(eg.p_a, eo.p_a) <= tol and rel(eg.hubble, eo.hubble) <= tol
     for f in range(nf):
@@ -60,12 +60,12 @@ def check_scalars(eg, eo, nf, tol=1e-10, static=False):
     assert rel(eg.pot, eo.pot) <= tol and rel(eg.rho, eo.rho) <= tol and rel(eg.pressure, eo.pressure) <= tol
 
 
-def compare(g, o, nf, tol_site, tol_scalar=1e-10, static=False):
+def compare(g, o, nf, tol_site, tol_scalar=1e-10, static=False, tol_eta=1e-14):
     pg, qg = g.read_fields()
     po, qo = o.read_fields()
     e1, e2 = rel_err_per_site(pg, po), rel_err_per_site(qg, qo)
     assert e1 <= tol_site and e2 <= tol_site, (e1, e2)
-    check_scalars(g.energies(), o.energies(), nf, tol_scalar, static)
+    check_scalars(g.energies(), o.energies(), nf, tol_scalar, static, tol_eta)
     return max(e1, e2)
 
 
@@ -281,6 +281,46 @@ def test_four_fields_auto_variant_fits_shared_memory(pc, precision):
     start(g, o, phi, pi, 1.0, 0.0)
     g.step(2); o.step(2)
     compare(g, o, nf, 5e-13 if precision == 64 else 1e-5, tol_scalar=1e-10 if precision == 64 else 1e-5, static=True)
+
+
+# ------------------------------------------------------------------------------------- adaptive conformal step
+@pytest.mark.parametrize("order,fused", [(2, True), (4, True), (4, False), (6, True)])
+def test_adaptive_step_matches_oracle(pc, order, fused):
+    """Constant physical-time increments: the conformal length dt / a_n of every step is formed on
+    the device from the a the step starts with; fields, a, p_a and the accumulated eta against the oracle."""
+    cfg = inputs.config("cfg0_chaotic32", N=20, dt=0.004, order=order)
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    g.set_fused_tail(fused)
+    start(g, o, phi, pi)
+    g.set_adaptive(True); o.set_adaptive(True)
+    g.step(2); g.step(3); o.step(5)
+    compare(g, o, 2, 5e-12, tol_eta=1e-13)
+    eg, eo = g.energies(), o.energies()
+    assert eg.a > 1.001 and 0 < eo.eta < 5 * cfg["dt"]             # expanding: the steps did shrink
+    assert rel(eg.eta, eo.eta) <= 1e-13
+    h = pc.from_config(cfg)                                       # one call == split calls, bitwise
+    h.set_fused_tail(fused)
+    h.set_fields(phi, pi); h.set_background(1.0); h.set_adaptive(True)
+    h.step(5)
+    assert np.array_equal(h.read_fields()[0], g.read_fields()[0]) and h.energies().eta == eg.eta
+
+
+def test_adaptive_step_radiation_only_recurrence_on_gpu(pc):
+    """a' is constant in a radiation-only universe, so a_{n+1} = a_n + C dt / a_n exactly (same closed form that
+    pins the oracle, P14), here for the device-side scalar update."""
+    N, mpl, rg, dt, n = 8, 1.5, 3.0, 0.02, 40
+    g = pc.Lattice(N, 1.0, 1, pc.FREE, [0.0], order=4, dt=dt, mpl=mpl, rho_gamma0=rg)
+    z = np.zeros((1, N, N, N))
+    g.set_fields(z, z); g.set_background(1.0); g.set_adaptive(True)
+    g.step(n)
+    C = math.sqrt(rg / 3) / mpl
+    a, eta = np.longdouble(1), np.longdouble(0)
+    for _ in range(n):
+        hh = np.longdouble(dt) / a
+        a, eta = a + np.longdouble(C) * hh, eta + hh
+    e = g.energies()
+    assert abs(e.a - float(a)) < 1e-13 and abs(e.eta - float(eta)) < 1e-13 and e.residual < 1e-13
 
 
 def test_bitwise_reproducible(pc):
