@@ -58,7 +58,7 @@ int stage_weights_ld(int order, long double* w) {
 constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
 constexpr size_t kMaxSmem = 227 * 1024;  // dynamic shared memory one block may opt in to on sm_100
 constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
-constexpr int kNumTiles = 14;            // + kick_tma variants (ghost layout only)
+constexpr int kNumTiles = 9;             // + kick_tma variants (ghost layout only)
 
 struct TileInfo { int tx, ty, nt, stages; };   // stages > 0: TMA ring depth
 
@@ -134,24 +134,20 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 //                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
 const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
-                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {64, 16, 512, 3}, {64, 16, 256, 4},
-                                    {64, 16, 512, 4}, {128, 8, 256, 3}, {128, 8, 512, 3},
-                                    {128, 16, 512, 3}, {64, 32, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}};
+                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {128, 8, 256, 3},
+                                    {128, 16, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}};
 using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 16, 2>;
-// kick_tma variants: <TX, TY, ring stages, rows per thread J, blocks per SM the registers are cut for>
-template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 256 threads x (2 x 2 sites)
-template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3, 2, 1>;   // 128 threads x (2 x 2 sites)
-template <typename Real> using TTile5 = TmaTile<Real, 64, 16, 3, 1, 1>;   // 512 threads x (2 x 1 sites)
-template <typename Real> using TTile6 = TmaTile<Real, 64, 16, 4, 2, 1>;   // as 3, ring of 4
-template <typename Real> using TTile7 = TmaTile<Real, 64, 16, 4, 1, 1>;   // as 5, ring of 4
-template <typename Real> using TTile8 = TmaTile<Real, 128, 8, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 256 threads x (2 x 2 sites), 1 KB rows
-template <typename Real> using TTile9 = TmaTile<Real, 128, 8, 3, 1, 1>;   // 512 threads x (2 x 1 sites), 1 KB rows
-template <typename Real> using TTile10 = TmaTile<Real, 128, 16, 3, 2, 1>; // 512 threads x (2 x 2 sites): twice the
-template <typename Real> using TTile11 = TmaTile<Real, 64, 32, 3, 2, 1>;  //   bytes per plane (fp32, one field)
-template <typename Real> using TTile12 = TmaTile<Real, 32, 16, 3, 1, 2>;  // 256 threads x (2 x 1 sites), two blocks
-template <typename Real> using TTile13 = TmaTile<Real, 64, 8, 3, 1, 2>;   //   per SM: one fills its ring while the other runs
+// kick_tma variants: <TX, TY, ring stages, rows per thread J, blocks per SM the registers are cut for>.
+// (Tried and dropped, profiles/r1c: ring of 4, 512-thread 2 x 1-site blocks, 64 x 32 tiles -- never faster.)
+template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 256 thr x (2 x 2 sites)
+template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3, 2, 1>;   // 128 threads x (2 x 2 sites): small N
+template <typename Real> using TTile5 = TmaTile<Real, 128, 8, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 1 KB rows
+template <typename Real> using TTile6 = TmaTile<Real, 128, 16, 3, 2, 1>;  // 512 threads: twice the bytes per plane (one field)
+template <typename Real> using TTile7 = TmaTile<Real, 32, 16, 3, 1, 2>;   // 256 threads x (2 x 1 sites), two blocks per
+template <typename Real> using TTile8 = TmaTile<Real, 64, 8, 3, 1, 2>;    //   SM: ALU-heavy models (Q-ball)
+#define PYCOOL_TMA_TILES(X) X(3, TTile3) X(4, TTile4) X(5, TTile5) X(6, TTile6) X(7, TTile7) X(8, TTile8)
 
 // Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
 Layout make_layout(int N, int nf, size_t esize) {
@@ -334,57 +330,37 @@ int launch_tma_t(pycool_ctx* c) {
 }
 template <typename Real, class Model>
 int launch_kick_m(pycool_ctx* c) {
-  switch (c->tile) {
+  const int tile_ = c->tile;
+  switch (tile_) {
     case 0: return launch_kick_t<Real, Model, Tile0>(c);
     case 1: return launch_kick_t<Real, Model, Tile1>(c);
     case 2: return launch_kick_t<Real, Model, Tile2>(c);
-    case 3: return launch_tma_t<Real, Model, TTile3<Real>>(c);
-    case 4: return launch_tma_t<Real, Model, TTile4<Real>>(c);
-    case 5: return launch_tma_t<Real, Model, TTile5<Real>>(c);
-    case 6: return launch_tma_t<Real, Model, TTile6<Real>>(c);
-    case 7: return launch_tma_t<Real, Model, TTile7<Real>>(c);
-    case 8: return launch_tma_t<Real, Model, TTile8<Real>>(c);
-    case 9: return launch_tma_t<Real, Model, TTile9<Real>>(c);
-    case 10: return launch_tma_t<Real, Model, TTile10<Real>>(c);
-    case 11: return launch_tma_t<Real, Model, TTile11<Real>>(c);
-    case 12: return launch_tma_t<Real, Model, TTile12<Real>>(c);
-    default: return launch_tma_t<Real, Model, TTile13<Real>>(c);
+#define X(ID, TT) case ID: return launch_tma_t<Real, Model, TT<Real>>(c);
+    PYCOOL_TMA_TILES(X)
+#undef X
+    default: return 0;
   }
 }
 template <typename Real, class Model>
-size_t kick_smem_m(int tile) {
-  switch (tile) {
+size_t kick_smem_m(int tile_) {
+  switch (tile_) {
     case 0: return kick_smem_bytes<Real, Model, Tile0>();
     case 1: return kick_smem_bytes<Real, Model, Tile1>();
     case 2: return kick_smem_bytes<Real, Model, Tile2>();
-    case 3: return TmaSmem<Real, Model, TTile3<Real>>::TOTAL;
-    case 4: return TmaSmem<Real, Model, TTile4<Real>>::TOTAL;
-    case 5: return TmaSmem<Real, Model, TTile5<Real>>::TOTAL;
-    case 6: return TmaSmem<Real, Model, TTile6<Real>>::TOTAL;
-    case 7: return TmaSmem<Real, Model, TTile7<Real>>::TOTAL;
-    case 8: return TmaSmem<Real, Model, TTile8<Real>>::TOTAL;
-    case 9: return TmaSmem<Real, Model, TTile9<Real>>::TOTAL;
-    case 10: return TmaSmem<Real, Model, TTile10<Real>>::TOTAL;
-    case 11: return TmaSmem<Real, Model, TTile11<Real>>::TOTAL;
-    case 12: return TmaSmem<Real, Model, TTile12<Real>>::TOTAL;
-    default: return TmaSmem<Real, Model, TTile13<Real>>::TOTAL;
+#define X(ID, TT) case ID: return TmaSmem<Real, Model, TT<Real>>::TOTAL;
+    PYCOOL_TMA_TILES(X)
+#undef X
+    default: return 0;
   }
 }
 template <typename Real, class Model>
-int kick_resident_m(pycool_ctx* c, int tile) {
-  switch (tile) {
+int kick_resident_m(pycool_ctx* c, int tile_) {
+  switch (tile_) {
     case 0: case 1: case 2: return 2 * 148;             // register-prefetch kernel: not persistent, a guess does
-    case 3: return tma_resident<Real, Model, TTile3<Real>>(c);
-    case 4: return tma_resident<Real, Model, TTile4<Real>>(c);
-    case 5: return tma_resident<Real, Model, TTile5<Real>>(c);
-    case 6: return tma_resident<Real, Model, TTile6<Real>>(c);
-    case 7: return tma_resident<Real, Model, TTile7<Real>>(c);
-    case 8: return tma_resident<Real, Model, TTile8<Real>>(c);
-    case 9: return tma_resident<Real, Model, TTile9<Real>>(c);
-    case 10: return tma_resident<Real, Model, TTile10<Real>>(c);
-    case 11: return tma_resident<Real, Model, TTile11<Real>>(c);
-    case 12: return tma_resident<Real, Model, TTile12<Real>>(c);
-    default: return tma_resident<Real, Model, TTile13<Real>>(c);
+#define X(ID, TT) case ID: return tma_resident<Real, Model, TT<Real>>(c);
+    PYCOOL_TMA_TILES(X)
+#undef X
+    default: return 0;
   }
 }
 template <typename Real, class Model>
@@ -432,7 +408,7 @@ int auto_tile(pycool_ctx* c) {
   const Layout& L = c->lay;
   if (L.gx == 0) return L.N <= 64 ? 0 : 1;
   if (L.N <= 64) return 4;
-  static const int pref_default[] = {3, 4}, pref_one[] = {10, 3, 4}, pref_alu[] = {12, 4};
+  static const int pref_default[] = {3, 4}, pref_one[] = {6, 3, 4}, pref_alu[] = {7, 4};
   const int* pref = pref_default;
   int n = 2;
   if (c->model == PYCOOL_QBALL) { pref = pref_alu; n = 2; }

@@ -140,21 +140,21 @@ def test_all_orders(pc, order):
 
 
 def set_tile_or_skip(pc, g, tile):
-    """Variants 10, 11 (twice the bytes per plane) do not fit in shared memory for two fp64 fields: EINVAL."""
+    """Variant 6 (128 x 16: twice the bytes per plane) does not fit in shared memory for two fp64 fields: EINVAL."""
     try:
         g.set_tile(tile)
     except pc.PycoolError as e:
-        assert e.code == pc.EINVAL and tile in (10, 11) and "shared memory" in str(e)
+        assert e.code == pc.EINVAL and tile == 6 and "shared memory" in str(e)
         return False
     return True
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8])
 @pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32), (6, 0),
                                   (70, 9), (136, 50)])
 def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
     """Several tiles with ragged tails in x, y and z, wrap-around at every face, for each variant of the fused
-    kernel: 0-2 register prefetch (any N), 3-7 TMA ring with ghost images (even N)."""
+    kernel: 0-2 register prefetch (any N), 3-8 TMA ring with ghost images (even N)."""
     cfg = inputs.config("cfg0_chaotic32", N=N, dt=0.002, order=4)
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg)
@@ -184,7 +184,7 @@ def test_variants_agree_and_ghost_images_hold(pc, precision):
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg, precision=precision)
     outs = []
-    for tile in range(14):
+    for tile in range(9):
         g = pc.from_config(cfg, precision=precision)
         if not set_tile_or_skip(pc, g, tile):
             assert precision == 64
@@ -239,7 +239,7 @@ def test_fused_tail_equals_separate_scalar_update(pc, tile, N):
     assert rel(ea.a, eb.a) < 1e-14 and rel(ea.p_a, eb.p_a) < 1e-13
 
 
-@pytest.mark.parametrize("tile,N,zc", [(3, 136, 5), (4, 70, 1), (8, 260, 4), (5, 136, 1), (13, 72, 1)])
+@pytest.mark.parametrize("tile,N,zc", [(3, 136, 5), (4, 70, 1), (5, 260, 4), (7, 136, 1), (8, 72, 1)])
 def test_persistent_launch_is_bitwise_the_one_block_per_item_launch(pc, tile, N, zc):
     """More work items than resident blocks (short z-chunks): every block walks several items with its TMA ring
     running on across them (ragged tiles, lattice faces and z-wrap included).  Partial sums are indexed by work
