@@ -85,12 +85,19 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
             self.proc = None
+
+    def wait_first(self, timeout=3.0):
+        """Block until nvidia-smi has delivered its first line (it needs ~0.1-1 s to start), so that samples fall
+        inside the warm-up and the timed region even when those last only tens of milliseconds."""
+        t0 = time.time()
+        while self.proc and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.01)
 
     def _read(self):
         for line in self.proc.stdout:
@@ -212,6 +219,12 @@ def main():
         lat.set_fused_tail(a.fused_tail)
     lat.set_fields(h_phi, h_pi)
     lat.set_background(1.0)
+    # clocks and throttle reasons are sampled from here (warm-up: the same steps as the timed region) to the end
+    # of the timed region; nvidia-smi needs ~0.1 s to deliver its first line, the timed region may be shorter
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        sampler.wait_first()
     lat.step(a.warmup)
     lat.sync()
 
@@ -221,9 +234,6 @@ def main():
         torch.cuda.synchronize(dev)
 
     # ---- device-resident timing, kernel brackets live in the same region
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     c0 = lat.launch_counts()
     lat.set_profiling(True)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -242,6 +252,17 @@ def main():
     launches = sum(c1) - sum(c0)
     ms = max_over_ranks(ms, world, dev)
     value = whole_job_value(N, nf, a.steps, world, ms * 1e-3)
+
+    # ---- row a7, on demand: pycool_energies (reads phi and pi once: 2 sizeof(real) bytes per field-site), wall
+    # clock of the synchronising call, best of 3
+    lat.energies()
+    t_en = []
+    for _ in range(3):
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        lat.energies()
+        t_en.append(time.perf_counter() - t0)
+    en_ms = min(t_en) * 1e3
 
     # ---- end to end: host buffers -> host buffers
     e2e = None
@@ -283,6 +304,10 @@ def main():
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f%d" % a.precision, "data": "synthetic", "config": config, "clocks": clocks,
             "gpu_launches": launches, "roofline": roof}
+    en_bytes = 2.0 * esz * N ** 3 * nf
+    line["energies"] = {"ms": en_ms, "achieved": en_bytes / (en_ms * 1e-3) / 1e9, "unit": "GB/s",
+                        "frac": en_bytes / (en_ms * 1e-3) / 1e9 / peak,
+                        "what": "pycool_energies (sums of pi^2, G, phi D phi, V; reduce; D2H), host wall clock"}
     if e2e:
         line["e2e"] = e2e
     if not a.no_cpu_baseline and world == 1:

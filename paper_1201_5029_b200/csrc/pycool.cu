@@ -22,6 +22,7 @@
 #include "../../include/pycool.h"
 #include "kernels.cuh"
 #include "kick_tma.cuh"
+#include "energy_tma.cuh"
 
 using namespace pycool;
 
@@ -88,6 +89,8 @@ struct pycool_ctx {
   double* sums = nullptr;       // 16 doubles: reduced rows
   Scalars* sc = nullptr;
   unsigned int* ticket = nullptr;   // blocks-done counter of the fused stage tail (zero between launches)
+  bool energy_tma = true;           // pycool_energies through the TMA-fed kernel where the layout allows
+  int energy_nb = 0;                // blocks (= partial sums per quantity) of the latest energy launch
   bool persistent = true;           // kick_tma: one block per resident slot, the TMA ring runs on across items
   int blocks_launched = 0;          // grid size of the latest kick launch
   bool fused_tail = true;           // last block of a kick reduces the partials and advances the scalars
@@ -223,9 +226,8 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// Tensor map over one padded array: dims (x: N + 2 gx, y: N + 2 gy, z: N, f: nf), box (TX + 2 gx, TY + 2, 1, nf)
-int encode_maps(pycool_ctx* c) {
-  const TileInfo& t = kTiles[c->tile];
+// Tensor map over one padded array: dims (x: N + 2 gx, y: N + 2 gy, z: N, f: nf), box (tx + 2 gx, ty + 2, 1, nf)
+int encode_one(pycool_ctx* c, void* ptr, int tx, int ty, CUtensorMap* out) {
   EncodeTiledFn enc = encode_fn();
   if (!enc) return fail(c, PYCOOL_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
   const Layout& L = c->lay;
@@ -233,17 +235,19 @@ int encode_maps(pycool_ctx* c) {
                               (cuuint64_t)c->nf};
   const cuuint64_t strides[3] = {(cuuint64_t)L.pitch * c->esize, (cuuint64_t)L.plane * c->esize,
                                  (cuuint64_t)L.field * c->esize};
-  const cuuint32_t box[4] = {(cuuint32_t)(t.tx + 2 * L.gx), (cuuint32_t)(t.ty + 2), 1u, (cuuint32_t)c->nf};
+  const cuuint32_t box[4] = {(cuuint32_t)(tx + 2 * L.gx), (cuuint32_t)(ty + 2), 1u, (cuuint32_t)c->nf};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   const CUtensorMapDataType dt = c->precision == 32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+  CUresult r = enc(out, dt, 4, ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(c, PYCOOL_ECUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+  return PYCOOL_OK;
+}
+int encode_maps(pycool_ctx* c) {
+  const TileInfo& t = kTiles[c->tile];
   for (int b = 0; b < 2; ++b)
-    for (int a = 0; a < 2; ++a) {
-      void* ptr = a == 0 ? c->phi[b] : c->pi[b];
-      CUresult r = enc(&c->tm[b][a], dt, 4, ptr, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      if (r != CUDA_SUCCESS) return fail(c, PYCOOL_ECUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
-    }
+    for (int a = 0; a < 2; ++a)
+      if (int st = encode_one(c, a == 0 ? c->phi[b] : c->pi[b], t.tx, t.ty, &c->tm[b][a])) return st;
   return PYCOOL_OK;
 }
 
@@ -363,11 +367,46 @@ int kick_resident_m(pycool_ctx* c, int tile_) {
     default: return 0;
   }
 }
+// TMA-fed energy sums (energy_tma.cuh): ghost layout, at most two fields (the ring of more does not fit).
+template <typename Real, class Model, class T>
+int launch_energy_tma(pycool_ctx* c) {
+  static bool attr_done = false;
+  constexpr size_t smem = EnergySmem<Real, Model, T>::TOTAL;
+  if (!attr_done) {
+    CUDA_TRY(c, cudaFuncSetAttribute(energy_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_done = true;
+  }
+  CUtensorMap tm_phi, tm_pi;
+  if (int st = encode_one(c, c->phi[c->cur], T::TX, T::TY, &tm_phi)) return st;
+  if (int st = encode_one(c, c->pi[c->cur], T::TX, T::TY, &tm_pi)) return st;
+  EnergyArgs<Real> g;
+  g.partials = c->partials;
+  g.L = c->lay;
+  g.zc = c->N < 32 ? c->N : 32;
+  g.nbx = (c->N + T::TX - 1) / T::TX;
+  g.nby = (c->N + T::TY - 1) / T::TY;
+  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
+  g.mp = c->mp;
+  const size_t nb = (size_t)g.nbx * g.nby * ((c->N + g.zc - 1) / g.zc);
+  if ((3 * (size_t)Model::NF + 1) * nb > c->partials_cap) return -1;       // caller falls back
+  energy_tma<Real, Model, T><<<(unsigned)nb, T::NT, smem, c->stream>>>(tm_phi, tm_pi, g);
+  CUDA_TRY(c, cudaGetLastError());
+  c->energy_nb = (int)nb;
+  return PYCOOL_OK;
+}
 template <typename Real, class Model>
 int launch_energy_m(pycool_ctx* c, int nb) {
+  if constexpr (Model::NF <= 2) {
+    if (c->lay.gx > 0 && c->energy_tma) {
+      const int st = c->N > 64 ? launch_energy_tma<Real, Model, TTile3<Real>>(c)
+                               : launch_energy_tma<Real, Model, TTile4<Real>>(c);
+      if (st >= 0) return st;
+    }
+  }
   energy_sums<Real, Model><<<nb, 256, 0, c->stream>>>((const Real*)c->phi[c->cur], (const Real*)c->pi[c->cur],
                                                       c->lay, c->c[1], c->c[2], c->c[3], c->mp, c->partials);
   CUDA_TRY(c, cudaGetLastError());
+  c->energy_nb = nb;
   return PYCOOL_OK;
 }
 
@@ -529,6 +568,7 @@ int energy_sums_host(pycool_ctx* c, double* out /* 3 nf + 1 */) {
   int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)kMaxSumBlocks);
   int st = (int)dispatch(c, OP_ENERGY, nb);
   if (st != PYCOOL_OK) return st;
+  nb = c->energy_nb;
   reduce_rows<<<nq, kReduceThreads, 0, c->stream>>>(c->partials, nb, c->sums);
   CUDA_TRY(c, cudaGetLastError());
   c->counts[3] += 2;
@@ -934,6 +974,12 @@ int pycool_set_zchunk(pycool_ctx* c, int planes) {
   if (planes < 0) return fail(c, PYCOOL_EINVAL, "planes < 0");
   c->zc_user = planes;
   return set_geometry(c);
+}
+
+int pycool_set_energy_kernel(pycool_ctx* c, int tma) {
+  if (!c) return PYCOOL_EINVAL;
+  c->energy_tma = tma != 0;
+  return PYCOOL_OK;
 }
 
 int pycool_set_persistent(pycool_ctx* c, int on) {

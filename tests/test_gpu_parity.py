@@ -283,6 +283,39 @@ def test_four_fields_auto_variant_fits_shared_memory(pc, precision):
     compare(g, o, nf, 5e-13 if precision == 64 else 1e-5, tol_scalar=1e-10 if precision == 64 else 1e-5, static=True)
 
 
+# ------------------------------------------------------------------------------------- energies (row a7)
+@pytest.mark.parametrize("name,N", [("cfg0_chaotic32", 32), ("cfg0_chaotic32", 70), ("cfg2_oscillon256", 136),
+                                    ("cfg3_qball256", 40), ("cfg3_qball256", 6)])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_energy_kernels_agree_with_each_other_and_the_oracle(pc, name, N, precision):
+    """pycool_energies through the TMA-fed z-march (G from 2 G[psi] = D[psi^2] - 2 psi D[psi]) and through the plain
+    kernel that evaluates (2.8) term by term, after a few steps, against the oracle's direct evaluation; ragged
+    tiles, several z-chunks (N = 70, 136) and a lattice smaller than a tile (N = 6)."""
+    cfg = inputs.config(name, N=N)
+    cfg["L"] = cfg["L"] * N / inputs.config(name)["N"]
+    phi, pi = inputs.make_initial(cfg, precision=precision)
+    g, o = make_pair(pc, cfg, precision=precision)
+    start(g, o, phi, pi)
+    g.step(2); o.step(2)
+    # fp32: one ulp of phi is 1e-3 of the Q-ball lattice's 1e-4 fluctuations, and G sums their squared differences
+    tol = 1e-10 if precision == 64 else 1e-4
+    eo = o.energies()
+    es = []
+    for tma in (True, False):
+        g.set_energy_kernel(tma)
+        n0 = g.launch_counts()[3]
+        es.append(g.energies())
+        assert g.launch_counts()[3] == n0 + 2
+        check_scalars(es[-1], eo, cfg["nfields"], tol)
+    a, b = es
+    for f in range(cfg["nfields"]):
+        assert rel(a.grad[f], b.grad[f]) <= (1e-12 if precision == 64 else 1e-6)
+        # sum phi D[phi] = phi_0 sum D + sum dphi D with sum D = 0 up to rounding: the order of the sum shows at 1e-10
+        assert rel(a.kin[f], b.kin[f]) <= 1e-13 and rel(a.sum_phiDphi[f], b.sum_phiDphi[f]) <= 1e-9
+        assert rel(a.grad[f], a.sum_phiDphi[f]) <= (1e-9 if precision == 64 else 1e-4)      # (2.17)
+    assert rel(a.pot, b.pot) <= 1e-13 and rel(a.rho, b.rho) <= 1e-12
+
+
 # ------------------------------------------------------------------------------------- adaptive conformal step
 @pytest.mark.parametrize("order,fused", [(2, True), (4, True), (4, False), (6, True)])
 def test_adaptive_step_matches_oracle(pc, order, fused):
