@@ -440,18 +440,20 @@ long long dispatch(pycool_ctx* c, Op op, int arg) {
 
 // Automatic variant (measured on B200, profiles/): the register-prefetch kernel where the layout has no ghosts
 // (odd N); else the first TMA variant of a preference list whose ring fits in shared memory.
-//   two fields fp64 / anything fp32: 64 x 16 tile (fp32 instances are cut for two blocks per SM);
+//   two fields fp64, one field fp32: 64 x 16 tile; two or more fields fp32: 128 x 8 (512-byte rows; the fp32
+//   instances of both are cut for two blocks per SM, which is what fp32 needs: half the bytes per plane);
 //   one field fp64: 128 x 16 (a plane of a 64 x 16 box is too few bytes in flight);
 //   Q-ball (the logarithm makes it ALU-heavy): 32 x 16 with 2 x 1 sites per thread, two blocks per SM.
 int auto_tile(pycool_ctx* c) {
   const Layout& L = c->lay;
   if (L.gx == 0) return L.N <= 64 ? 0 : 1;
   if (L.N <= 64) return 4;
-  static const int pref_default[] = {3, 4}, pref_one[] = {6, 3, 4}, pref_alu[] = {7, 4};
+  static const int pref_default[] = {3, 4}, pref_one[] = {6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {5, 3, 4};
   const int* pref = pref_default;
   int n = 2;
-  if (c->model == PYCOOL_QBALL) { pref = pref_alu; n = 2; }
+  if (c->model == PYCOOL_QBALL && c->precision == 64) { pref = pref_alu; n = 2; }
   else if (c->nf == 1 && c->precision == 64) { pref = pref_one; n = 3; }
+  else if (c->precision == 32 && c->nf >= 2) { pref = pref_f32; n = 3; }
   for (int i = 0; i < n; ++i)
     if ((size_t)dispatch(c, OP_SMEM, pref[i]) <= kMaxSmem) return pref[i];
   return 1;
