@@ -12,6 +12,7 @@
 //                                                                               (3.4) PAPER.md:481 (G6-G8)
 #pragma once
 #include <cfloat>
+#include <cstring>
 
 namespace pycool {
 
@@ -24,7 +25,51 @@ template <typename T> __device__ __forceinline__ T min_normal();
 template <> __device__ __forceinline__ double min_normal<double>() { return DBL_MIN; }
 template <> __device__ __forceinline__ float min_normal<float>() { return FLT_MIN; }
 
-__device__ __forceinline__ double log_of(double x) { return log(x); }
+// Natural logarithm of a positive finite double, for the Q-ball potential (3.4).  CUDA's log() costs ~150
+// instructions per call in this kernel (slow-path branches, integer work), which made the Q-ball kick ALU-bound;
+// this one is ~45: x = 2^e m with m in [sqrt(1/2), sqrt(2)), s = (m-1)/(m+1), ln m = 2 s sum_k s^(2k)/(2k+1)
+// (|s| <= 0.1716, 11 terms: truncation 2e-19), ln x = e ln2_hi + (e ln2_lo + ln m) with the two-part ln 2 of
+// fdlibm.  Error <= 2.1 ulp against logl over [1e-300, 1e300], near 1 and at the sqrt 2 switch
+// (tests/test_abi_cpu.py compiles this very function for the host, tests/log_pos_check.cu, and checks it).
+__host__ __device__ __forceinline__ double log_pos(double x) {
+  int e = 0;
+  if (x < 2.2250738585072014e-308) { x *= 18014398509481984.0; e = -54; }      // subnormal: scale by 2^54
+#if defined(__CUDA_ARCH__)
+  int hi = __double2hiint(x);
+  const int lo = __double2loint(x);
+#else
+  unsigned long long bits;
+  memcpy(&bits, &x, sizeof bits);
+  int hi = (int)(bits >> 32);
+  const int lo = (int)(unsigned)(bits & 0xffffffffu);
+#endif
+  e += (hi >> 20) - 1023;
+  hi = (hi & 0x000fffff) | 0x3ff00000;                                           // m in [1, 2)
+  if (hi >= 0x3ff6a09e) { hi -= 0x00100000; e += 1; }                            // m >= ~sqrt 2: halve it
+#if defined(__CUDA_ARCH__)
+  const double m = __hiloint2double(hi, lo);
+#else
+  bits = ((unsigned long long)(unsigned)hi << 32) | (unsigned)lo;
+  double m;
+  memcpy(&m, &bits, sizeof m);
+#endif
+  const double s = (m - 1.0) / (m + 1.0);
+  const double z = s * s;
+  // sum_{k=0..10} z^k / (2k + 3), Estrin's scheme: 5 dependent operations instead of Horner's 11 (the kick
+  // has two of these chains per thread in flight and few warps to hide them behind)
+  const double z2 = z * z, z4 = z2 * z2, z8 = z4 * z4;
+  const double a0 = fma(1.0 / 5.0, z, 1.0 / 3.0), a1 = fma(1.0 / 9.0, z, 1.0 / 7.0);
+  const double a2 = fma(1.0 / 13.0, z, 1.0 / 11.0), a3 = fma(1.0 / 17.0, z, 1.0 / 15.0);
+  const double a4 = fma(1.0 / 21.0, z, 1.0 / 19.0), a5 = 1.0 / 23.0;
+  const double b0 = fma(a1, z2, a0), b1 = fma(a3, z2, a2), b2 = fma(a5, z2, a4);
+  const double p = fma(b2, z8, fma(b1, z4, b0));
+  const double two_s = s + s;
+  const double lnm = fma(two_s * z, p, two_s);                                   // 2 s (1 + z p)
+  const double de = (double)e;
+  return fma(de, 6.93147180369123816490e-01, fma(de, 1.90821492927058770002e-10, lnm));
+}
+
+__device__ __forceinline__ double log_of(double x) { return log_pos(x); }
 __device__ __forceinline__ float log_of(float x) { return logf(x); }
 
 // Coefficients are converted to the compute type T once per thread (Coef), then eval() is pure T arithmetic.

@@ -113,3 +113,18 @@ def test_product_does_not_touch_the_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1201_5029_b200" not in txt and "from paper_1201_5029_b200" not in txt, f
             assert "pycool.h" not in txt or f == "oracle.h", f
+
+
+def test_device_log_against_libm(tmp_path):
+    """The Q-ball kick uses its own fp64 logarithm (potentials.cuh: log_pos, __host__ __device__).  The same source
+    compiled for the host against logl: <= 2.5 ulp over 1e-300..1e300, around 1, at the sqrt(2) range switch,
+    and for a subnormal argument."""
+    import subprocess
+    exe = str(tmp_path / "log_pos_check")
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    subprocess.run([nvcc, "-O2", "-std=c++17", "-o", exe, os.path.join(ROOT, "tests", "log_pos_check.cu")], check=True,
+                   capture_output=True)
+    out = subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()
+    assert out[0] == "worst" and float(out[1]) <= 2.5, out
+    sub = out[out.index("sub") + 1:]
+    assert abs(float(sub[0]) - float(sub[1])) <= 1e-13 * abs(float(sub[1]))
