@@ -530,3 +530,47 @@ def test_full_size_periodic_replication(pc, N, base):
                 d = np.abs(blocks[iz] - arr_o[f][:, None, :, None, :]) / den[:, None, :, None, :]
                 worst = max(worst, float(d.max()))
         assert worst <= 2e-12, worst
+
+
+def test_largest_lattice_1024_cubed_fp32_on_device(pc):
+    """1024^3 x 2 fields = 2^31 elements per array (the largest lattice one B200 holds in fp64 too): 64-bit offsets,
+    32768 work items, 1028-element rows.  fp32 keeps it to 34 GB of state; input and comparison stay on the device
+    (set_fields_device / read_fields_device).  Same replication argument as above against the oracle's 32^3."""
+    import torch
+    N, base = 1024, 32
+    r = N // base
+    small = inputs.config("cfg4_chaotic1024", N=base)
+    small["L"] = 10.0 * base / N
+    small["dt"] = 10.0 / N / 20.0
+    phi_s, pi_s = inputs.make_initial(small, precision=32)
+    big = inputs.config("cfg4_chaotic1024", N=N)
+    g = pc.from_config(big, precision=32)
+    o = oracle.Oracle(base, small["L"], 2, oracle.CHAOTIC, small["p"], order=4, dt=small["dt"], mpl=1.0, precision=32)
+    dev = g.device
+    tp = torch.from_numpy(phi_s).to(dev).repeat(1, r, r, r).contiguous()
+    tq = torch.from_numpy(pi_s).to(dev).repeat(1, r, r, r).contiguous()
+    assert tp.numel() == 2 ** 31
+    g.set_fields(tp, tq)
+    del tp, tq
+    g.set_background(1.0)
+    o.set_fields(phi_s, pi_s)
+    o.set_background(1.0)
+    g.step(1); o.step(1)
+    geo = g.kick_geometry()
+    assert geo["blocks"] >= 16384 and geo["tma_stages"] > 0
+    po, qo = o.read_fields()
+    pg, qg = g.read_fields_device()
+    eg, eo = g.energies(), o.energies()
+    assert rel(eg.a, eo.a) < 1e-6 and rel(eg.p_a / r ** 3, eo.p_a) < 1e-5
+    assert rel(eg.kin[0], eo.kin[0]) < 1e-5 and rel(eg.grad[1], eo.grad[1]) < 1e-4 and rel(eg.pot, eo.pot) < 1e-5
+    for arr_g, arr_o in ((pg, po), (qg, qo)):
+        for f in range(2):
+            want = torch.from_numpy(arr_o[f]).to(dev)
+            rms = float(want.double().pow(2).mean().sqrt())
+            den = torch.clamp(want.abs(), min=rms)
+            blocks = arr_g[f].view(r, base, r, base, r, base)
+            worst = 0.0
+            for iz in range(r):                              # every replica, every site
+                d = (blocks[iz] - want[:, None, :, None, :]).abs() / den[:, None, :, None, :]
+                worst = max(worst, float(d.max()))
+            assert worst <= 1e-5, (f, worst)
