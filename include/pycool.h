@@ -183,6 +183,10 @@ int pycool_set_zchunk(pycool_ctx*, int planes);
  * so a stage is ONE launch.  Off: a separate reduce + scalar-update launch follows every kick.  Both orders of
  * summation are fixed; they differ from each other in the last bits only. */
 int pycool_set_fused_tail(pycool_ctx*, int on);
+/* Programmatic dependent launch of the TMA-fed kernel (default on): the next stage's blocks are scheduled while
+ * the current stage drains and wait (griddepcontrol.wait) until it has completed before they read anything it
+ * wrote.  Hides launch latency and prologue on small lattices; results are unchanged. */
+int pycool_set_overlap(pycool_ctx*, int on);
 /* pycool_energies kernel: 1 (default) = TMA-fed z-march (even N, at most two fields; G from the identity
  * 2 G[psi] = D[psi^2] - 2 psi D[psi]); 0 = the plain one-thread-per-site kernel that evaluates (2.8) term by term
  * (always used for odd N or more than two fields).  They agree to rounding. */

@@ -22,7 +22,7 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
-           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel")
+           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap")
 
 
 class Params(C.Structure):
@@ -93,6 +93,7 @@ def lib():
         L.pycool_flush.argtypes = [vp]
         L.pycool_set_adaptive.argtypes = [vp, ip]
         L.pycool_set_energy_kernel.argtypes = [vp, ip]
+        L.pycool_set_overlap.argtypes = [vp, ip]
         _lib = L
     return _lib
 
@@ -252,6 +253,9 @@ class Lattice:
     def set_adaptive(self, on=True):
         """dt becomes a physical-time increment: step n has conformal length dt / a_n."""
         self._chk(lib().pycool_set_adaptive(self._h, 1 if on else 0))
+
+    def set_overlap(self, on=True):
+        self._chk(lib().pycool_set_overlap(self._h, 1 if on else 0))
 
     def set_energy_kernel(self, tma=True):
         self._chk(lib().pycool_set_energy_kernel(self._h, 1 if tma else 0))

@@ -372,11 +372,17 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     }
   };
 
+  // Programmatic dependent launch: the next stage's grid may be scheduled while this one drains (its blocks take
+  // the SMs this grid's blocks leave, set up their barriers and indices, then wait below), which hides the launch
+  // latency and the prologue behind this grid's tail -- the last block's reduction and scalar update.  Nothing
+  // above the wait reads what the previous stage wrote (fields, scalars, partials, counters).
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   if (tid == 0) {
     for (int s = 0; s < S; ++s) mbar_init(bars + 8u * s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   pr_decode();
+  asm volatile("griddepcontrol.wait;" ::: "memory");           // previous kernel complete, its writes visible
   for (int s = 0; s < S; ++s) {
     issue_next(s);
     __syncthreads();                                           // also: barriers initialised before anyone waits

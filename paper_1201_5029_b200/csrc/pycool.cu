@@ -89,6 +89,7 @@ struct pycool_ctx {
   double* sums = nullptr;       // 16 doubles: reduced rows
   Scalars* sc = nullptr;
   unsigned int* ticket = nullptr;   // blocks-done counter of the fused stage tail (zero between launches)
+  bool overlap_launch = true;       // kick_tma launched with programmatic stream serialization (PDL)
   bool energy_tma = true;           // pycool_energies through the TMA-fed kernel where the layout allows
   int energy_nb = 0;                // blocks (= partial sums per quantity) of the latest energy launch
   bool persistent = true;           // kick_tma: one block per resident slot, the TMA ring runs on across items
@@ -181,10 +182,10 @@ int blocks_xy(int N, int tile) {
   return ((N + t.tx - 1) / t.tx) * ((N + t.ty - 1) / t.ty);
 }
 int auto_zchunk(pycool_ctx* c);
-// partial-sum capacity actually reserved: automatic geometry of every tile with zc >= min(N, 4)
+// partial-sum capacity actually reserved: automatic geometry of every tile with zc >= min(N, 2)
 size_t partials_capacity(int N) {
   size_t m = 13 * (size_t)kMaxSumBlocks;
-  const int zmin = N < 4 ? N : 4;
+  const int zmin = N < 2 ? N : 2;
   for (int t = 0; t < kNumTiles; ++t) {
     size_t b = 3 * (size_t)blocks_xy(N, t) * (size_t)((N + zmin - 1) / zmin);
     if (b > m) m = b;
@@ -328,8 +329,17 @@ int launch_tma_t(pycool_ctx* c) {
   // persistent: one block per resident slot, items dealt round-robin; else one block per item
   const int nblocks = c->persistent && resident < g.nitems ? resident : g.nitems;
   c->blocks_launched = nblocks;
-  kick_tma<Real, Model, T><<<nblocks, T::NT, smem, c->stream>>>(c->tm[c->cur][0], c->tm[c->cur][1], g);
-  CUDA_TRY(c, cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)nblocks);
+  cfg.blockDim = dim3(T::NT);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = c->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;    // see the kernel's griddepcontrol.wait
+  attr[0].val.programmaticStreamSerializationAllowed = c->overlap_launch ? 1 : 0;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  CUDA_TRY(c, cudaLaunchKernelEx(&cfg, kick_tma<Real, Model, T>, c->tm[c->cur][0], c->tm[c->cur][1], g));
   return PYCOOL_OK;
 }
 template <typename Real, class Model>
@@ -471,9 +481,9 @@ int auto_zchunk(pycool_ctx* c) {
   const int cap = N >= 1024 ? 32 : 16;
   auto items = [&](int zc) { return (long long)bxy * ((N + zc - 1) / zc); };
   if (items(cap) >= 4LL * R) return cap;
-  int best = cap;
+  int best = cap < N ? cap : N;
   long long best_cost = -1;
-  for (int zc = cap; zc <= N; zc += 8) {
+  for (int zc = 2; zc <= N; zc += 2) {                        // tiny lattices: a few planes per block
     const long long rounds = (items(zc) + R - 1) / R;
     const long long cost = rounds * (zc + 2) + 4;
     if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = zc; }
@@ -976,6 +986,12 @@ int pycool_set_zchunk(pycool_ctx* c, int planes) {
   if (planes < 0) return fail(c, PYCOOL_EINVAL, "planes < 0");
   c->zc_user = planes;
   return set_geometry(c);
+}
+
+int pycool_set_overlap(pycool_ctx* c, int on) {
+  if (!c) return PYCOOL_EINVAL;
+  c->overlap_launch = on != 0;
+  return PYCOOL_OK;
 }
 
 int pycool_set_energy_kernel(pycool_ctx* c, int tma) {
