@@ -109,6 +109,19 @@ int pycool_set_fields(pycool_ctx*, const void* phi_host, const void* pi_host);
 /* Same from dense device arrays (D2D on the context stream, asynchronous). */
 int pycool_set_fields_device(pycool_ctx*, const void* d_phi_src, const void* d_pi_src);
 
+/* Seeded Gaussian initial conditions generated on the device (the paper takes its
+ * fluctuations from Defrost without describing the generator, so the recipe is DESIGN.md's reading
+ * G21).  Array (field f, phi or pi) = mean + a real Gaussian random field with spectrum
+ *     A(k) = amp (k^2 + m2)^q   for 0 < k <= kmax (kmax <= 0: every k),   k = 2 pi |n| / L,
+ * F_k = A(k)(g1 + i g2)/sqrt 2 with (g1, g2) from Philox4x32-10(counter = (mode index, array id 2f | 2f+1), key =
+ * seed) through Box-Muller, field = mean + sqrt(2)/L^1.5 sum_k F_k exp(2 pi i n.x/N) (cuFFT, loaded on demand).
+ * Vacuum fluctuations |phi_k|^2 = 1/(2 omega_k): amp = c/sqrt 2, q = -1/4 for phi and +1/4 for pi, m2 = m_eff^2.
+ * phi_spec, pi_spec: nfields entries each (host).  Replaces set_fields; even N only.  Synchronises.  The same seed
+ * gives the same lattice on any GPU.  Scratch: one N^2 (N/2 + 1) x 16-byte buffer plus cuFFT's work area. */
+typedef struct { double mean, amp, m2, q, kmax; } pycool_spectrum;
+int pycool_init_fields(pycool_ctx*, unsigned long long seed, const pycool_spectrum* phi_spec,
+                       const pycool_spectrum* pi_spec);
+
 /* Set a (> 0) and p_a.  p_a = NaN asks the library to solve the first Friedmann equation (2.18) on the
  * current lattice, expanding branch (reading G10): p_a = -6 V_L mpl a^2 sqrt(rho/3); needs fields and a
  * finite mpl.  With mpl = +INF pass p_a = 0. */

@@ -22,13 +22,17 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
-           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap")
+           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_init_fields")
 
 
 class Params(C.Structure):
     _fields_ = [("model", C.c_int), ("p", C.c_double * 8), ("mpl", C.c_double),
                 ("rho_gamma0", C.c_double), ("rho_m0", C.c_double), ("stencil", C.c_double * 4),
                 ("precision", C.c_int)]
+
+
+class Spectrum(C.Structure):
+    _fields_ = [("mean", C.c_double), ("amp", C.c_double), ("m2", C.c_double), ("q", C.c_double), ("kmax", C.c_double)]
 
 
 class Energy(C.Structure):
@@ -94,6 +98,7 @@ def lib():
         L.pycool_set_adaptive.argtypes = [vp, ip]
         L.pycool_set_energy_kernel.argtypes = [vp, ip]
         L.pycool_set_overlap.argtypes = [vp, ip]
+        L.pycool_init_fields.argtypes = [vp, C.c_ulonglong, C.POINTER(Spectrum), C.POINTER(Spectrum)]
         _lib = L
     return _lib
 
@@ -176,6 +181,14 @@ class Lattice:
             return
         phi, pi = self._host(phi), self._host(pi)
         self._chk(lib().pycool_set_fields(self._h, phi.ctypes.data, pi.ctypes.data))
+
+    def init_fields(self, seed, phi_spec, pi_spec):
+        """Seeded Gaussian initial conditions generated on the device.  *_spec: per field (mean, amp, m2, q, kmax),
+        spectrum A(k) = amp (k^2 + m2)^q for k <= kmax (kmax <= 0: all k); see pycool_init_fields."""
+        assert len(phi_spec) == self.nf and len(pi_spec) == self.nf
+        a = (Spectrum * self.nf)(*[Spectrum(*map(float, t)) for t in phi_spec])
+        b = (Spectrum * self.nf)(*[Spectrum(*map(float, t)) for t in pi_spec])
+        self._chk(lib().pycool_init_fields(self._h, int(seed), a, b))
 
     def set_background(self, a=1.0, p_a=math.nan):
         self._chk(lib().pycool_set_background(self._h, a, p_a))

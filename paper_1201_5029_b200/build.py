@@ -13,12 +13,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpycool.so")
 SOURCES = [os.path.join(CSRC, "pycool.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "kick_tma.cuh"), os.path.join(CSRC, "energy_tma.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "kick_tma.cuh"), os.path.join(CSRC, "energy_tma.cuh"), os.path.join(CSRC, "init_fields.cuh"),
                   os.path.join(CSRC, "potentials.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "pycool.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xptxas", "-v",
-         "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static"]
+         "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static", "-ldl"]
 
 
 def up_to_date():

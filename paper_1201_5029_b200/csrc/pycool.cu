@@ -18,11 +18,14 @@
 
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <cufft.h>      // types only: the library is loaded on demand (dlopen), not linked
+#include <dlfcn.h>
 
 #include "../../include/pycool.h"
 #include "kernels.cuh"
 #include "kick_tma.cuh"
 #include "energy_tma.cuh"
+#include "init_fields.cuh"
 
 using namespace pycool;
 
@@ -616,6 +619,52 @@ int averages(pycool_ctx* c, double a, Averages* av) {
   return PYCOOL_OK;
 }
 
+// ---- cuFFT, loaded on first use (pycool_init_fields only): a library FFT is a step the scope allows; loading it
+// lazily keeps the hot path free of it and fails loudly when it is missing.
+struct CufftApi {
+  cufftResult (*plan3d)(cufftHandle*, int, int, int, cufftType) = nullptr;
+  cufftResult (*set_stream)(cufftHandle, cudaStream_t) = nullptr;
+  cufftResult (*exec_z2d)(cufftHandle, cufftDoubleComplex*, cufftDoubleReal*) = nullptr;
+  cufftResult (*destroy)(cufftHandle) = nullptr;
+  bool ok = false;
+};
+const CufftApi& cufft_api() {
+  static CufftApi api;
+  static bool tried = false;
+  if (tried) return api;
+  tried = true;
+  void* h = nullptr;
+  for (const char* name : {"libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so.11"}) {
+    h = dlopen(name, RTLD_NOW | RTLD_LOCAL);
+    if (h) break;
+  }
+  if (!h) return api;
+  api.plan3d = (decltype(api.plan3d))dlsym(h, "cufftPlan3d");
+  api.set_stream = (decltype(api.set_stream))dlsym(h, "cufftSetStream");
+  api.exec_z2d = (decltype(api.exec_z2d))dlsym(h, "cufftExecZ2D");
+  api.destroy = (decltype(api.destroy))dlsym(h, "cufftDestroy");
+  api.ok = api.plan3d && api.set_stream && api.exec_z2d && api.destroy;
+  return api;
+}
+
+template <typename Real>
+int init_one_array(pycool_ctx* c, const CufftApi& fft, cufftHandle plan, double2* scratch, Real* dst,
+                   const Spectrum& sp, uint32_t aid, unsigned long long seed) {
+  const int N = c->N;
+  const size_t nmodes = (size_t)N * N * (N / 2 + 1);
+  int nb = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)148 * 64);
+  fill_spectrum<<<nb, 256, 0, c->stream>>>(scratch, N, c->L, sp, aid, seed);
+  CUDA_TRY(c, cudaGetLastError());
+  if (fft.exec_z2d(plan, (cufftDoubleComplex*)scratch, (cufftDoubleReal*)scratch) != CUFFT_SUCCESS)
+    return fail(c, PYCOOL_ECUDA, "cufftExecZ2D failed");
+  nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)148 * 64);
+  const double scale = std::sqrt(2.0) / (c->L * std::sqrt(c->L));
+  scatter_real<Real><<<nb, 256, 0, c->stream>>>(dst, c->lay, (const double*)scratch, sp.mean, scale);
+  CUDA_TRY(c, cudaGetLastError());
+  c->counts[3] += 2;
+  return PYCOOL_OK;
+}
+
 int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params* p, int order, double dt,
                   void* d_work, size_t work_bytes, void* stream, bool ext) {
   if (!out) return fail(nullptr, PYCOOL_EINVAL, "out is NULL");
@@ -768,6 +817,50 @@ int pycool_set_fields_device(pycool_ctx* c, const void* d_phi_src, const void* d
   if (!c) return PYCOOL_EINVAL;
   if (!d_phi_src || !d_pi_src) return fail(c, PYCOOL_EINVAL, "source pointer is NULL");
   return upload(c, d_phi_src, d_pi_src, cudaMemcpyDeviceToDevice);
+}
+
+int pycool_init_fields(pycool_ctx* c, unsigned long long seed, const pycool_spectrum* phi_spec,
+                       const pycool_spectrum* pi_spec) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!phi_spec || !pi_spec) return fail(c, PYCOOL_EINVAL, "phi_spec / pi_spec is NULL");
+  if (c->N % 2) return fail(c, PYCOOL_EINVAL, "pycool_init_fields needs an even N (Hermitian planes ix = 0, N/2)");
+  for (int f = 0; f < c->nf; ++f)
+    for (const pycool_spectrum* sp : {phi_spec + f, pi_spec + f})
+      if (!std::isfinite(sp->mean) || !std::isfinite(sp->amp) || !std::isfinite(sp->m2) || !std::isfinite(sp->q) ||
+          !std::isfinite(sp->kmax) || sp->m2 < 0)
+        return fail(c, PYCOOL_EINVAL, "spectrum parameters must be finite, m2 >= 0");
+  const CufftApi& fft = cufft_api();
+  if (!fft.ok) return fail(c, PYCOOL_ECUDA, "cuFFT (libcufft.so.11) could not be loaded");
+  const int N = c->N;
+  double2* scratch = nullptr;
+  CUDA_TRY(c, cudaMalloc(&scratch, (size_t)N * N * (N / 2 + 1) * sizeof(double2)));
+  cufftHandle plan = 0;
+  int st = PYCOOL_OK;
+  if (fft.plan3d(&plan, N, N, N, CUFFT_Z2D) != CUFFT_SUCCESS || fft.set_stream(plan, c->stream) != CUFFT_SUCCESS) {
+    cudaFree(scratch);
+    return fail(c, PYCOOL_ENOMEM, "cufftPlan3d(%d^3, Z2D) failed", N);
+  }
+  c->cur = 0;
+  c->pending_drift = false;
+  for (int f = 0; f < c->nf && st == PYCOOL_OK; ++f)
+    for (int kind = 0; kind < 2 && st == PYCOOL_OK; ++kind) {
+      const pycool_spectrum& u = kind == 0 ? phi_spec[f] : pi_spec[f];
+      const Spectrum sp{u.mean, u.amp, u.m2, u.q, u.kmax};
+      void* base = kind == 0 ? c->phi[0] : c->pi[0];
+      if (c->precision == 32)
+        st = init_one_array<float>(c, fft, plan, scratch, (float*)base + (size_t)f * c->lay.field, sp, 2u * f + kind, seed);
+      else
+        st = init_one_array<double>(c, fft, plan, scratch, (double*)base + (size_t)f * c->lay.field, sp, 2u * f + kind, seed);
+    }
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  fft.destroy(plan);
+  cudaFree(scratch);
+  if (st != PYCOOL_OK) return st;
+  CUDA_TRY(c, e);
+  c->have_fields = true;
+  c->nonfinite_seen = false;
+  CUDA_TRY(c, cudaMemsetAsync(&c->sc->nonfinite, 0, sizeof(int), c->stream));
+  return launch_sum_pi2(c);
 }
 
 int pycool_set_background(pycool_ctx* c, double a, double p_a) {

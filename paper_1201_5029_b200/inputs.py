@@ -136,6 +136,34 @@ def make_initial(cfg, precision=64, fft_max=256):
     return phi, pi
 
 
+def spectra(cfg):
+    """The same workloads as spectrum parameters for the on-device generator (pycool_init_fields) and its oracle
+    (oracle/ics.py): per field (mean, amp, m2, q, kmax) with A(k) = amp (k^2 + m2)^q for 0 < k <= kmax.
+      vacuum: A_phi = c/sqrt(2 w_k) = (c/sqrt 2)(k^2 + m_eff^2)^(-1/4), A_pi = (c/sqrt 2)(k^2 + m_eff^2)^(+1/4);
+      flat / white: constant A, normalised so that the EXPECTED rms is cfg["amp"]: var = 2 A^2 M / L^3 with M the
+      number of modes 0 < k <= kmax (white: all N^3 - 1)."""
+    N, L, nf = cfg["N"], cfg["L"], cfg["nfields"]
+    phi_spec, pi_spec = [], []
+    for f in range(nf):
+        if cfg["init"] == "vacuum":
+            meff2 = cfg["p"][0] if f == 0 else cfg["p"][1] * cfg["phi0"][0] ** 2
+            c = cfg["amp"] / math.sqrt(2.0)
+            phi_spec.append((cfg["phi0"][f], c, meff2, -0.25, 0.0))
+            pi_spec.append((cfg["phidot0"][f], c, meff2, 0.25, 0.0))
+        elif cfg["init"] in ("flat", "white"):
+            kmax = cfg["kmax"] if cfg["init"] == "flat" else 0.0
+            n1 = np.fft.fftfreq(N, d=1.0 / N)
+            n2 = (n1 * n1)[:, None, None] + (n1 * n1)[None, :, None] + (n1 * n1)[None, None, :]
+            M = np.count_nonzero((n2 > 0) & ((kmax <= 0) | (2.0 * math.pi / L * np.sqrt(n2) <= kmax))) if N <= 256 else \
+                (N ** 3 - 1 if kmax <= 0 else max(1, int(4.0 / 3.0 * math.pi * (kmax * L / (2.0 * math.pi)) ** 3)))
+            A = cfg["amp"] * math.sqrt(L ** 3 / (2.0 * max(M, 1)))
+            phi_spec.append((cfg["phi0"][f], A, 0.0, 0.0, kmax))
+            pi_spec.append((cfg["phidot0"][f], A if cfg["init"] == "white" else 0.0, 0.0, 0.0, kmax))
+        else:
+            raise ValueError("unknown init %r" % (cfg["init"],))
+    return phi_spec, pi_spec
+
+
 def random_fields(N, nf, seed, mean=0.0, amp=1.0, precision=64):
     """Plain seeded N(mean, amp) lattices for unit tests of single operators."""
     rng = np.random.default_rng(seed)
