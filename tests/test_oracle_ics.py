@@ -98,3 +98,33 @@ def test_arrays_and_seeds_are_independent_streams():
     c = ics.gaussian_field(8, 1.0, 2, 0, 0.0, 1.0, 1.0, 0.0, 0.0)
     assert abs(np.corrcoef(a.ravel(), b.ravel())[0, 1]) < 0.2 and abs(np.corrcoef(a.ravel(), c.ravel())[0, 1]) < 0.2
     assert np.array_equal(a, ics.gaussian_field(8, 1.0, 1, 0, 0.0, 1.0, 1.0, 0.0, 0.0))
+
+
+# ---------------------------------------------------------------- shell spectrum (rank 3)
+def test_shell_spectrum_of_a_single_mode_and_parseval():
+    """A cos(2 pi m.x / N) has |F_{+-m}|^2 = (L^3/2)(A/2)^2 each: the shell round(|m|) holds L^3 A^2 / 4 and nothing
+    else; counts: 1, 18 (|n|^2 = 1 and 2), ... and N^3 in total; Parseval: sum_i S_i = L^3 / (2 N^3) sum_x field^2."""
+    N, L, A = 12, 3.0, 0.7
+    z, y, x = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    for m in ((1, 0, 0), (0, 2, 1), (3, 3, 2), (0, 0, 5)):
+        f = A * np.cos(2 * np.pi * (m[0] * x + m[1] * y + m[2] * z) / N + 0.3)
+        S, C = ics.shell_spectrum(f, L)
+        i = int(math.floor(math.sqrt(sum(v * v for v in m)) + 0.5))
+        assert abs(S[i] - L ** 3 * A * A / 4) < 1e-12 * S[i]
+        assert np.all(np.delete(S, i) < 1e-25)
+    assert C[0] == 1 and C[1] == 6 + 12 and C.sum() == N ** 3 and len(C) == int(math.sqrt(3) * N / 2) + 1
+    rng = np.random.default_rng(0)
+    f = rng.standard_normal((N, N, N)) + 0.4
+    S, _ = ics.shell_spectrum(f, L)
+    assert abs(S.sum() - L ** 3 / (2 * N ** 3) * np.sum(f * f)) < 1e-12 * S.sum()
+    assert abs(S[0] - L ** 3 / 2 * f.mean() ** 2) < 1e-12 * S[0]
+
+
+def test_shell_spectrum_returns_the_generators_spectrum():
+    N, L, amp = 32, 5.0, 0.2
+    f = ics.gaussian_field(N, L, 11, 0, 0.0, amp, 2.0, -0.25, 0.0)
+    S, C = ics.shell_spectrum(f, L)
+    for i in (3, 8, 14):
+        k = 2 * math.pi / L * i
+        want = amp ** 2 * (k * k + 2.0) ** -0.5
+        assert abs(S[i] / C[i] / want - 1) < 6 / math.sqrt(C[i]) + 0.05      # shell width: k varies by +-1/(2i)
