@@ -122,6 +122,16 @@ typedef struct { double mean, amp, m2, q, kmax; } pycool_spectrum;
 int pycool_init_fields(pycool_ctx*, unsigned long long seed, const pycool_spectrum* phi_spec,
                        const pycool_spectrum* pi_spec);
 
+/* Shell-summed spectrum of one array (the paper's spectra are LATTICEEASY's and Defrost's,
+ * not defined in it: this is the field spectrum they are all built from, reading G22).  With
+ * F_k = L^1.5 / (sqrt 2 N^3) sum_x field(x) exp(-2 pi i n.x/N) -- the convention of pycool_init_fields turned around,
+ * so a field made with spectrum A(k) gives <power/count> = A(k)^2 --
+ *   power[i] = sum |F_k|^2 and count[i] = number of modes over the full spectrum with round(|n|) = i, i < nbins
+ * (nbins = round(sqrt 3 N/2) + 1 covers every mode; the mean sits in power[0]).  field in [0, nfields), which = 0
+ * for phi, 1 for pi.  cuFFT D2Z on a double copy; the shell sums use atomics, so the last bits are not
+ * reproducible from run to run.  Applies a pending closing drift first.  Synchronises. */
+int pycool_field_spectrum(pycool_ctx*, int field, int which, int nbins, double* power_host, double* count_host);
+
 /* Set a (> 0) and p_a.  p_a = NaN asks the library to solve the first Friedmann equation (2.18) on the
  * current lattice, expanding branch (reading G10): p_a = -6 V_L mpl a^2 sqrt(rho/3); needs fields and a
  * finite mpl.  With mpl = +INF pass p_a = 0. */

@@ -109,7 +109,7 @@ def shell_spectrum(field, L):
     """Shell-summed field spectrum (reading G22): with the generator's convention
     turned around, F_k = L^1.5 / (sqrt 2 N^3) sum_x field(x) exp(-2 pi i n.x / N), returns (S, C) with
     S[i] = sum of |F_k|^2 and C[i] = number of modes over the FULL spectrum with round(|n|) = i,
-    i = 0 .. floor(sqrt 3 N / 2).  A field made with spectrum A(k) has <S[i] / C[i]> = A(k_i)^2."""
+    i = 0 .. round(sqrt 3 N / 2).  A field made with spectrum A(k) has <S[i] / C[i]> = A(k_i)^2."""
     N = field.shape[0]
     F = np.fft.rfftn(np.asarray(field, dtype=np.float64), axes=(0, 1, 2)) * (L ** 1.5 / (math.sqrt(2.0) * N ** 3))
     n1 = np.arange(N)
@@ -121,7 +121,7 @@ def shell_spectrum(field, L):
     w[:, :, 0] = 1.0
     if N % 2 == 0:
         w[:, :, N // 2] = 1.0
-    nb = int(math.floor(math.sqrt(3.0) * N / 2.0)) + 1
+    nb = int(math.floor(math.sqrt(3.0) * N / 2.0 + 0.5)) + 1
     S = np.bincount(shell.ravel(), weights=(w * np.abs(F) ** 2).ravel(), minlength=nb)[:nb]
     C = np.bincount(shell.ravel(), weights=w.ravel(), minlength=nb)[:nb]
     return S, C

@@ -22,7 +22,8 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
-           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_init_fields")
+           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_init_fields",
+           "pycool_field_spectrum")
 
 
 class Params(C.Structure):
@@ -98,6 +99,7 @@ def lib():
         L.pycool_set_adaptive.argtypes = [vp, ip]
         L.pycool_set_energy_kernel.argtypes = [vp, ip]
         L.pycool_set_overlap.argtypes = [vp, ip]
+        L.pycool_field_spectrum.argtypes = [vp, ip, ip, ip, C.POINTER(d), C.POINTER(d)]
         L.pycool_init_fields.argtypes = [vp, C.c_ulonglong, C.POINTER(Spectrum), C.POINTER(Spectrum)]
         _lib = L
     return _lib
@@ -189,6 +191,14 @@ class Lattice:
         a = (Spectrum * self.nf)(*[Spectrum(*map(float, t)) for t in phi_spec])
         b = (Spectrum * self.nf)(*[Spectrum(*map(float, t)) for t in pi_spec])
         self._chk(lib().pycool_init_fields(self._h, int(seed), a, b))
+
+    def field_spectrum(self, field, which=0, nbins=None):
+        """(power, count) per shell round(|n|) of phi (which = 0) or pi (1) of one field; see pycool_field_spectrum."""
+        import numpy as np
+        nbins = nbins or int(math.floor(math.sqrt(3.0) * self.N / 2.0 + 0.5)) + 1
+        p, c = (C.c_double * nbins)(), (C.c_double * nbins)()
+        self._chk(lib().pycool_field_spectrum(self._h, field, which, nbins, p, c))
+        return np.array(p[:]), np.array(c[:])
 
     def set_background(self, a=1.0, p_a=math.nan):
         self._chk(lib().pycool_set_background(self._h, a, p_a))

@@ -93,4 +93,57 @@ scatter_real(Real* __restrict__ dst, Layout L, const double* __restrict__ src, d
   }
 }
 
+// ------------------------------------------------------------------------------------------------ shell spectrum
+// SURVEY.md 8(f) rank 3 (reading G22).  gather_real copies one array of the padded state into the
+// in-place R2C layout [z][y][2 (N/2 + 1)] as doubles, cuFFT transforms it (D2Z), bin_shells adds w |F_k|^2 into the
+// shell round(|n|) (w = 2 for the modes the half-spectrum stores once for a conjugate pair, 1 on the planes ix = 0
+// and ix = N/2), F_k = norm * (D2Z output).  Per-block shared-memory histograms (atomics: the order of the adds
+// inside a block is not fixed, so the last bits may differ from run to run -- a diagnostic, not part of the step),
+// then reduce_shells adds the per-block rows in block order.
+template <typename Real>
+__global__ void __launch_bounds__(256)
+gather_real(double* __restrict__ dst, const Real* __restrict__ src, Layout L) {
+  const int N = L.N;
+  const size_t rp = 2 * (size_t)(N / 2 + 1);
+  const size_t V = (size_t)N * N * N;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += stride) {
+    const int x = (int)(i % N), y = (int)((i / N) % N), z = (int)(i / ((size_t)N * N));
+    dst[((size_t)z * N + y) * rp + x] = (double)src[L.at(0, z, y, x)];
+  }
+}
+
+__global__ void __launch_bounds__(256)
+bin_shells(const double2* __restrict__ F, int N, double norm2, int nbins, double* __restrict__ part /* [grid][2 nbins] */) {
+  extern __shared__ double hist[];                             // [nbins] power, [nbins] counts
+  for (int i = threadIdx.x; i < 2 * nbins; i += blockDim.x) hist[i] = 0.0;
+  __syncthreads();
+  const int H = N / 2 + 1;
+  const unsigned long long nmodes = (unsigned long long)N * N * H;
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; j < nmodes; j += stride) {
+    const int ix = (int)(j % H);
+    const unsigned long long zy = j / H;
+    const int iy = (int)(zy % N), iz = (int)(zy / N);
+    const int nz = iz <= N / 2 ? iz : iz - N, ny = iy <= N / 2 ? iy : iy - N;
+    const long long n2 = (long long)nz * nz + (long long)ny * ny + (long long)ix * ix;
+    const int shell = (int)floor(sqrt((double)n2) + 0.5);
+    if (shell >= nbins) continue;
+    const double w = (ix == 0 || (N % 2 == 0 && ix == N / 2)) ? 1.0 : 2.0;
+    const double2 f = F[j];
+    atomicAdd(&hist[shell], w * norm2 * fma(f.x, f.x, f.y * f.y));
+    atomicAdd(&hist[nbins + shell], w);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < 2 * nbins; i += blockDim.x) part[(size_t)blockIdx.x * 2 * nbins + i] = hist[i];
+}
+
+__global__ void __launch_bounds__(256) reduce_shells(const double* __restrict__ part, int nblocks, int n, double* __restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double s = 0.0;
+  for (int b = 0; b < nblocks; ++b) s += part[(size_t)b * n + i];
+  out[i] = s;
+}
+
 }  // namespace pycool

@@ -625,6 +625,7 @@ struct CufftApi {
   cufftResult (*plan3d)(cufftHandle*, int, int, int, cufftType) = nullptr;
   cufftResult (*set_stream)(cufftHandle, cudaStream_t) = nullptr;
   cufftResult (*exec_z2d)(cufftHandle, cufftDoubleComplex*, cufftDoubleReal*) = nullptr;
+  cufftResult (*exec_d2z)(cufftHandle, cufftDoubleReal*, cufftDoubleComplex*) = nullptr;
   cufftResult (*destroy)(cufftHandle) = nullptr;
   bool ok = false;
 };
@@ -642,8 +643,9 @@ const CufftApi& cufft_api() {
   api.plan3d = (decltype(api.plan3d))dlsym(h, "cufftPlan3d");
   api.set_stream = (decltype(api.set_stream))dlsym(h, "cufftSetStream");
   api.exec_z2d = (decltype(api.exec_z2d))dlsym(h, "cufftExecZ2D");
+  api.exec_d2z = (decltype(api.exec_d2z))dlsym(h, "cufftExecD2Z");
   api.destroy = (decltype(api.destroy))dlsym(h, "cufftDestroy");
-  api.ok = api.plan3d && api.set_stream && api.exec_z2d && api.destroy;
+  api.ok = api.plan3d && api.set_stream && api.exec_z2d && api.exec_d2z && api.destroy;
   return api;
 }
 
@@ -861,6 +863,54 @@ int pycool_init_fields(pycool_ctx* c, unsigned long long seed, const pycool_spec
   c->nonfinite_seen = false;
   CUDA_TRY(c, cudaMemsetAsync(&c->sc->nonfinite, 0, sizeof(int), c->stream));
   return launch_sum_pi2(c);
+}
+
+int pycool_field_spectrum(pycool_ctx* c, int field, int which, int nbins, double* power_host, double* count_host) {
+  if (!c) return PYCOOL_EINVAL;
+  if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "spectrum before set_fields");
+  if (field < 0 || field >= c->nf || (which != 0 && which != 1)) return fail(c, PYCOOL_EINVAL, "bad field / which");
+  if (nbins < 1 || nbins > 4096 || !power_host || !count_host) return fail(c, PYCOOL_EINVAL, "bad nbins or NULL output");
+  int st = ensure_flushed(c);
+  if (st != PYCOOL_OK) return st;
+  const CufftApi& fft = cufft_api();
+  if (!fft.ok) return fail(c, PYCOOL_ECUDA, "cuFFT (libcufft.so.11) could not be loaded");
+  const int N = c->N;
+  const size_t nmodes = (size_t)N * N * (N / 2 + 1);
+  const int nblk = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)148 * 8);
+  double2* scratch = nullptr;
+  double* part = nullptr;
+  CUDA_TRY(c, cudaMalloc(&scratch, nmodes * sizeof(double2)));
+  if (cudaMalloc(&part, ((size_t)nblk + 1) * 2 * nbins * sizeof(double)) != cudaSuccess) {
+    cudaFree(scratch);
+    return fail(c, PYCOOL_ENOMEM, "out of device memory");
+  }
+  cufftHandle plan = 0;
+  if (fft.plan3d(&plan, N, N, N, CUFFT_D2Z) != CUFFT_SUCCESS || fft.set_stream(plan, c->stream) != CUFFT_SUCCESS) {
+    cudaFree(scratch); cudaFree(part);
+    return fail(c, PYCOOL_ENOMEM, "cufftPlan3d(%d^3, D2Z) failed", N);
+  }
+  const int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)148 * 64);
+  const void* base = which == 0 ? c->phi[c->cur] : c->pi[c->cur];
+  if (c->precision == 32)
+    gather_real<float><<<nb, 256, 0, c->stream>>>((double*)scratch, (const float*)base + (size_t)field * c->lay.field, c->lay);
+  else
+    gather_real<double><<<nb, 256, 0, c->stream>>>((double*)scratch, (const double*)base + (size_t)field * c->lay.field, c->lay);
+  cufftResult fr = fft.exec_d2z(plan, (cufftDoubleReal*)scratch, (cufftDoubleComplex*)scratch);
+  const double norm = c->L * std::sqrt(c->L) / (std::sqrt(2.0) * (double)N * (double)N * (double)N);
+  bin_shells<<<nblk, 256, 2 * nbins * sizeof(double), c->stream>>>(scratch, N, norm * norm, nbins, part);
+  double* out = part + (size_t)nblk * 2 * nbins;
+  reduce_shells<<<(2 * nbins + 255) / 256, 256, 0, c->stream>>>(part, nblk, 2 * nbins, out);
+  cudaError_t e = cudaGetLastError();
+  std::vector<double> h(2 * (size_t)nbins);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), out, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  fft.destroy(plan);
+  cudaFree(scratch); cudaFree(part);
+  c->counts[3] += 3;
+  if (fr != CUFFT_SUCCESS) return fail(c, PYCOOL_ECUDA, "cufftExecD2Z failed");
+  CUDA_TRY(c, e);
+  for (int i = 0; i < nbins; ++i) { power_host[i] = h[i]; count_host[i] = h[nbins + i]; }
+  return PYCOOL_OK;
 }
 
 int pycool_set_background(pycool_ctx* c, double a, double p_a) {

@@ -111,3 +111,57 @@ def test_init_fields_argument_errors(pc):
     h.init_fields(1, [(0, 1, 1, 0, 0)], [(0, 1, 1, 0, 0)])
     h.set_background(1.0, 0.0)
     h.step(1)
+
+
+# ------------------------------------------------------------------------------------- shell spectrum (rank 3)
+@pytest.mark.parametrize("N,precision", [(16, 64), (40, 64), (33, 64), (64, 32), (130, 64)])
+def test_field_spectrum_matches_the_oracle(pc, N, precision):
+    """pycool_field_spectrum (gather + cuFFT D2Z + shell sums) of phi and pi of both fields, after two steps, against
+    numpy's rfftn + bincount on the lattice read back; even, odd and ragged N; mode counts exact."""
+    cfg = inputs.config("cfg0b_chaotic32_resolved", N=N)
+    cfg["amp"] = 1e-3
+    phi, pi = inputs.make_initial(cfg, precision=precision)
+    g = pc.from_config(cfg, precision=precision)
+    g.set_fields(phi, pi); g.set_background(1.0)
+    g.step(2)
+    pg, qg = g.read_fields()
+    for f in range(2):
+        for which, arr in ((0, pg), (1, qg)):
+            S, Cn = g.field_spectrum(f, which)
+            So, Co = ics.shell_spectrum(arr[f], cfg["L"])
+            assert len(S) == len(So) == int(math.sqrt(3) * N / 2 + 0.5) + 1
+            assert np.array_equal(Cn, Co) and Cn.sum() == N ** 3
+            nz = So > 0
+            assert np.max(np.abs(S[nz] - So[nz]) / So[nz]) <= 1e-10
+            assert np.all(S[~nz] == 0)
+    short, _ = g.field_spectrum(0, 0, nbins=5)
+    full, _ = g.field_spectrum(0, 0)
+    assert np.allclose(short, full[:5], rtol=1e-12, atol=0)
+
+
+def test_spectrum_of_the_generated_lattice_returns_its_amplitude(pc):
+    """Round trip on the device: init_fields with A(k), field_spectrum back: power/count = A(k_shell)^2 within the
+    statistical error of the shell (and the shell's width in k)."""
+    N, L, amp, m2 = 128, 10.0, 1e-3, 4.0
+    g = pc.Lattice(N, L, 1, pc.FREE, [1.0], order=2, dt=0.01, mpl=1.0)
+    g.init_fields(5, [(0.5, amp, m2, -0.25, 0.0)], [(0.0, amp, m2, 0.25, 0.0)])
+    for which, q in ((0, -0.25), (1, 0.25)):
+        S, Cn = g.field_spectrum(0, which)
+        for i in (4, 10, 30, 60):
+            k = 2 * math.pi / L * i
+            want = (amp * (k * k + m2) ** q) ** 2
+            assert abs(S[i] / Cn[i] / want - 1) < 6 / math.sqrt(Cn[i]) + 0.02
+    S, _ = g.field_spectrum(0, 0)
+    assert abs(S[0] - L ** 3 / 2 * 0.25) < 1e-9 * S[0]                      # the mean sits in shell 0
+
+
+def test_field_spectrum_argument_errors(pc):
+    g = pc.Lattice(8, 1.0, 1, pc.FREE, [1.0], order=2, dt=0.01, mpl=1.0)
+    with pytest.raises(pc.PycoolError) as ei:
+        g.field_spectrum(0)
+    assert ei.value.code == pc.ESTATE
+    g.init_fields(1, [(0, 1, 1, 0, 0)], [(0, 1, 1, 0, 0)])
+    for args in ((1, 0), (0, 2), (-1, 0)):
+        with pytest.raises(pc.PycoolError) as ei:
+            g.field_spectrum(*args)
+        assert ei.value.code == pc.EINVAL

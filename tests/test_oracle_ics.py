@@ -112,7 +112,7 @@ def test_shell_spectrum_of_a_single_mode_and_parseval():
         i = int(math.floor(math.sqrt(sum(v * v for v in m)) + 0.5))
         assert abs(S[i] - L ** 3 * A * A / 4) < 1e-12 * S[i]
         assert np.all(np.delete(S, i) < 1e-25)
-    assert C[0] == 1 and C[1] == 6 + 12 and C.sum() == N ** 3 and len(C) == int(math.sqrt(3) * N / 2) + 1
+    assert C[0] == 1 and C[1] == 6 + 12 and C.sum() == N ** 3 and len(C) == int(math.sqrt(3) * N / 2 + 0.5) + 1
     rng = np.random.default_rng(0)
     f = rng.standard_normal((N, N, N)) + 0.4
     S, _ = ics.shell_spectrum(f, L)
