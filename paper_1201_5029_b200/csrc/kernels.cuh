@@ -1,10 +1,14 @@
 // kernels.cuh -- sm_100a kernels of the symplectic lattice step (arXiv 1201.5029 §2.3, eq. (2.47)-(2.48)).
 //
 //   kick_fused      one pass per stage: merged drift (H2 halves of two adjacent stages) + kick (H3) + the three
-//                   lattice sums, 2.5D z-march with an x-y tile (+1 halo) in shared memory.
-//   scalar_update   fixed-order reduction of the per-block partial sums and the (a, p_a) updates of H1, H2, H3
+//                   lattice sums, 2.5D z-march with an x-y tile (+1 halo) in shared memory; register-prefetch
+//                   loads, any N (the TMA-fed kernel for even N is kick_tma.cuh).
+//   stage_finish    tail of either kick: the last block to finish adds the per-item partial sums in index order
+//                   and advances (a, p_a) through H3, H2, H1 and the next stage's coefficients (scalar_advance)
 //                   on the device (the paper does these on the CPU after a D2H copy).
-//   drift_flush     closing half drift phi += c pi at the end of a pycool_step call.
+//   scalar_update   the same as a stand-alone launch: opens a pycool_step call (and follows every kick when the
+//                   fused tail is switched off).
+//   drift_flush     deferred closing half drift phi += c pi, applied when phi is looked at.
 //   sumsq / energy  lattice sums for set_fields and pycool_energies ((2.8), (2.16)).
 //
 // Layout [field][z][y][x], x fastest.  See DESIGN.md for the derivation of the merged drift, the register

@@ -2,11 +2,14 @@
 //
 // The host side only validates arguments, owns buffers and enqueues kernels; a, p_a and every lattice sum live
 // on the device, so pycool_step never synchronises (the paper copies the sums to the host at every sub-step,
-// PAPER.md:395).  Sequence of one pycool_step(n) call, stages h_1..h_S (S = n * stages(order), h = w dt):
-//     scalar_update(mode 0, h_next = h_1)
-//     for i in 1..S:  kick_fused (drift by c_drift, kick by h_i, sums)  ->  scalar_update(mode 1, h_i, h_{i+1})
-//     drift_flush  (closing half drift, c_drift = h_S/(2 a^2))
+// PAPER.md:395).  Sequence of one pycool_step(n) call, stages w_1..w_S (S = n * stages(order), h = w * step length):
+//     scalar_update(mode 0, or 2 when the previous call's closing half drift is still pending)
+//     for i in 1..S:  kick_tma / kick_fused: drift by c_drift, kick by h_i, sums; its last block reduces the
+//                     partial sums and advances a, p_a, c_drift, kD, kV for stage i+1 (stage_finish)
+//     (the closing half drift stays pending: the next call merges it, anything that reads phi applies it first)
 // which is (2.48) composed per (2.43)-(2.45) with adjacent H1 and H2 halves merged.
+// Other files: kick_tma.cuh (the hot kernel), kernels.cuh (scalars, generic kernel, pointwise kernels),
+// energy_tma.cuh (pycool_energies), init_fields.cuh (initial conditions, spectra), potentials.cuh (models).
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
