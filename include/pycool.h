@@ -220,8 +220,9 @@ int pycool_set_energy_kernel(pycool_ctx*, int tma);
 int pycool_set_persistent(pycool_ctx*, int on);
 /* Select the variant of the fused kernel; -1 = automatic (by model, precision, number of fields and N).
  *   0..2: register-prefetch kernel, x-y tiles 32x8, 32x16, 64x16 sites (any N);
- *   3..8: TMA-fed kernel (even N >= 4 only, else PYCOOL_EINVAL): tiles 64x16, 32x16, 128x8, 128x16 with 2 x 2
- *         sites per thread; 32x16, 64x8 with 2 x 1 sites per thread and two blocks per SM.
+ *   3..9: TMA-fed kernel (even N >= 4 only, else PYCOOL_EINVAL): tiles 64x16, 32x16, 128x8, 128x16 with 2 x 2
+ *         sites per thread; 32x16, 64x8 with 2 x 1 sites per thread and two blocks per SM; 128x16 with 2 x 4
+ *         sites per thread (one-field lattices).
  * PYCOOL_EINVAL also if the variant's TMA ring does not fit in shared memory for this model and precision. */
 int pycool_set_tile(pycool_ctx*, int tile);
 

@@ -69,7 +69,7 @@ struct TmaTile {
   static constexpr int NT = (TX / 2) * (TY / J);        // threads: 2 x J sites each
   static constexpr int HR = (TX + 4) / 2;               // halo pairs in the top (and bottom) box row: x = -2 .. TX+1
   static constexpr int NHP = 2 * HR + 2 * TY;           // ring of halo pairs the stencil reads (x pairs)
-  static_assert(TX % 2 == 0 && TY % J == 0 && (J == 1 || J == 2), "2 x J sites per thread");
+  static_assert(TX % 2 == 0 && TY % J == 0 && (J == 1 || J == 2 || J == 4), "2 x J sites per thread");
   static_assert(NT % 32 == 0 && NT <= 1024, "block size");
   static_assert(PX <= 256 && RY <= 256, "TMA box extents");
 };

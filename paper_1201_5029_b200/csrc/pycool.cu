@@ -65,7 +65,7 @@ int stage_weights_ld(int order, long double* w) {
 constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
 constexpr size_t kMaxSmem = 227 * 1024;  // dynamic shared memory one block may opt in to on sm_100
 constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
-constexpr int kNumTiles = 9;             // + kick_tma variants (ghost layout only)
+constexpr int kNumTiles = 10;            // + kick_tma variants (ghost layout only)
 
 struct TileInfo { int tx, ty, nt, stages; };   // stages > 0: TMA ring depth
 
@@ -145,7 +145,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 //                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
 const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
                                     {64, 16, 256, 3}, {32, 16, 128, 3}, {128, 8, 256, 3},
-                                    {128, 16, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}};
+                                    {128, 16, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}, {128, 16, 256, 3}};
 using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 16, 2>;
@@ -157,7 +157,8 @@ template <typename Real> using TTile5 = TmaTile<Real, 128, 8, 3, 2, sizeof(Real)
 template <typename Real> using TTile6 = TmaTile<Real, 128, 16, 3, 2, 1>;  // 512 threads: twice the bytes per plane (one field)
 template <typename Real> using TTile7 = TmaTile<Real, 32, 16, 3, 1, 2>;   // 256 threads x (2 x 1 sites), two blocks per
 template <typename Real> using TTile8 = TmaTile<Real, 64, 8, 3, 1, 2>;    //   SM: ALU-heavy models (Q-ball)
-#define PYCOOL_TMA_TILES(X) X(3, TTile3) X(4, TTile4) X(5, TTile5) X(6, TTile6) X(7, TTile7) X(8, TTile8)
+template <typename Real> using TTile9 = TmaTile<Real, 128, 16, 3, 4, 1>;   // 256 threads x (2 x 4 sites): one field
+#define PYCOOL_TMA_TILES(X) X(3, TTile3) X(4, TTile4) X(5, TTile5) X(6, TTile6) X(7, TTile7) X(8, TTile8) X(9, TTile9)
 
 // Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
 Layout make_layout(int N, int nf, size_t esize) {
@@ -458,17 +459,18 @@ long long dispatch(pycool_ctx* c, Op op, int arg) {
 // (odd N); else the first TMA variant of a preference list whose ring fits in shared memory.
 //   two fields fp64, one field fp32: 64 x 16 tile; two or more fields fp32: 128 x 8 (512-byte rows; the fp32
 //   instances of both are cut for two blocks per SM, which is what fp32 needs: half the bytes per plane);
-//   one field fp64: 128 x 16 (a plane of a 64 x 16 box is too few bytes in flight);
+//   one field fp64: 128 x 16 with 2 x 4 sites per thread (twice the work per plane and per barrier; a ring of 6
+//   with the 64 x 16 tile gains nothing, so it is the per-plane fixed cost, not the bytes in flight);
 //   Q-ball (the logarithm makes it ALU-heavy): 32 x 16 with 2 x 1 sites per thread, two blocks per SM.
 int auto_tile(pycool_ctx* c) {
   const Layout& L = c->lay;
   if (L.gx == 0) return L.N <= 64 ? 0 : 1;
   if (L.N <= 64) return 4;
-  static const int pref_default[] = {3, 4}, pref_one[] = {6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {5, 3, 4};
+  static const int pref_default[] = {3, 4}, pref_one[] = {9, 6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {5, 3, 4};
   const int* pref = pref_default;
   int n = 2;
   if (c->model == PYCOOL_QBALL && c->precision == 64) { pref = pref_alu; n = 2; }
-  else if (c->nf == 1 && c->precision == 64) { pref = pref_one; n = 3; }
+  else if (c->nf == 1 && c->precision == 64) { pref = pref_one; n = 4; }
   else if (c->precision == 32 && c->nf >= 2) { pref = pref_f32; n = 3; }
   for (int i = 0; i < n; ++i)
     if ((size_t)dispatch(c, OP_SMEM, pref[i]) <= kMaxSmem) return pref[i];

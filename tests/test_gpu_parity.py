@@ -140,16 +140,16 @@ def test_all_orders(pc, order):
 
 
 def set_tile_or_skip(pc, g, tile):
-    """Variant 6 (128 x 16: twice the bytes per plane) does not fit in shared memory for two fp64 fields: EINVAL."""
+    """Variants 6 and 9 (128 x 16: twice the bytes per plane) do not fit in shared memory for two fp64 fields: EINVAL."""
     try:
         g.set_tile(tile)
     except pc.PycoolError as e:
-        assert e.code == pc.EINVAL and tile == 6 and "shared memory" in str(e)
+        assert e.code == pc.EINVAL and tile in (6, 9) and "shared memory" in str(e)
         return False
     return True
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9])
 @pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32), (6, 0),
                                   (70, 9), (136, 50)])
 def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
@@ -184,7 +184,7 @@ def test_variants_agree_and_ghost_images_hold(pc, precision):
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg, precision=precision)
     outs = []
-    for tile in range(9):
+    for tile in range(10):
         g = pc.from_config(cfg, precision=precision)
         if not set_tile_or_skip(pc, g, tile):
             assert precision == 64
@@ -281,6 +281,24 @@ def test_four_fields_auto_variant_fits_shared_memory(pc, precision):
     start(g, o, phi, pi, 1.0, 0.0)
     g.step(2); o.step(2)
     compare(g, o, nf, 5e-13 if precision == 64 else 1e-5, tol_scalar=1e-10 if precision == 64 else 1e-5, static=True)
+
+
+@pytest.mark.parametrize("N,zc", [(6, 0), (40, 7), (70, 16), (136, 5), (260, 0)])
+def test_one_field_variant_two_by_four_sites_per_thread(pc, N, zc):
+    """Variant 9 (128 x 16 tile, 2 x 4 sites per thread: the automatic choice for one fp64 field above N = 64) on
+    the oscillon model: ragged tiles in x and y, lattice faces, z-chunks, against the oracle."""
+    cfg = inputs.config("cfg2_oscillon256", N=N)
+    cfg["L"] = cfg["L"] * N / 256
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    g.set_tile(9); g.set_zchunk(zc)
+    geo = g.kick_geometry()
+    assert geo["variant"] == 9 and geo["threads"] == 256 and geo["tx"] == 128 and geo["ty"] == 16
+    start(g, o, phi, pi)
+    g.step(3); o.step(3)
+    compare(g, o, 1, 5e-12)
+    if N > 64:
+        assert pc.from_config(cfg).kick_geometry()["variant"] == 9
 
 
 # ------------------------------------------------------------------------------------- energies (row a7)
