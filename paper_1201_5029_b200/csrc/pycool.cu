@@ -478,15 +478,22 @@ int auto_tile(pycool_ctx* c) {
 }
 
 // Automatic z-chunk.  Short chunks keep the blocks in flight (x-y neighbours) within a few planes of each other,
-// so their halo rows hit L2; each chunk re-reads two halo planes.  Measured optimum for lattices with many
-// items per resident block: 16 planes (32 at N >= 1024).  Small lattices: the chunk length that minimises
+// so their halo rows hit L2; each chunk re-reads two halo planes and costs a fixed number of instructions.  Which
+// length wins depends on the board's power state (profiles/r1d): measured cold (a pause before every sample) the
+// fp64 64 x 16 kernel is fastest at 8 planes at 512^3 (1.446 ms; 16: 1.466; 32: 1.508) and 12 at 1024^3, but inside
+// a sustained run (bench.py: 60-140 launches back to back, sw_power_cap) 8 planes lose 7 % (4.83 vs 4.51-4.57
+// ms/step) and 16-24 are level (order 6: 24 best; 1024^3: 24 best, 37.9 vs 38.4 (16) and 39.1 (32) ms/step).
+// Chosen for the sustained case: 16 planes, 24 at N >= 1024; fp32 128 x 8 tile: 24 at 512^3, 16 at 1024^3 (cold:
+// 0.776 vs 0.785 ms, 6.19 vs 6.34 ms).  Small lattices: the chunk length that minimises
 // rounds x (planes + 2 halo planes) + pipeline fill over the resident blocks.
 int auto_zchunk(pycool_ctx* c) {
   const int N = c->N, bxy = blocks_xy(N, c->tile);
   if (N <= 16) return N;
   int R = (int)dispatch(c, OP_RESIDENT, c->tile);
   if (R < 1) R = 148;
-  const int cap = N >= 1024 ? 32 : 16;
+  int cap = 16;
+  if (c->precision == 64 && c->tile == 3) cap = N >= 1024 ? 24 : 16;
+  else if (c->precision == 32 && c->tile == 5) cap = N >= 1024 ? 16 : (N >= 512 ? 24 : 16);
   auto items = [&](int zc) { return (long long)bxy * ((N + zc - 1) / zc); };
   if (items(cap) >= 4LL * R) return cap;
   int best = cap < N ? cap : N;
