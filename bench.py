@@ -65,13 +65,16 @@ def measured_peaks():
 
 
 def recorded_traffic(key):
-    """DRAM bytes per launch of the fused kernel from the committed ncu --set full capture, if any."""
-    p = os.path.join(ROOT, "profiles", "kick_traffic.json")
-    if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(key)
-        except Exception:
-            return None
+    """DRAM bytes per launch of the fused kernel from the committed ncu --set full capture, if any
+    (profiles/kick_traffic.txt: "<workload>/order<o>/fp<bits> <bytes>" lines)."""
+    p = os.path.join(ROOT, "profiles", "kick_traffic.txt")
+    try:
+        for line in open(p):
+            w = line.split()
+            if len(w) == 2 and w[0] == key:
+                return float(w[1])
+    except OSError:
+        pass
     return None
 
 
