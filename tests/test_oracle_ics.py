@@ -105,6 +105,7 @@ def test_shell_spectrum_of_a_single_mode_and_parseval():
     """A cos(2 pi m.x / N) has |F_{+-m}|^2 = (L^3/2)(A/2)^2 each: the shell round(|m|) holds L^3 A^2 / 4 and nothing
     else; counts: 1, 18 (|n|^2 = 1 and 2), ... and N^3 in total; Parseval: sum_i S_i = L^3 / (2 N^3) sum_x field^2."""
     N, L, A = 12, 3.0, 0.7
+    rng = np.random.default_rng(0)
     z, y, x = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
     for m in ((1, 0, 0), (0, 2, 1), (3, 3, 2), (0, 0, 5)):
         f = A * np.cos(2 * np.pi * (m[0] * x + m[1] * y + m[2] * z) / N + 0.3)
@@ -113,7 +114,16 @@ def test_shell_spectrum_of_a_single_mode_and_parseval():
         assert abs(S[i] - L ** 3 * A * A / 4) < 1e-12 * S[i]
         assert np.all(np.delete(S, i) < 1e-25)
     assert C[0] == 1 and C[1] == 6 + 12 and C.sum() == N ** 3 and len(C) == int(math.sqrt(3) * N / 2 + 0.5) + 1
-    rng = np.random.default_rng(0)
+    # The farthest mode sits at |n| = sqrt 3 N/2 (even N), so the last shell is round(sqrt 3 N/2), not
+    # floor(sqrt 3 N/2): the two differ whenever frac(sqrt 3 N/2) >= 1/2 (N = 16: 13.86 -> 14 vs 13; N = 12 cannot
+    # tell them apart).  A floor() binning would drop that shell and C.sum() would fall short of N^3.  Odd N: the
+    # farthest mode is at sqrt 3 (N-1)/2, every mode must still land in a bin.
+    for n in (16, 10, 9, 15):
+        Sn, Cn = ics.shell_spectrum(rng.standard_normal((n, n, n)), L)
+        far = math.sqrt(3) * (n // 2)
+        assert len(Cn) == int(math.floor(math.sqrt(3) * n / 2 + 0.5)) + 1 and Cn.sum() == n ** 3, n
+        assert Cn[int(math.floor(far + 0.5))] >= 1, n                           # the corner mode's own shell exists
+    assert math.floor(math.sqrt(3) * 16 / 2) + 1 == 14 and len(ics.shell_spectrum(np.ones((16,) * 3), L)[1]) == 15
     f = rng.standard_normal((N, N, N)) + 0.4
     S, _ = ics.shell_spectrum(f, L)
     assert abs(S.sum() - L ** 3 / (2 * N ** 3) * np.sum(f * f)) < 1e-12 * S.sum()
