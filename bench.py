@@ -3,6 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4_chaotic512] [--order 4]
                     [--precision 64] [--impl ours|reference]
+    python bench.py --sweep cfg4      # BASELINE.json configs[4]: 512^3, 1024^3 x fp64, fp32 x order 2, 4, 6, 50 steps
+                                      # each, one JSON line per cell (device-generated initial conditions)
 
 One "step" is one whole composite step of the chosen order (all stages: merged drift + kick + lattice sums +
 scalar update) over the whole lattice.  The metric is BASELINE.json's: lattice
@@ -14,7 +16,11 @@ site-updates per second per field, SU/s = N^3 * nfields * steps / time.  One JSO
   roofline  the fused drift+kick kernel: algorithmic bytes per launch (4 * sizeof(real) per field-site)
             / its average duration, bracketed per launch by CUDA events in a second pass of the same K steps
             (brackets between launches would switch off the launch overlap the first, timed pass runs with).
-  cpu_baseline  the CPU oracle, as it stands, on a bounded sub-lattice of the same workload (1 thread).
+            bound / traffic come from the committed ncu --set full summary of the SAME launch geometry
+            (profiles/kick_counters.txt, keyed by workload, precision, kernel variant and z-chunk); when the live
+            geometry has no capture they are reported as unknown, never carried over from another geometry.
+  cpu_baseline  the CPU oracle, as it stands, on a bounded sub-lattice of the same workload (1 thread): an accuracy
+            reference (three passes per stage, compensated long-double sums), NOT a tuned CPU implementation.
 --impl reference times that oracle alone (there is no reference implementation to install: the paper ships no
 code).  Multi-GPU: the path does not shard (north_star: one GPU); --gpus N runs N
 independent replicas, one per rank ("replicas only", weak scaling, no collective on the data path).
@@ -51,6 +57,9 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-init", action="store_true", help="skip the on-device initial-conditions timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--device-init", action="store_true",
+                    help="initial conditions from pycool_init_fields instead of host arrays (no e2e): for 1024^3 captures")
+    ap.add_argument("--sweep", default=None, choices=["cfg4"], help="print the configs[4] matrix, one JSON line per cell")
     return ap.parse_args()
 
 
@@ -64,18 +73,51 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def recorded_traffic(key):
-    """DRAM bytes per launch of the fused kernel from the committed ncu --set full capture, if any
-    (profiles/kick_traffic.txt: "<workload>/order<o>/fp<bits> <bytes>" lines)."""
-    p = os.path.join(ROOT, "profiles", "kick_traffic.txt")
+COUNTER_COLUMNS = ("dram_bytes", "duration_us", "dram_pct", "fp64_pct", "issue_pct", "warps_active_pct", "l2_hit_pct")
+
+
+def geometry_key(workload, precision, geo):
+    return "%s/fp%d/tile%d/zc%d" % (workload, precision, geo["variant"], geo["zchunk"])
+
+
+def recorded_counters(key):
+    """Per-launch ncu --set full counters of the fused kernel for exactly this workload, precision, kernel variant and
+    z-chunk, from the committed summary profiles/kick_counters.txt (lines "<key> <dram bytes> <duration us>
+    <dram %> <fp64 pipe %> <issue slots %> <warps active %> <L2 hit %>"), or None when that geometry has no capture."""
+    p = os.path.join(ROOT, "profiles", "kick_counters.txt")
     try:
         for line in open(p):
             w = line.split()
-            if len(w) == 2 and w[0] == key:
-                return float(w[1])
+            if len(w) == 1 + len(COUNTER_COLUMNS) and w[0] == key:
+                return dict(zip(COUNTER_COLUMNS, (float(x) for x in w[1:])))
     except OSError:
         pass
     return None
+
+
+def bound_from_counters(c):
+    """What the counters of the capture say limits the kernel: "hbm" when DRAM throughput is the busiest unit and it
+    is busy (>= 70 % of its peak); "alu" when the fp64 pipe or the issue slots are; otherwise the kernel waits on
+    latency with every unit partly idle -- then the roofline it is measured against stays HBM (the unit it would
+    saturate first: the busiest one) and `limiter` says so."""
+    units = {"dram": c["dram_pct"], "fp64 pipe": c["fp64_pct"], "issue slots": c["issue_pct"]}
+    top = max(units, key=units.get)
+    desc = ", ".join("%s %.0f %%" % kv for kv in units.items()) + ", warps active %.0f %%" % c["warps_active_pct"]
+    if units[top] < 70.0:
+        return "hbm", "latency/occupancy: no unit above 70 %% busy (%s); busiest: %s" % (desc, top)
+    return ("hbm" if top == "dram" else "alu"), "%s (%s)" % (top, desc)
+
+
+def host_description():
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"nproc": os.cpu_count(), "cpu_model": model}
 
 
 class ClockSampler:
@@ -168,6 +210,102 @@ def time_oracle(cfg, order, steps, warmup, precision):
     return units / dt, dt / steps * 1e3, sample
 
 
+ORACLE_NOTE = ("accuracy oracle: three passes per stage, Neumaier-compensated long-double sums, -ffp-contract=off, "
+               "1 thread; not a tuned CPU implementation and not a speed-up denominator")
+
+
+def cpu_baseline_block(v, sample):
+    d = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "note": ORACLE_NOTE}
+    d.update(host_description())
+    return d
+
+
+def timed_steps(lat, steps, barrier, stream):
+    """EXACTLY `steps` steps (one pycool_step call + the deferred closing drift) between two CUDA events on the
+    context's stream, nothing else in the stream.  Returns milliseconds."""
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    lat.step(steps)
+    lat.flush()                  # the deferred closing half drift belongs to these steps: inside the timed region
+    e1.record(stream)
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def roofline_block(lat, workload, precision, N, nf, steps, barrier):
+    """Second pass of the same `steps` steps with every fused drift+kick launch bracketed by CUDA events on the same
+    stream (pycool_set_profiling); the whole pass is timed too, for the kernel's share of a step."""
+    lat.sync()
+    time.sleep(1.0)              # let the board's power average recover, so both passes start from the same state
+    lat.step(1)                  # (untimed) clocks back up
+    lat.set_profiling(True)
+    ms_prof = timed_steps(lat, steps, barrier, lat.stream)
+    kick_ms, kick_n = lat.kick_time_ms()
+    lat.set_profiling(False)
+    peak, peak_src = measured_peaks()
+    esz = precision // 8
+    alg_bytes = 4.0 * esz * N ** 3 * nf                       # read phi, pi; write phi, pi (DESIGN.md)
+    kick_avg_ms = kick_ms / max(kick_n, 1)
+    achieved = alg_bytes / (kick_avg_ms * 1e-3) / 1e9
+    geo = lat.kick_geometry()
+    key = geometry_key(workload, precision, geo)
+    cnt = recorded_counters(key)
+    roof = {"bound": "hbm", "kernel": "kick_tma" if geo["tma_stages"] > 0 else "kick_fused", "achieved": achieved,
+            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
+            "algorithmic_bytes_per_launch": alg_bytes, "launches_timed": kick_n, "avg_launch_ms": kick_avg_ms,
+            "kernel_share_of_step": kick_ms / ms_prof, "geometry": geo, "capture_key": key,
+            "measured": "second pass of the same %d steps with every launch bracketed by CUDA events" % steps}
+    if cnt:
+        roof["bound"], roof["limiter"] = bound_from_counters(cnt)
+        roof["traffic"] = cnt["dram_bytes"]
+        roof["traffic_over_algorithmic"] = cnt["dram_bytes"] / alg_bytes
+        roof["ncu"] = cnt
+        roof["bound_source"] = "ncu --set full capture of this geometry (profiles/kick_counters.txt)"
+    else:
+        roof["bound_source"] = ("assumed: no committed ncu capture for %s (traffic unknown, never carried over from "
+                                "another geometry)" % key)
+    return roof
+
+
+def sweep_cfg4(a, dev, barrier):
+    """BASELINE.json configs[4]: the two-field chaotic model at 512^3 and 1024^3, fp64 and fp32, order 2/4/6, 50
+    steps each.  Initial conditions are generated on the device (pycool_init_fields: no 34 GB host arrays), so the
+    cells carry no e2e; one JSON line per cell."""
+    import torch
+    from paper_1201_5029_b200 import binding, inputs
+    steps = 50
+    for name in ("cfg4_chaotic512", "cfg4_chaotic1024"):
+        for precision in (64, 32):
+            cfg = inputs.config(name)
+            N, nf = cfg["N"], cfg["nfields"]
+            for order in (2, 4, 6):
+                lat = binding.from_config(cfg, device=dev, order=order, precision=precision)
+                lat.init_fields(cfg["seed"], *inputs.spectra(cfg))
+                lat.set_background(1.0)
+                sampler = ClockSampler(dev.index or 0)
+                sampler.start(); sampler.wait_first()
+                lat.step(max(a.warmup, 3)); lat.sync()
+                c0 = lat.launch_counts()
+                ms = timed_steps(lat, steps, barrier, lat.stream)
+                launches = sum(lat.launch_counts()) - sum(c0)
+                roof = roofline_block(lat, name, precision, N, nf, steps, barrier)
+                clocks = sampler.stop()
+                line = {"metric": METRIC, "value": whole_job_value(N, nf, steps, 1, ms * 1e-3), "unit": UNIT, "n_gpus": 1,
+                        "steps": steps, "warmup": max(a.warmup, 3), "ms_per_step": ms / steps, "higher_is_better": True,
+                        "scaling": "weak", "vs_baseline": None, "dtype": "f%d" % precision, "data": "synthetic",
+                        "config": {"workload": "%s: %d^3 x %d fields, model %d, order %d, dt=%g, %d-bit (sweep cell)"
+                                   % (name, N, nf, cfg["model"], order, cfg["dt"], precision),
+                                   "l2": "inputs larger than L2", "parallelism": "single GPU",
+                                   "inputs": "pycool_init_fields (device-generated vacuum spectrum)"},
+                        "clocks": clocks, "gpu_launches": launches, "roofline": roof, "a_final": lat.energies().a}
+                print(json.dumps(line), flush=True)
+                lat.close()
+                del lat
+                torch.cuda.empty_cache()
+
+
 def main():
     a = parse()
     from paper_1201_5029_b200 import inputs
@@ -180,7 +318,9 @@ def main():
     N, nf = cfg["N"], cfg["nfields"]
     config = {"workload": "%s: %d^3 x %d fields, model %d, order %d, dt=%g, %d-bit" %
               (a.workload, N, nf, cfg["model"], order, cfg["dt"], a.precision),
-              "l2": "inputs larger than L2 (state %.1f GiB vs 126 MB)" % (2 * nf * N ** 3 * (a.precision // 8) / 2 ** 30),
+              "l2": ("inputs larger than L2 (state %.1f GiB vs 126 MB)" if 2 * nf * N ** 3 * (a.precision // 8) > 126e6 else
+                     "state %.3f GiB FITS in the 126 MB L2: the HBM roofline is not the yardstick for this workload")
+                    % (2 * nf * N ** 3 * (a.precision // 8) / 2 ** 30),
               "parallelism": "replicas only" if a.gpus > 1 else "single GPU"}
 
     if a.impl == "reference":
@@ -191,7 +331,7 @@ def main():
         line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
                 "warmup": a.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f%d" % a.precision, "data": "synthetic", "config": config,
-                "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                "cpu_baseline": cpu_baseline_block(v, sample),
                 "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                 "gpu_launches": 0}
         print(json.dumps(line))
@@ -208,11 +348,26 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    phi, pi = inputs.make_initial(cfg, precision=a.precision)
-    tdt = torch.float32 if a.precision == 32 else torch.float64
-    h_phi = torch.from_numpy(phi).pin_memory()
-    h_pi = torch.from_numpy(pi).pin_memory()
-    del phi, pi
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    if a.sweep:
+        if rank == 0:
+            sweep_cfg4(a, dev, barrier if world == 1 else (lambda: torch.cuda.synchronize(dev)))
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    if a.device_init:
+        a.no_e2e = True
+    else:
+        phi, pi = inputs.make_initial(cfg, precision=a.precision)
+        h_phi = torch.from_numpy(phi).pin_memory()
+        h_pi = torch.from_numpy(pi).pin_memory()
+        del phi, pi
     lat = binding.from_config(cfg, device=dev, order=order, precision=a.precision)
     if a.tile >= 0:
         lat.set_tile(a.tile)
@@ -222,7 +377,11 @@ def main():
         lat.set_persistent(a.persistent)
     if a.fused_tail >= 0:
         lat.set_fused_tail(a.fused_tail)
-    lat.set_fields(h_phi, h_pi)
+    if a.device_init:
+        lat.init_fields(cfg["seed"], *inputs.spectra(cfg))
+        config["inputs"] = "pycool_init_fields (device-generated)"
+    else:
+        lat.set_fields(h_phi, h_pi)
     lat.set_background(1.0)
     # clocks and throttle reasons are sampled from here (warm-up: the same steps as the timed region) to the end
     # of the timed region; nvidia-smi needs ~0.1 s to deliver its first line, the timed region may be shorter
@@ -233,43 +392,17 @@ def main():
     lat.step(a.warmup)
     lat.sync()
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize(dev)
-
     # ---- device-resident timing: EXACTLY K steps between two events on the context stream, nothing else in the
     # stream (event records between launches would switch off the stage-to-stage launch overlap)
     c0 = lat.launch_counts()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record(lat.stream)
-    lat.step(a.steps)
-    lat.flush()                  # the deferred closing half drift belongs to these steps: inside the timed region
-    ev1.record(lat.stream)
-    barrier()
-    ms = ev0.elapsed_time(ev1)
+    ms = timed_steps(lat, a.steps, barrier, lat.stream)
     c1 = lat.launch_counts()
     launches = sum(c1) - sum(c0)
     ms = max_over_ranks(ms, world, dev)
     value = whole_job_value(N, nf, a.steps, world, ms * 1e-3)
 
-    # ---- roofline pass: the same K steps again, every fused drift+kick launch bracketed by CUDA events on the
-    # same stream (pycool_set_profiling); the whole pass is timed too, for the kernel's share of a step
-    lat.sync()
-    time.sleep(1.0)              # let the board's power average recover, so both passes start from the same state
-    lat.step(1)                  # (untimed) clocks back up
-    lat.set_profiling(True)
-    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev2.record(lat.stream)
-    lat.step(a.steps)
-    lat.flush()
-    ev3.record(lat.stream)
-    barrier()
-    ms_prof = ev2.elapsed_time(ev3)
-    kick_ms, kick_n = lat.kick_time_ms()
-    lat.set_profiling(False)
+    # ---- roofline pass (per-launch CUDA events)
+    roof = roofline_block(lat, a.workload, a.precision, N, nf, a.steps, barrier)
     clocks = sampler.stop() if rank == 0 else None
     lat.sync()
 
@@ -328,18 +461,8 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    peak, peak_src = measured_peaks()
+    peak, _ = measured_peaks()
     esz = a.precision // 8
-    alg_bytes = 4.0 * esz * N ** 3 * nf                       # read phi, pi; write phi, pi
-    kick_avg_ms = kick_ms / max(kick_n, 1)
-    achieved = alg_bytes / (kick_avg_ms * 1e-3) / 1e9
-    geo = lat.kick_geometry()
-    roof = {"bound": "hbm", "kernel": "kick_tma" if geo["tma_stages"] > 0 else "kick_fused", "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "peak_source": peak_src,
-            "traffic": recorded_traffic("%s/order%d/fp%d" % (a.workload, order, a.precision)),
-            "algorithmic_bytes_per_launch": alg_bytes, "launches_timed": kick_n, "avg_launch_ms": kick_avg_ms,
-            "kernel_share_of_step": kick_ms / ms_prof, "geometry": geo,
-            "measured": "second pass of the same %d steps with every launch bracketed by CUDA events" % a.steps}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f%d" % a.precision, "data": "synthetic", "config": config, "clocks": clocks,
@@ -355,7 +478,7 @@ def main():
     if not a.no_cpu_baseline and world == 1:
         stages = {2: 1, 4: 3, 6: 7, 8: 15}[order]
         v, _, sample = time_oracle(cfg, order, max(1, round(100 / stages)), 1, a.precision)     # ~13 s of CPU work
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+        line["cpu_baseline"] = cpu_baseline_block(v, sample)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

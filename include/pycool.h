@@ -25,6 +25,10 @@
  *     (reading G16).
  *   - work is enqueued on the context's CUDA stream; calls that return data synchronise that stream first.
  *   - a context is not thread-safe; distinct contexts are independent.
+ *   - a context lives on one CUDA device: the device that is current when pycool_create is called, or the device
+ *     that owns d_work for pycool_create_ext.  Every later call switches to that device for its own duration and
+ *     restores the caller's current device, so contexts on several GPUs can be driven from one thread
+ *     ("many simulations simultaneously").
  */
 #ifndef PYCOOL_H
 #define PYCOOL_H
@@ -127,7 +131,7 @@ int pycool_init_fields(pycool_ctx*, unsigned long long seed, const pycool_spectr
  * F_k = L^1.5 / (sqrt 2 N^3) sum_x field(x) exp(-2 pi i n.x/N) -- the convention of pycool_init_fields turned around,
  * so a field made with spectrum A(k) gives <power/count> = A(k)^2 --
  *   power[i] = sum |F_k|^2 and count[i] = number of modes over the full spectrum with round(|n|) = i, i < nbins
- * (nbins = round(sqrt 3 N/2) + 1 covers every mode; the mean sits in power[0]).  field in [0, nfields), which = 0
+ * (nbins = round(sqrt 3 N/2) + 1 covers every mode; 1 <= nbins <= 3072; the mean sits in power[0]).  field in [0, nfields), which = 0
  * for phi, 1 for pi.  cuFFT D2Z on a double copy; the shell sums use atomics, so the last bits are not
  * reproducible from run to run.  Applies a pending closing drift first.  Synchronises. */
 int pycool_field_spectrum(pycool_ctx*, int field, int which, int nbins, double* power_host, double* count_host);
@@ -196,7 +200,9 @@ int pycool_set_profiling(pycool_ctx*, int on);
 /* Sum of the bracketed durations (ms) and their number since profiling was switched on.  Synchronises. */
 int pycool_kick_time_ms(pycool_ctx*, double* total_ms, unsigned long long* launches);
 /* Launch geometry of the fused kernel: tile[0..2] = TX, TY, z-chunk; tile[3] = threads per block;
- * tile[4] = blocks per launch; tile[5] = dynamic shared memory bytes; tile[6] = variant index (pycool_set_tile);
+ * tile[4] = work items (x-y tile, z-chunk) per launch -- the grid size of a one-block-per-item launch; a persistent
+ * launch uses min(items, resident blocks) blocks; tile[5] = dynamic shared memory bytes; tile[6] = variant index
+ * (pycool_set_tile);
  * tile[7] = TMA ring stages (0 = the register-prefetch kernel). */
 int pycool_kick_geometry(const pycool_ctx*, int tile[8]);
 /* Override the z-chunk length (planes per block; 0 = automatic) before the next step. */
@@ -214,16 +220,22 @@ int pycool_set_overlap(pycool_ctx*, int on);
  * 2 G[psi] = D[psi^2] - 2 psi D[psi]); 0 = the plain one-thread-per-site kernel that evaluates (2.8) term by term
  * (always used for odd N or more than two fields).  They agree to rounding. */
 int pycool_set_energy_kernel(pycool_ctx*, int tma);
-/* Persistent launch of the TMA-fed kernel (default on): as many blocks as fit on the device at once, each
- * taking work items (x-y tile, z-chunk) round-robin with its TMA ring running on across item boundaries.
- * Off: one block per work item.  Partial sums are indexed by work item, so results are bitwise the same. */
+/* Persistent launch of the TMA-fed kernel (default on): as many blocks as fit on the device at once; a block's
+ * first work item (x-y tile, z-chunk) is its index, every further one is claimed from a device counter
+ * (atomicAdd) in index order -- the order a hardware block scheduler would hand them out, which keeps the blocks
+ * in flight x-y neighbours (a static round-robin deal was measured 1.5x slower) -- with the TMA ring
+ * running on across item boundaries.  Off: one block per work item.  Partial sums are indexed by work item, so
+ * results are bitwise the same whichever block computes what. */
 int pycool_set_persistent(pycool_ctx*, int on);
 /* Select the variant of the fused kernel; -1 = automatic (by model, precision, number of fields and N).
- *   0..2: register-prefetch kernel, x-y tiles 32x8, 32x16, 64x16 sites (any N);
- *   3..9: TMA-fed kernel (even N >= 4 only, else PYCOOL_EINVAL): tiles 64x16, 32x16, 128x8, 128x16 with 2 x 2
+ *   0..2: register-prefetch kernel, x-y tiles 32x8, 32x16, 64x8 sites (any N);
+ *   3..10: TMA-fed kernel (even N >= 4 only, else PYCOOL_EINVAL): tiles 64x16, 32x16, 128x8, 128x16 with 2 x 2
  *         sites per thread; 32x16, 64x8 with 2 x 1 sites per thread and two blocks per SM; 128x16 with 2 x 4
- *         sites per thread (one-field lattices).
- * PYCOOL_EINVAL also if the variant's TMA ring does not fit in shared memory for this model and precision. */
+ *         sites per thread (one-field lattices); 32x16 with 2 x 1 sites per thread, one block per SM (three and
+ *         four fp64 fields).
+ * PYCOOL_EINVAL also if the variant's TMA ring does not fit in shared memory for this model and precision, or
+ * if its per-thread state would not fit the register budget for this number of fields (such instances are not
+ * compiled: no variant that spills is shipped). */
 int pycool_set_tile(pycool_ctx*, int tile);
 
 #if defined(__GNUC__)

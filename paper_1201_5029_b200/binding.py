@@ -133,7 +133,9 @@ class Lattice:
     """One simulation context on a CUDA device.  Same call names as the C ABI.
 
     device: a torch device (default cuda:0).  The field and work buffers are torch tensors owned by this
-    object; the library computes in them on torch's current stream for that device.
+    object; the library computes in them on the stream that is torch's current stream for that device when the
+    Lattice is made.  The library records the device of the work buffer and runs every later call on it,
+    whatever device is current in the calling thread (several Lattices on several GPUs in one process are fine).
     """
 
     def __init__(self, N, L, nfields, model, p=(), order=4, dt=0.01, device=None, **kw):
@@ -170,16 +172,28 @@ class Lattice:
             raise PycoolError(EINVAL, "field buffer has %d elements" % x.size)
         return x
 
+    def _check_tensor(self, t, name, want_cuda=None):
+        """A torch tensor handed to the library as a raw pointer: right dtype, size, layout and device."""
+        n = self.nf * self.N ** 3
+        if t.dtype != self._tdtype or t.numel() != n or not t.is_contiguous():
+            raise PycoolError(EINVAL, "%s must be a contiguous %s tensor of %d elements (got %s, %d, contiguous=%s)"
+                              % (name, self._tdtype, n, t.dtype, t.numel(), t.is_contiguous()))
+        if want_cuda is not None and t.is_cuda != want_cuda:
+            raise PycoolError(EINVAL, "%s is on %s: phi and pi must both be host or both be device tensors" % (name, t.device))
+        if t.is_cuda and t.device != self.device:
+            raise PycoolError(EINVAL, "%s is on %s, the lattice on %s" % (name, t.device, self.device))
+
     def set_fields(self, phi, pi):
-        """phi, pi: host arrays (numpy, or pinned torch CPU tensors) of nf*N^3 elements."""
+        """phi, pi: host arrays (numpy, or pinned torch CPU tensors) or torch tensors on the lattice's device, of
+        nf*N^3 elements each."""
         torch = self._torch
-        if isinstance(phi, torch.Tensor) and not phi.is_cuda:
-            assert phi.dtype == self._tdtype and phi.is_contiguous() and pi.is_contiguous()
-            self._chk(lib().pycool_set_fields(self._h, phi.data_ptr(), pi.data_ptr()))
-            return
-        if isinstance(phi, torch.Tensor):
-            assert phi.dtype == self._tdtype and phi.is_contiguous() and pi.is_contiguous()
-            self._chk(lib().pycool_set_fields_device(self._h, phi.data_ptr(), pi.data_ptr()))
+        if isinstance(phi, torch.Tensor) or isinstance(pi, torch.Tensor):
+            if not (isinstance(phi, torch.Tensor) and isinstance(pi, torch.Tensor)):
+                raise PycoolError(EINVAL, "phi and pi must both be torch tensors or both be arrays")
+            self._check_tensor(phi, "phi")
+            self._check_tensor(pi, "pi", want_cuda=phi.is_cuda)
+            fn = lib().pycool_set_fields_device if phi.is_cuda else lib().pycool_set_fields
+            self._chk(fn(self._h, phi.data_ptr(), pi.data_ptr()))
             return
         phi, pi = self._host(phi), self._host(pi)
         self._chk(lib().pycool_set_fields(self._h, phi.ctypes.data, pi.ctypes.data))
@@ -187,7 +201,8 @@ class Lattice:
     def init_fields(self, seed, phi_spec, pi_spec):
         """Seeded Gaussian initial conditions generated on the device.  *_spec: per field (mean, amp, m2, q, kmax),
         spectrum A(k) = amp (k^2 + m2)^q for k <= kmax (kmax <= 0: all k); see pycool_init_fields."""
-        assert len(phi_spec) == self.nf and len(pi_spec) == self.nf
+        if len(phi_spec) != self.nf or len(pi_spec) != self.nf:
+            raise PycoolError(EINVAL, "one spectrum per field is needed")
         a = (Spectrum * self.nf)(*[Spectrum(*map(float, t)) for t in phi_spec])
         b = (Spectrum * self.nf)(*[Spectrum(*map(float, t)) for t in pi_spec])
         self._chk(lib().pycool_init_fields(self._h, int(seed), a, b))
@@ -213,10 +228,20 @@ class Lattice:
         self._chk(lib().pycool_sync(self._h))
 
     def read_fields(self, out_phi=None, out_pi=None):
-        """Download to new numpy arrays, or into given host buffers (numpy or pinned torch tensors)."""
+        """Download to new numpy arrays, or into given host buffers (numpy or pinned torch CPU tensors)."""
         shape = (self.nf, self.N, self.N, self.N)
-        phi = np.empty(shape, self._np) if out_phi is None else out_phi
-        pi = np.empty(shape, self._np) if out_pi is None else out_pi
+        out = []
+        for name, buf in (("out_phi", out_phi), ("out_pi", out_pi)):
+            if buf is None:
+                buf = np.empty(shape, self._np)
+            elif isinstance(buf, self._torch.Tensor):
+                self._check_tensor(buf, name, want_cuda=False)
+            elif not (isinstance(buf, np.ndarray) and buf.dtype == self._np and buf.size == self.nf * self.N ** 3
+                      and buf.flags["C_CONTIGUOUS"] and buf.flags["WRITEABLE"]):
+                raise PycoolError(EINVAL, "%s must be a writable C-contiguous %s array of %d elements"
+                                  % (name, np.dtype(self._np).name, self.nf * self.N ** 3))
+            out.append(buf)
+        phi, pi = out
         ptr = lambda t: t.data_ptr() if isinstance(t, self._torch.Tensor) else t.ctypes.data
         self._chk(lib().pycool_read_fields(self._h, ptr(phi), ptr(pi)))
         return phi, pi
@@ -267,7 +292,7 @@ class Lattice:
     def kick_geometry(self):
         t = (C.c_int * 8)()
         self._chk(lib().pycool_kick_geometry(self._h, t))
-        return dict(tx=t[0], ty=t[1], zchunk=t[2], threads=t[3], blocks=t[4], smem_bytes=t[5], variant=t[6],
+        return dict(tx=t[0], ty=t[1], zchunk=t[2], threads=t[3], blocks=t[4], items=t[4], smem_bytes=t[5], variant=t[6],
                     tma_stages=t[7])
 
     def set_zchunk(self, planes):

@@ -173,24 +173,6 @@ __device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k,
   }
 }
 
-// Stand-alone form: reduces partials [3][nblocks] (mode 1) and advances the scalars.  Used for the opening of a
-// call (mode 0) and when the fused tail is switched off.
-__global__ void __launch_bounds__(kReduceThreads)
-scalar_update(Scalars* __restrict__ sc, const double* __restrict__ partials, int nblocks, ScalarConst k,
-              StageLen len, int mode) {
-  __shared__ double sh[kReduceThreads];
-  double SD = 0, SV = 0, SP = 0;
-  if (mode == 1) {
-    SD = block_sum_fixed<kReduceThreads>(partials, nblocks, sh);
-    SV = block_sum_fixed<kReduceThreads>(partials + nblocks, nblocks, sh);
-    SP = block_sum_fixed<kReduceThreads>(partials + 2 * (size_t)nblocks, nblocks, sh);
-  }
-  if (threadIdx.x != 0) return;
-  Scalars s = *sc;
-  scalar_advance(s, k, len, mode, SD, SV, SP);
-  *sc = s;
-}
-
 // Tail of a kick kernel.  Thread 0 of every block publishes the block's three partial sums (index = linear
 // block id, so the final order does not depend on arrival).  With a ticket counter (fused mode) the block that
 // arrives last -- every other block has published by then -- reduces all partials in index order and advances
@@ -534,23 +516,6 @@ __global__ void __launch_bounds__(256) sumsq(const Real* __restrict__ v, Layout 
   }
   block_reduce<1, 256>(acc, sh);
   if (threadIdx.x == 0) partials[blockIdx.x] = acc[0];
-}
-
-// out[q] = fixed-order sum of partials[q][0..nb);  grid = nq blocks
-__global__ void __launch_bounds__(kReduceThreads) reduce_rows(const double* __restrict__ partials, int nb,
-                                                             double* __restrict__ out) {
-  __shared__ double sh[kReduceThreads];
-  const double r = block_sum_fixed<kReduceThreads>(partials + (size_t)blockIdx.x * nb, nb, sh);
-  if (threadIdx.x == 0) out[blockIdx.x] = r;
-}
-
-__global__ void store_spi2(Scalars* sc, const double* v) {
-  sc->Spi2 = *v;
-  if (!isfinite(*v)) sc->nonfinite = 1;
-}
-__global__ void set_scalars(Scalars* sc, double a, double p_a, int set_pa) {
-  sc->a = a;
-  if (set_pa) sc->p_a = p_a;
 }
 
 // ------------------------------------------------------------------------------------------------ energies

@@ -311,11 +311,8 @@ template <typename Real, class Model, class T>
 __global__ void __launch_bounds__(T::NT, T::MINB)
 kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_pi,
          const TmaArgs<Real> g) {
-  using R2 = typename Vec2T<Real>::type;
   using SM = TmaSmem<Real, Model, T>;
-  constexpr int NF = Model::NF, TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J;
-  constexpr int PLANE = T::PLANE;
-  constexpr uint32_t ES = (uint32_t)sizeof(Real);
+  constexpr int TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J;
 
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* base = smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u);

@@ -76,6 +76,7 @@ __device__ __forceinline__ float log_of(float x) { return logf(x); }
 template <int NF_>
 struct Free {
   static constexpr int NF = NF_;
+  static constexpr bool kTestModel = true;
   template <typename T> struct Coef {
     T m2[NF_];
     __device__ explicit Coef(const ModelParams& mp) {
@@ -97,6 +98,7 @@ struct Free {
 
 struct Chaotic {
   static constexpr int NF = 2;
+  static constexpr bool kTestModel = false;
   template <typename T> struct Coef {
     T m2, g2;
     __device__ explicit Coef(const ModelParams& mp) : m2(T(mp.p[0])), g2(T(mp.p[1])) {}
@@ -114,6 +116,7 @@ struct Chaotic {
 
 struct Oscillon {
   static constexpr int NF = 1;
+  static constexpr bool kTestModel = false;
   template <typename T> struct Coef {
     T m2, lam, g6, hm2, ql, sg;
     __device__ explicit Coef(const ModelParams& mp)
@@ -130,6 +133,7 @@ struct Oscillon {
 
 struct QBall {
   static constexpr int NF = 2;
+  static constexpr bool kTestModel = false;
   template <typename T> struct Coef {
     T m2, K, invM2, six;
     __device__ explicit Coef(const ModelParams& mp)

@@ -24,11 +24,10 @@
 #include <cufft.h>      // types only: the library is loaded on demand (dlopen), not linked
 #include <dlfcn.h>
 
-#include "../../include/pycool.h"
-#include "kernels.cuh"
-#include "kick_tma.cuh"
-#include "energy_tma.cuh"
+#include "context.h"
 #include "init_fields.cuh"
+#include "scalar_kernels.cuh"
+#include "potentials.cuh"
 
 using namespace pycool;
 
@@ -62,70 +61,11 @@ int stage_weights_ld(int order, long double* w) {
   return 0;
 }
 
-constexpr int kMaxSumBlocks = 1184;      // 8 x 148 blocks for the sum / energy kernels
-constexpr size_t kMaxSmem = 227 * 1024;  // dynamic shared memory one block may opt in to on sm_100
-constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
-constexpr int kNumTiles = 10;            // + kick_tma variants (ghost layout only)
-
-struct TileInfo { int tx, ty, nt, stages; };   // stages > 0: TMA ring depth
-
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+thread_local std::string g_create_err = "no error";
 
 }  // namespace
 
-struct pycool_ctx {
-  int N = 0, nf = 0, order = 0, model = 0, precision = 64;
-  double L = 0, dx = 0, dt = 0, mpl = 1, rho_g = 0, rho_m = 0;
-  size_t V = 0, elems = 0, esize = 8;
-  double c[4] = {0, 0, 0, 0};
-  ModelParams mp{};
-  ScalarConst kc{};
-  int nstages = 0;
-  double w[16];
-  // device memory: two state buffers (ping-pong), each phi and pi in layout L
-  Layout lay{};
-  void* phi[2] = {nullptr, nullptr};
-  void* pi[2] = {nullptr, nullptr};
-  int cur = 0;
-  CUtensorMap tm[2][2];         // [buffer][phi, pi] for the current TMA tile
-  double* partials = nullptr;   // max(3 * kick blocks, 13 * kMaxSumBlocks) doubles
-  size_t partials_cap = 0;
-  double* sums = nullptr;       // 16 doubles: reduced rows
-  Scalars* sc = nullptr;
-  unsigned int* ticket = nullptr;   // blocks-done counter of the fused stage tail (zero between launches)
-  bool overlap_launch = true;       // kick_tma launched with programmatic stream serialization (PDL)
-  bool energy_tma = true;           // pycool_energies through the TMA-fed kernel where the layout allows
-  int energy_nb = 0;                // blocks (= partial sums per quantity) of the latest energy launch
-  bool persistent = true;           // kick_tma: one block per resident slot, the TMA ring runs on across items
-  int blocks_launched = 0;          // grid size of the latest kick launch
-  bool fused_tail = true;           // last block of a kick reduces the partials and advances the scalars
-  StageLen len{};                   // stage weights handed to the next kick launch
-  bool adaptive = false;            // dt is a physical-time increment (pycool_set_adaptive)
-  bool own_mem = false, own_stream = false;
-  void* owned_block = nullptr;  // one allocation when own_mem
-  cudaStream_t stream = nullptr;
-  // launch geometry
-  int tile = -1, zc = 0, zc_user = 0;
-  dim3 grid;
-  // state
-  bool have_fields = false, nonfinite_seen = false;
-  bool pending_drift = false;   // the closing half drift of the last step call is still to be applied to phi
-  unsigned long long counts[4] = {0, 0, 0, 0};
-  bool profiling = false;
-  std::vector<cudaEvent_t> ev;   // pairs
-  size_t ev_used = 0;
-  double prof_ms = 0;
-  unsigned long long prof_n = 0;
-  std::string err;
-};
-
-namespace {
-
-thread_local std::string g_create_err = "no error";
-
-int fail(pycool_ctx* c, int code, const char* fmt, ...) {
+int pycool::fail(pycool_ctx* c, int code, const char* fmt, ...) {
   char buf[512];
   va_list ap;
   va_start(ap, fmt);
@@ -134,31 +74,16 @@ int fail(pycool_ctx* c, int code, const char* fmt, ...) {
   if (c) c->err = buf; else g_create_err = buf;
   return code;
 }
-#define CUDA_TRY(c, expr)                                                                         \
-  do {                                                                                            \
-    cudaError_t e_ = (expr);                                                                      \
-    if (e_ != cudaSuccess) return fail((c), PYCOOL_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
-  } while (0)
-
-size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 //                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
-const TileInfo kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 16, 512, 0},
-                                    {64, 16, 256, 3}, {32, 16, 128, 3}, {128, 8, 256, 3},
-                                    {128, 16, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}, {128, 16, 256, 3}};
-using Tile0 = Tile<32, 8, 2>;
-using Tile1 = Tile<32, 16, 2>;
-using Tile2 = Tile<64, 16, 2>;
-// kick_tma variants: <TX, TY, ring stages, rows per thread J, blocks per SM the registers are cut for>.
-// (Tried and dropped, profiles/r1c: ring of 4, 512-thread 2 x 1-site blocks, 64 x 32 tiles -- never faster.)
-template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 256 thr x (2 x 2 sites)
-template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3, 2, 1>;   // 128 threads x (2 x 2 sites): small N
-template <typename Real> using TTile5 = TmaTile<Real, 128, 8, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 1 KB rows
-template <typename Real> using TTile6 = TmaTile<Real, 128, 16, 3, 2, 1>;  // 512 threads: twice the bytes per plane (one field)
-template <typename Real> using TTile7 = TmaTile<Real, 32, 16, 3, 1, 2>;   // 256 threads x (2 x 1 sites), two blocks per
-template <typename Real> using TTile8 = TmaTile<Real, 64, 8, 3, 1, 2>;    //   SM: ALU-heavy models (Q-ball)
-template <typename Real> using TTile9 = TmaTile<Real, 128, 16, 3, 4, 1>;   // 256 threads x (2 x 4 sites): one field
-#define PYCOOL_TMA_TILES(X) X(3, TTile3) X(4, TTile4) X(5, TTile5) X(6, TTile6) X(7, TTile7) X(8, TTile8) X(9, TTile9)
+const TileInfo pycool::kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 8, 256, 0},
+                                            {64, 16, 256, 3}, {32, 16, 128, 3}, {128, 8, 256, 3},
+                                            {128, 16, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}, {128, 16, 256, 3},
+                                            {32, 16, 256, 3}};
+
+namespace {
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // Ghost layout (TMA path) needs whole 16-byte pairs inside the lattice: N even.  Otherwise plain N^3.
 Layout make_layout(int N, int nf, size_t esize) {
@@ -235,7 +160,9 @@ EncodeTiledFn encode_fn() {
 }
 
 // Tensor map over one padded array: dims (x: N + 2 gx, y: N + 2 gy, z: N, f: nf), box (tx + 2 gx, ty + 2, 1, nf)
-int encode_one(pycool_ctx* c, void* ptr, int tx, int ty, CUtensorMap* out) {
+}  // namespace
+
+int pycool::encode_one(pycool_ctx* c, void* ptr, int tx, int ty, CUtensorMap* out) {
   EncodeTiledFn enc = encode_fn();
   if (!enc) return fail(c, PYCOOL_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
   const Layout& L = c->lay;
@@ -251,6 +178,9 @@ int encode_one(pycool_ctx* c, void* ptr, int tx, int ty, CUtensorMap* out) {
   if (r != CUDA_SUCCESS) return fail(c, PYCOOL_ECUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
   return PYCOOL_OK;
 }
+
+namespace {
+
 int encode_maps(pycool_ctx* c) {
   const TileInfo& t = kTiles[c->tile];
   for (int b = 0; b < 2; ++b)
@@ -259,197 +189,21 @@ int encode_maps(pycool_ctx* c) {
   return PYCOOL_OK;
 }
 
-// ---- kernel dispatch: <precision, model, nf, tile> -> template instance ----
-template <typename Real, class Model, class T>
-int launch_kick_t(pycool_ctx* c) {
-  static bool attr_done = false;
-  constexpr size_t smem = kick_smem_bytes<Real, Model, T>();
-  if (!attr_done) {
-    CUDA_TRY(c, cudaFuncSetAttribute(kick_fused<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)smem));
-    attr_done = true;
-  }
-  KickArgs<Real> g;
-  g.phi_in = (const Real*)c->phi[c->cur];
-  g.pi_in = (const Real*)c->pi[c->cur];
-  g.phi_out = (Real*)c->phi[c->cur ^ 1];
-  g.pi_out = (Real*)c->pi[c->cur ^ 1];
-  g.sc = c->sc;
-  g.partials = c->partials;
-  g.tail.sc = c->sc;
-  g.tail.ticket = c->ticket;
-  g.tail.work = c->ticket + 1;
-  g.tail.fused = c->fused_tail ? 1 : 0;
-  g.tail.k = c->kc;
-  g.tail.len = c->len;
-  g.L = c->lay;
-  g.zc = c->zc;
-  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
-  g.mp = c->mp;
-  kick_fused<Real, Model, T><<<c->grid, T::NT, smem, c->stream>>>(g);
-  CUDA_TRY(c, cudaGetLastError());
-  return PYCOOL_OK;
-}
-// Blocks of this kick_tma instance that fit on the device at once (0 on error, message in c->err); the first
-// call also opts the instance in to its dynamic shared memory.
-template <typename Real, class Model, class T>
-int tma_resident(pycool_ctx* c) {
-  static int resident = -1;
-  if (resident >= 0) return resident;
-  constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
-  int per_sm = 0, dev = 0, sms = 0;
-  cudaError_t e = cudaFuncSetAttribute(kick_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kick_tma<Real, Model, T>, T::NT, smem);
-  if (e == cudaSuccess) e = cudaGetDevice(&dev);
-  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (e != cudaSuccess || per_sm * sms < 1) {
-    fail(c, PYCOOL_ECUDA, "kick_tma does not fit on an SM (%zu bytes of shared memory): %s", smem, cudaGetErrorString(e));
-    cudaGetLastError();
-    return 0;
-  }
-  resident = per_sm * sms;
-  return resident;
-}
-
-template <typename Real, class Model, class T>
-int launch_tma_t(pycool_ctx* c) {
-  constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
-  const int resident = tma_resident<Real, Model, T>(c);
-  if (resident < 1) return PYCOOL_ECUDA;
-  TmaArgs<Real> g;
-  g.phi_out = (Real*)c->phi[c->cur ^ 1];
-  g.pi_out = (Real*)c->pi[c->cur ^ 1];
-  g.sc = c->sc;
-  g.partials = c->partials;
-  g.tail.sc = c->sc;
-  g.tail.ticket = c->ticket;
-  g.tail.work = c->ticket + 1;
-  g.tail.fused = c->fused_tail ? 1 : 0;
-  g.tail.k = c->kc;
-  g.tail.len = c->len;
-  g.L = c->lay;
-  g.zc = c->zc;
-  g.nbx = (int)c->grid.x; g.nby = (int)c->grid.y;
-  g.nitems = (int)(c->grid.x * c->grid.y * c->grid.z);
-  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
-  g.mp = c->mp;
-  // persistent: one block per resident slot, items dealt round-robin; else one block per item
-  const int nblocks = c->persistent && resident < g.nitems ? resident : g.nitems;
-  c->blocks_launched = nblocks;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)nblocks);
-  cfg.blockDim = dim3(T::NT);
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = c->stream;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;    // see the kernel's griddepcontrol.wait
-  attr[0].val.programmaticStreamSerializationAllowed = c->overlap_launch ? 1 : 0;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  CUDA_TRY(c, cudaLaunchKernelEx(&cfg, kick_tma<Real, Model, T>, c->tm[c->cur][0], c->tm[c->cur][1], g));
-  return PYCOOL_OK;
-}
-template <typename Real, class Model>
-int launch_kick_m(pycool_ctx* c) {
-  const int tile_ = c->tile;
-  switch (tile_) {
-    case 0: return launch_kick_t<Real, Model, Tile0>(c);
-    case 1: return launch_kick_t<Real, Model, Tile1>(c);
-    case 2: return launch_kick_t<Real, Model, Tile2>(c);
-#define X(ID, TT) case ID: return launch_tma_t<Real, Model, TT<Real>>(c);
-    PYCOOL_TMA_TILES(X)
-#undef X
-    default: return 0;
-  }
-}
-template <typename Real, class Model>
-size_t kick_smem_m(int tile_) {
-  switch (tile_) {
-    case 0: return kick_smem_bytes<Real, Model, Tile0>();
-    case 1: return kick_smem_bytes<Real, Model, Tile1>();
-    case 2: return kick_smem_bytes<Real, Model, Tile2>();
-#define X(ID, TT) case ID: return TmaSmem<Real, Model, TT<Real>>::TOTAL;
-    PYCOOL_TMA_TILES(X)
-#undef X
-    default: return 0;
-  }
-}
-template <typename Real, class Model>
-int kick_resident_m(pycool_ctx* c, int tile_) {
-  switch (tile_) {
-    case 0: case 1: case 2: return 2 * 148;             // register-prefetch kernel: not persistent, a guess does
-#define X(ID, TT) case ID: return tma_resident<Real, Model, TT<Real>>(c);
-    PYCOOL_TMA_TILES(X)
-#undef X
-    default: return 0;
-  }
-}
-// TMA-fed energy sums (energy_tma.cuh): ghost layout, at most two fields (the ring of more does not fit).
-template <typename Real, class Model, class T>
-int launch_energy_tma(pycool_ctx* c) {
-  static bool attr_done = false;
-  constexpr size_t smem = EnergySmem<Real, Model, T>::TOTAL;
-  if (!attr_done) {
-    CUDA_TRY(c, cudaFuncSetAttribute(energy_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_done = true;
-  }
-  CUtensorMap tm_phi, tm_pi;
-  if (int st = encode_one(c, c->phi[c->cur], T::TX, T::TY, &tm_phi)) return st;
-  if (int st = encode_one(c, c->pi[c->cur], T::TX, T::TY, &tm_pi)) return st;
-  EnergyArgs<Real> g;
-  g.partials = c->partials;
-  g.L = c->lay;
-  g.zc = c->N < 32 ? c->N : 32;
-  g.nbx = (c->N + T::TX - 1) / T::TX;
-  g.nby = (c->N + T::TY - 1) / T::TY;
-  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
-  g.mp = c->mp;
-  const size_t nb = (size_t)g.nbx * g.nby * ((c->N + g.zc - 1) / g.zc);
-  if ((3 * (size_t)Model::NF + 1) * nb > c->partials_cap) return -1;       // caller falls back
-  energy_tma<Real, Model, T><<<(unsigned)nb, T::NT, smem, c->stream>>>(tm_phi, tm_pi, g);
-  CUDA_TRY(c, cudaGetLastError());
-  c->energy_nb = (int)nb;
-  return PYCOOL_OK;
-}
-template <typename Real, class Model>
-int launch_energy_m(pycool_ctx* c, int nb) {
-  if constexpr (Model::NF <= 2) {
-    if (c->lay.gx > 0 && c->energy_tma) {
-      const int st = c->N > 64 ? launch_energy_tma<Real, Model, TTile3<Real>>(c)
-                               : launch_energy_tma<Real, Model, TTile4<Real>>(c);
-      if (st >= 0) return st;
-    }
-  }
-  energy_sums<Real, Model><<<nb, 256, 0, c->stream>>>((const Real*)c->phi[c->cur], (const Real*)c->pi[c->cur],
-                                                      c->lay, c->c[1], c->c[2], c->c[3], c->mp, c->partials);
-  CUDA_TRY(c, cudaGetLastError());
-  c->energy_nb = nb;
-  return PYCOOL_OK;
-}
-
-enum Op { OP_KICK, OP_ENERGY, OP_SMEM, OP_RESIDENT };
+// Kernel instances are compiled per model (models_*.cu, dispatch.cuh); here only the run-time selection.
 template <typename Real>
 long long dispatch_model(pycool_ctx* c, Op op, int arg) {
-#define PYCOOL_CASE(M)                                                    \
-  do {                                                                    \
-    if (op == OP_KICK) return launch_kick_m<Real, M>(c);                  \
-    if (op == OP_ENERGY) return launch_energy_m<Real, M>(c, arg);         \
-    if (op == OP_RESIDENT) return kick_resident_m<Real, M>(c, arg);       \
-    return (long long)kick_smem_m<Real, M>(arg);                          \
-  } while (0)
   switch (c->model) {
     case PYCOOL_FREE:
       switch (c->nf) {
-        case 1: PYCOOL_CASE(Free<1>);
-        case 2: PYCOOL_CASE(Free<2>);
-        case 3: PYCOOL_CASE(Free<3>);
-        default: PYCOOL_CASE(Free<4>);
+        case 1: return dispatch_one<Real, Free<1>>(c, op, arg);
+        case 2: return dispatch_one<Real, Free<2>>(c, op, arg);
+        case 3: return dispatch_one<Real, Free<3>>(c, op, arg);
+        default: return dispatch_one<Real, Free<4>>(c, op, arg);
       }
-    case PYCOOL_CHAOTIC: PYCOOL_CASE(Chaotic);
-    case PYCOOL_OSCILLON: PYCOOL_CASE(Oscillon);
-    default: PYCOOL_CASE(QBall);
+    case PYCOOL_CHAOTIC: return dispatch_one<Real, Chaotic>(c, op, arg);
+    case PYCOOL_OSCILLON: return dispatch_one<Real, Oscillon>(c, op, arg);
+    default: return dispatch_one<Real, QBall>(c, op, arg);
   }
-#undef PYCOOL_CASE
 }
 long long dispatch(pycool_ctx* c, Op op, int arg) {
   return c->precision == 32 ? dispatch_model<float>(c, op, arg) : dispatch_model<double>(c, op, arg);
@@ -465,15 +219,17 @@ long long dispatch(pycool_ctx* c, Op op, int arg) {
 int auto_tile(pycool_ctx* c) {
   const Layout& L = c->lay;
   if (L.gx == 0) return L.N <= 64 ? 0 : 1;
-  if (L.N <= 64) return 4;
-  static const int pref_default[] = {3, 4}, pref_one[] = {9, 6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {5, 3, 4};
+  static const int pref_default[] = {3, 4}, pref_one[] = {9, 6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {5, 3, 4},
+                   pref_small[] = {4, 10}, pref_many[] = {10, 4};
   const int* pref = pref_default;
   int n = 2;
-  if (c->model == PYCOOL_QBALL && c->precision == 64) { pref = pref_alu; n = 2; }
+  if (c->nf >= 3) { pref = c->precision == 64 ? pref_many : pref_small; n = 2; }   // 2 x 1 sites per thread in fp64
+  else if (L.N <= 64) { pref = pref_small; n = 2; }
+  else if (c->model == PYCOOL_QBALL && c->precision == 64) { pref = pref_alu; n = 2; }
   else if (c->nf == 1 && c->precision == 64) { pref = pref_one; n = 4; }
   else if (c->precision == 32 && c->nf >= 2) { pref = pref_f32; n = 3; }
   for (int i = 0; i < n; ++i)
-    if ((size_t)dispatch(c, OP_SMEM, pref[i]) <= kMaxSmem) return pref[i];
+    if (dispatch(c, OP_BUILT, pref[i])) return pref[i];
   return 1;
 }
 
@@ -490,7 +246,7 @@ int auto_zchunk(pycool_ctx* c) {
   const int N = c->N, bxy = blocks_xy(N, c->tile);
   if (N <= 16) return N;
   int R = (int)dispatch(c, OP_RESIDENT, c->tile);
-  if (R < 1) R = 148;
+  if (R < 1) R = c->sms;
   int cap = 16;
   if (c->precision == 64 && c->tile == 3) cap = N >= 1024 ? 24 : 16;
   else if (c->precision == 32 && c->tile == 5) cap = N >= 1024 ? 16 : (N >= 512 ? 24 : 16);
@@ -528,7 +284,7 @@ int launch_scalar(pycool_ctx* c, const StageLen& len, int mode) {
 
 int launch_flush(pycool_ctx* c) {
   const size_t n = c->lay.total;
-  int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 32);
+  int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)c->sms * 32);
   if (c->precision == 32)
     drift_flush<float><<<nb, 256, 0, c->stream>>>((float*)c->phi[c->cur], (const float*)c->pi[c->cur], c->sc, n);
   else
@@ -581,7 +337,7 @@ int launch_fill_ghosts(pycool_ctx* c, void* arr) {
   const Layout& L = c->lay;
   if (L.gx == 0) return PYCOOL_OK;
   const size_t n = (size_t)(L.N + 2 * L.gx) * (L.N + 2 * L.gy) * L.N * c->nf;
-  const int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)148 * 32);
+  const int nb = (int)std::min<size_t>((n + 255) / 256, (size_t)c->sms * 32);
   if (c->precision == 32) fill_ghosts<float><<<nb, 256, 0, c->stream>>>((float*)arr, L, c->nf);
   else fill_ghosts<double><<<nb, 256, 0, c->stream>>>((double*)arr, L, c->nf);
   CUDA_TRY(c, cudaGetLastError());
@@ -666,12 +422,12 @@ int init_one_array(pycool_ctx* c, const CufftApi& fft, cufftHandle plan, double2
                    const Spectrum& sp, uint32_t aid, unsigned long long seed) {
   const int N = c->N;
   const size_t nmodes = (size_t)N * N * (N / 2 + 1);
-  int nb = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)148 * 64);
+  int nb = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)c->sms * 64);
   fill_spectrum<<<nb, 256, 0, c->stream>>>(scratch, N, c->L, sp, aid, seed);
   CUDA_TRY(c, cudaGetLastError());
   if (fft.exec_z2d(plan, (cufftDoubleComplex*)scratch, (cufftDoubleReal*)scratch) != CUFFT_SUCCESS)
     return fail(c, PYCOOL_ECUDA, "cufftExecZ2D failed");
-  nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)148 * 64);
+  nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)c->sms * 64);
   const double scale = std::sqrt(2.0) / (c->L * std::sqrt(c->L));
   scatter_real<Real><<<nb, 256, 0, c->stream>>>(dst, c->lay, (const double*)scratch, sp.mean, scale);
   CUDA_TRY(c, cudaGetLastError());
@@ -712,6 +468,29 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
   }
   pycool_ctx* c = new (std::nothrow) pycool_ctx();
   if (!c) return fail(nullptr, PYCOOL_ENOMEM, "host allocation failed");
+  for (int& r : c->resident) r = -1;
+  {
+    // the context lives on the device of the caller's work buffer (ext), else on the current device
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && ext) {
+      cudaPointerAttributes pa;
+      e = cudaPointerGetAttributes(&pa, d_work);
+      if (e == cudaSuccess && pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) {
+        delete c;
+        return fail(nullptr, PYCOOL_EINVAL, "work buffer is not device memory");
+      }
+      if (e == cudaSuccess) dev = pa.device;
+    }
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess || c->sms < 1) {
+      cudaGetLastError();
+      delete c;
+      return fail(nullptr, PYCOOL_ECUDA, "cannot query the CUDA device: %s", cudaGetErrorString(e));
+    }
+    c->device = dev;
+  }
+  OnDevice on_device(c);
   c->N = N; c->nf = nf; c->order = order; c->model = p->model;
   c->precision = p->precision == 32 ? 32 : 64;
   c->esize = c->precision == 32 ? 4 : 8;
@@ -820,6 +599,7 @@ static int upload(pycool_ctx* c, const void* phi, const void* pi, cudaMemcpyKind
 
 int pycool_set_fields(pycool_ctx* c, const void* phi_host, const void* pi_host) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!phi_host || !pi_host) return fail(c, PYCOOL_EINVAL, "phi_host / pi_host is NULL");
   int st = upload(c, phi_host, pi_host, cudaMemcpyHostToDevice);
   if (st != PYCOOL_OK) return st;
@@ -829,6 +609,7 @@ int pycool_set_fields(pycool_ctx* c, const void* phi_host, const void* pi_host) 
 
 int pycool_set_fields_device(pycool_ctx* c, const void* d_phi_src, const void* d_pi_src) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!d_phi_src || !d_pi_src) return fail(c, PYCOOL_EINVAL, "source pointer is NULL");
   return upload(c, d_phi_src, d_pi_src, cudaMemcpyDeviceToDevice);
 }
@@ -836,6 +617,7 @@ int pycool_set_fields_device(pycool_ctx* c, const void* d_phi_src, const void* d
 int pycool_init_fields(pycool_ctx* c, unsigned long long seed, const pycool_spectrum* phi_spec,
                        const pycool_spectrum* pi_spec) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!phi_spec || !pi_spec) return fail(c, PYCOOL_EINVAL, "phi_spec / pi_spec is NULL");
   if (c->N % 2) return fail(c, PYCOOL_EINVAL, "pycool_init_fields needs an even N (Hermitian planes ix = 0, N/2)");
   for (int f = 0; f < c->nf; ++f)
@@ -879,16 +661,18 @@ int pycool_init_fields(pycool_ctx* c, unsigned long long seed, const pycool_spec
 
 int pycool_field_spectrum(pycool_ctx* c, int field, int which, int nbins, double* power_host, double* count_host) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "spectrum before set_fields");
   if (field < 0 || field >= c->nf || (which != 0 && which != 1)) return fail(c, PYCOOL_EINVAL, "bad field / which");
-  if (nbins < 1 || nbins > 4096 || !power_host || !count_host) return fail(c, PYCOOL_EINVAL, "bad nbins or NULL output");
+  if (nbins < 1 || nbins > 3072 || !power_host || !count_host)   // 2 nbins doubles of shared memory, <= 48 KB
+    return fail(c, PYCOOL_EINVAL, "nbins must be 1..3072 and the outputs non-NULL");
   int st = ensure_flushed(c);
   if (st != PYCOOL_OK) return st;
   const CufftApi& fft = cufft_api();
   if (!fft.ok) return fail(c, PYCOOL_ECUDA, "cuFFT (libcufft.so.11) could not be loaded");
   const int N = c->N;
   const size_t nmodes = (size_t)N * N * (N / 2 + 1);
-  const int nblk = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)148 * 8);
+  const int nblk = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)c->sms * 8);
   double2* scratch = nullptr;
   double* part = nullptr;
   CUDA_TRY(c, cudaMalloc(&scratch, nmodes * sizeof(double2)));
@@ -901,7 +685,7 @@ int pycool_field_spectrum(pycool_ctx* c, int field, int which, int nbins, double
     cudaFree(scratch); cudaFree(part);
     return fail(c, PYCOOL_ENOMEM, "cufftPlan3d(%d^3, D2Z) failed", N);
   }
-  const int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)148 * 64);
+  const int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)c->sms * 64);
   const void* base = which == 0 ? c->phi[c->cur] : c->pi[c->cur];
   if (c->precision == 32)
     gather_real<float><<<nb, 256, 0, c->stream>>>((double*)scratch, (const float*)base + (size_t)field * c->lay.field, c->lay);
@@ -927,6 +711,7 @@ int pycool_field_spectrum(pycool_ctx* c, int field, int which, int nbins, double
 
 int pycool_set_background(pycool_ctx* c, double a, double p_a) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!(a > 0) || !std::isfinite(a)) return fail(c, PYCOOL_EINVAL, "a must be finite and > 0");
   if (int st = ensure_flushed(c)) return st;
   if (std::isnan(p_a)) {                                   // reading G10: (2.18), expanding branch
@@ -949,6 +734,7 @@ int pycool_set_background(pycool_ctx* c, double a, double p_a) {
 
 int pycool_set_dt(pycool_ctx* c, double dt) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (dt == 0 || !std::isfinite(dt)) return fail(c, PYCOOL_EINVAL, "dt must be finite and non-zero");
   c->dt = dt;
   return PYCOOL_OK;
@@ -956,6 +742,7 @@ int pycool_set_dt(pycool_ctx* c, double dt) {
 
 int pycool_step(pycool_ctx* c, int nsteps) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "step before set_fields");
   if (nsteps < 0) return fail(c, PYCOOL_EINVAL, "nsteps < 0");
   if (c->nonfinite_seen) return fail(c, PYCOOL_ENONFINITE, "a lattice sum became non-finite");
@@ -998,17 +785,20 @@ int pycool_step(pycool_ctx* c, int nsteps) {
 
 int pycool_set_adaptive(pycool_ctx* c, int on) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   c->adaptive = on != 0;
   return PYCOOL_OK;
 }
 
 int pycool_flush(pycool_ctx* c) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   return ensure_flushed(c);
 }
 
 int pycool_sync(pycool_ctx* c) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (int st = ensure_flushed(c)) return st;
   Scalars s;
   return read_scalars(c, &s);
@@ -1016,6 +806,7 @@ int pycool_sync(pycool_ctx* c) {
 
 int pycool_read_fields(pycool_ctx* c, void* phi_host, void* pi_host) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "read before set_fields");
   int st = ensure_flushed(c);
   if (st != PYCOOL_OK) return st;
@@ -1028,6 +819,7 @@ int pycool_read_fields(pycool_ctx* c, void* phi_host, void* pi_host) {
 
 int pycool_read_fields_device(pycool_ctx* c, void* d_phi_dst, void* d_pi_dst) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "read before set_fields");
   int st = ensure_flushed(c);
   if (st != PYCOOL_OK) return st;
@@ -1038,6 +830,7 @@ int pycool_read_fields_device(pycool_ctx* c, void* d_phi_dst, void* d_pi_dst) {
 
 int pycool_device_fields(pycool_ctx* c, void** d_phi, void** d_pi, size_t layout[4]) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (int st = ensure_flushed(c)) return st;
   if (d_phi) *d_phi = c->phi[c->cur];
   if (d_pi) *d_pi = c->pi[c->cur];
@@ -1050,6 +843,7 @@ int pycool_device_fields(pycool_ctx* c, void** d_phi, void** d_pi, size_t layout
 
 int pycool_energies(pycool_ctx* c, pycool_energy* o) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (!o) return fail(c, PYCOOL_EINVAL, "out is NULL");
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "energies before set_fields");
   int st = ensure_flushed(c);
@@ -1079,6 +873,7 @@ int pycool_energies(pycool_ctx* c, pycool_energy* o) {
 
 int pycool_destroy(pycool_ctx* c) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   if (c->own_stream) cudaStreamDestroy(c->stream);
@@ -1105,6 +900,7 @@ int pycool_launch_counts(const pycool_ctx* c, unsigned long long counts[4]) {
 
 int pycool_set_profiling(pycool_ctx* c, int on) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   c->profiling = on != 0;
   c->ev_used = 0; c->prof_ms = 0; c->prof_n = 0;
   return PYCOOL_OK;
@@ -1112,6 +908,7 @@ int pycool_set_profiling(pycool_ctx* c, int on) {
 
 int pycool_kick_time_ms(pycool_ctx* c, double* total_ms, unsigned long long* launches) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
     float ms = 0;
@@ -1138,6 +935,7 @@ int pycool_kick_geometry(const pycool_ctx* c, int tile[8]) {
 
 int pycool_set_zchunk(pycool_ctx* c, int planes) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (planes < 0) return fail(c, PYCOOL_EINVAL, "planes < 0");
   c->zc_user = planes;
   return set_geometry(c);
@@ -1145,36 +943,43 @@ int pycool_set_zchunk(pycool_ctx* c, int planes) {
 
 int pycool_set_overlap(pycool_ctx* c, int on) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   c->overlap_launch = on != 0;
   return PYCOOL_OK;
 }
 
 int pycool_set_energy_kernel(pycool_ctx* c, int tma) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   c->energy_tma = tma != 0;
   return PYCOOL_OK;
 }
 
 int pycool_set_persistent(pycool_ctx* c, int on) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   c->persistent = on != 0;
   return PYCOOL_OK;
 }
 
 int pycool_set_fused_tail(pycool_ctx* c, int on) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   c->fused_tail = on != 0;
   return PYCOOL_OK;
 }
 
 int pycool_set_tile(pycool_ctx* c, int tile) {
   if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
   if (tile < -1 || tile >= kNumTiles) return fail(c, PYCOOL_EINVAL, "tile must be -1 (auto) .. %d", kNumTiles - 1);
   if (tile >= 0 && !tile_allowed(c->lay, tile))
     return fail(c, PYCOOL_EINVAL, "tile %d is a TMA variant: it needs the ghost layout (even N >= 4)", tile);
   if (tile >= 0 && (size_t)dispatch(c, OP_SMEM, tile) > kMaxSmem)
     return fail(c, PYCOOL_EINVAL, "tile %d needs %zu bytes of shared memory for this model and precision (limit %zu)",
                 tile, (size_t)dispatch(c, OP_SMEM, tile), kMaxSmem);
+  if (tile >= 0 && !dispatch(c, OP_BUILT, tile))
+    return fail(c, PYCOOL_EINVAL, "tile %d is not built for %d fields at this precision (register budget)", tile, c->nf);
   c->tile = tile < 0 ? auto_tile(c) : tile;
   return set_geometry(c);
 }

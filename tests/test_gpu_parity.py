@@ -108,10 +108,16 @@ def test_cfg0_paper_phi0_reading_g19(pc):
 # ------------------------------------------------------------------------------------- reduced-size cfg1-3
 # Tolerance after one step: a 1-ulp difference in phi' (merged vs separate half drifts, FMA) enters pi through
 # kD D, i.e. amplified by (|c0| + sum |c_d|) a^2 h/dx^2 ~ 8.5 * 1.35 dt/dx^2 per stage.  For cfg0-cfg2 that factor
-# is < 1 and 1e-12 holds; for the Q-ball lattice dt/dx^2 = 5.1 and |pi_1| ~ 1e-3 |phi_1|, so ulp(phi) 60/rms(pi)
-# ~ 1e-11 is the floor of ANY fp64 evaluation order there.
+# is < 1 and 1e-12 holds.  For the Q-ball lattice dt/dx^2 = 5.1 and |pi_1| ~ 1e-3 |phi_1|: the oracle in double
+# against the oracle in long double differs by 1.7e-12 after ONE step there (measured, -m "not gpu":
+# tests/test_oracle_pins.py::test_fp64_rounding_floor_of_one_step), so 1e-12 is below the floor of any fp64
+# evaluation order.  The GPU's measured error on it is 2.3e-12 after one step (printed by
+# the tests below); the tolerance is 3 x the oracle's own floor.
+QBALL_TOL_1STEP = 5.2e-12
+
+
 @pytest.mark.parametrize("name,N,steps,tol1", [("cfg1_chaotic128", 48, 6, 1e-12), ("cfg2_oscillon256", 40, 20, 1e-12),
-                                               ("cfg3_qball256", 40, 20, 2e-11)])
+                                               ("cfg3_qball256", 40, 20, QBALL_TOL_1STEP)])
 def test_models_reduced_size(pc, name, N, steps, tol1):
     cfg = inputs.config(name, N=N)
     if name == "cfg2_oscillon256":
@@ -122,9 +128,10 @@ def test_models_reduced_size(pc, name, N, steps, tol1):
     g, o = make_pair(pc, cfg)
     start(g, o, phi, pi)
     g.step(1); o.step(1)
-    compare(g, o, cfg["nfields"], tol1)
+    e1 = compare(g, o, cfg["nfields"], tol1)
     g.step(steps - 1); o.step(steps - 1)
-    compare(g, o, cfg["nfields"], 100 * tol1)
+    en = compare(g, o, cfg["nfields"], 100 * tol1)
+    print("%s at N = %d: per-site error %.2e after 1 step, %.2e after %d" % (name, N, e1, en, steps))
 
 
 # ------------------------------------------------------------------------------------- orders, tiles, chunks
@@ -140,16 +147,17 @@ def test_all_orders(pc, order):
 
 
 def set_tile_or_skip(pc, g, tile):
-    """Variants 6 and 9 (128 x 16: twice the bytes per plane) do not fit in shared memory for two fp64 fields: EINVAL."""
+    """Variants 6 and 9 (128 x 16: twice the bytes per plane) do not fit in shared memory for two fp64 fields, and
+    variant 9 (2 x 4 sites per thread) is built for one-field lattices only: EINVAL, with the reason."""
     try:
         g.set_tile(tile)
     except pc.PycoolError as e:
-        assert e.code == pc.EINVAL and tile in (6, 9) and "shared memory" in str(e)
+        assert e.code == pc.EINVAL and tile in (6, 9) and ("shared memory" in str(e) or "not built" in str(e))
         return False
     return True
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10])
 @pytest.mark.parametrize("N,zc", [(40, 0), (40, 7), (40, 40), (67, 16), (3, 0), (4, 1), (5, 2), (33, 32), (6, 0),
                                   (70, 9), (136, 50)])
 def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
@@ -175,6 +183,29 @@ def test_tiles_ragged_edges_and_zchunks(pc, tile, N, zc):
     compare(g, o, 2, 2e-12)
 
 
+@pytest.mark.parametrize("tile", [4, 7, 8, 10])
+@pytest.mark.parametrize("N,zc", [(70, 9), (136, 50), (40, 0)])
+def test_qball_variants_ragged_edges_and_zchunks(pc, tile, N, zc):
+    """The Q-ball model (own logarithm, 2 x 1 sites per thread, two blocks per SM: variants 7 and 8 are its
+    automatic choice above N = 64) on ragged tiles with short and long z-chunks, against the oracle.  Tolerance:
+    the fp64 rounding floor of this lattice is 1.7e-12 per step (tests/test_oracle_pins.py,
+    test_fp64_rounding_floor_of_one_step); the GPU's measured error is in DESIGN.md "Tolerances"."""
+    cfg = inputs.config("cfg3_qball256", N=N)
+    cfg["L"] = 8.0 * N / 256
+    phi, pi = inputs.make_initial(cfg)
+    g, o = make_pair(pc, cfg)
+    g.set_tile(tile); g.set_zchunk(zc)
+    assert g.kick_geometry()["variant"] == tile
+    start(g, o, phi, pi)
+    g.step(1); o.step(1)
+    e1 = compare(g, o, 2, QBALL_TOL_1STEP)
+    g.step(1); o.step(1)
+    e2 = compare(g, o, 2, 2 * QBALL_TOL_1STEP)
+    print("qball tile %d N %d zc %d: per-site error %.2e after 1 step, %.2e after 2" % (tile, N, zc, e1, e2))
+    if N > 64:
+        assert pc.from_config(cfg).kick_geometry()["variant"] == 7
+
+
 @pytest.mark.parametrize("precision", [64, 32])
 def test_variants_agree_and_ghost_images_hold(pc, precision):
     """Every kernel variant from the same state: results agree to rounding, and the ghost columns / rows of the
@@ -184,10 +215,10 @@ def test_variants_agree_and_ghost_images_hold(pc, precision):
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg, precision=precision)
     outs = []
-    for tile in range(10):
+    for tile in range(11):
         g = pc.from_config(cfg, precision=precision)
         if not set_tile_or_skip(pc, g, tile):
-            assert precision == 64
+            assert precision == 64 or tile == 9
             continue
         g.set_fields(phi, pi)
         g.set_background(1.0)
@@ -514,81 +545,102 @@ def test_fp32_one_step(pc, tile):
     check_scalars(g.energies(), o.energies(), 2, tol=1e-5)
 
 
-# ------------------------------------------------------------------------------------- full size, bench config
-@pytest.mark.parametrize("N,base", [(512, 32)])
-def test_full_size_periodic_replication(pc, N, base):
-    """At BASELINE's 512^3 in the launch configuration bench.py times: the input is a base^3 lattice
-    replicated periodically; the method is translation-equivariant, so every output site must equal the
-    oracle's base^3 evolution of the same tile (sums scale with the volume, a is unchanged)."""
-    r = N // base
-    small = inputs.config("cfg4_chaotic512", N=base)
-    small["L"] = 10.0 * base / N                             # same dx and dt as the 512^3 configuration
-    small["dt"] = 10.0 / N / 20.0
-    phi_s, pi_s = inputs.make_initial(small)
-    big = inputs.config("cfg4_chaotic512", N=N)
-    g = pc.from_config(big)
-    o = oracle.Oracle(base, small["L"], 2, oracle.CHAOTIC, small["p"], order=4, dt=small["dt"], mpl=1.0)
-    g.set_fields(np.tile(phi_s, (1, r, r, r)), np.tile(pi_s, (1, r, r, r)))
-    g.set_background(1.0)
-    o.set_fields(phi_s, pi_s)
-    o.set_background(1.0)
-    g.step(2); o.step(2)
-    po, qo = o.read_fields()
-    pg, qg = g.read_fields()
-    eg, eo = g.energies(), o.energies()
-    assert rel(eg.a, eo.a) < 1e-12 and rel(eg.p_a / r ** 3, eo.p_a) < 1e-12
-    assert rel(eg.kin[0], eo.kin[0]) < 1e-10 and rel(eg.grad[1], eo.grad[1]) < 1e-10 and rel(eg.pot, eo.pot) < 1e-10
-    for arr_g, arr_o in ((pg, po), (qg, qo)):
-        worst = 0.0
-        for f in range(2):
-            rms = math.sqrt(float(np.mean(arr_o[f] ** 2)))
-            den = np.maximum(np.abs(arr_o[f]), rms)
-            blocks = arr_g[f].reshape(r, base, r, base, r, base)
-            for iz in range(r):                              # every replica, every site
-                d = np.abs(blocks[iz] - arr_o[f][:, None, :, None, :]) / den[:, None, :, None, :]
-                worst = max(worst, float(d.max()))
-        assert worst <= 2e-12, worst
-
-
-def test_largest_lattice_1024_cubed_fp32_on_device(pc):
-    """1024^3 x 2 fields = 2^31 elements per array (the largest lattice one B200 holds in fp64 too): 64-bit offsets,
-    32768 work items, 1028-element rows.  fp32 keeps it to 34 GB of state; input and comparison stay on the device
-    (set_fields_device / read_fields_device).  Same replication argument as above against the oracle's 32^3."""
+# ------------------------------------------------------------------------------------- full size, bench configs
+def replicate_on_device(arr, r, dev):
     import torch
-    N, base = 1024, 32
+    return torch.from_numpy(arr).to(dev).repeat(1, r, r, r).contiguous()
+
+
+def worst_replica_error(big, small_np, r, base, dev):
+    """max over every replica and every site of |big - small| / max(|small|, rms(small)) (reading G18), on the device."""
+    import torch
+    worst = 0.0
+    for f in range(small_np.shape[0]):
+        want = torch.from_numpy(small_np[f]).to(dev)
+        rms = float(want.double().pow(2).mean().sqrt())
+        den = torch.clamp(want.abs(), min=rms)
+        blocks = big[f].view(r, base, r, base, r, base)
+        for iz in range(r):
+            d = (blocks[iz] - want[:, None, :, None, :]).abs() / den[:, None, :, None, :]
+            worst = max(worst, float(d.max()))
+    return worst
+
+
+# (workload, N, base, order, precision, per-site tolerance after `steps` steps, steps, kernel variant expected)
+FULL_SIZE = [
+    ("cfg4_chaotic512", 512, 32, 4, 64, 2e-12, 2, 3),       # the bench default
+    ("cfg4_chaotic512", 512, 32, 6, 64, 4e-12, 1, 3),
+    ("cfg4_chaotic512", 512, 32, 4, 32, 1e-5, 1, 5),
+    ("cfg1_chaotic128", 128, 32, 6, 64, 2e-12, 2, 3),       # configs[1]: order 6 at its own size
+    ("cfg2_oscillon256", 256, 32, 4, 64, 2e-12, 2, 9),      # configs[2]: one field, 2 x 4 sites per thread
+    ("cfg3_qball256", 256, 32, 4, 64, 2 * QBALL_TOL_1STEP, 2, 7),   # configs[3]: QBall x (2 x 1 sites, 2 blocks/SM)
+    ("cfg4_chaotic1024", 1024, 32, 4, 64, 2e-12, 1, 3),     # configs[4]: 69 GB of state, byte offsets > 2^34
+    ("cfg4_chaotic1024", 1024, 32, 4, 32, 1e-5, 1, 5),      # 2^31 elements per array
+]
+
+
+@pytest.mark.parametrize("name,N,base,order,precision,tol,steps,variant", FULL_SIZE)
+def test_full_size_periodic_replication(pc, name, N, base, order, precision, tol, steps, variant):
+    """Every configuration BASELINE.md's table quotes, at its full size and in the automatic launch geometry that
+    bench.py times: the input is a base^3 lattice replicated periodically; the method is translation-equivariant,
+    so every output site of every replica must equal the oracle's base^3 evolution of the same tile (lattice sums
+    scale with the volume, a is unchanged).  Input, output and comparison stay on the device
+    (set_fields_device / read_fields_device): 1024^3 x 2 fp64 is 17 GB per array."""
+    import torch
     r = N // base
-    small = inputs.config("cfg4_chaotic1024", N=base)
-    small["L"] = 10.0 * base / N
-    small["dt"] = 10.0 / N / 20.0
-    phi_s, pi_s = inputs.make_initial(small, precision=32)
-    big = inputs.config("cfg4_chaotic1024", N=N)
-    g = pc.from_config(big, precision=32)
-    o = oracle.Oracle(base, small["L"], 2, oracle.CHAOTIC, small["p"], order=4, dt=small["dt"], mpl=1.0, precision=32)
+    full = inputs.config(name)
+    small = inputs.config(name, N=base, order=order)
+    small["L"] = full["L"] * base / N                        # same dx and dt as the full configuration
+    small["dt"] = full["dt"]
+    phi_s, pi_s = inputs.make_initial(small, precision=precision)
+    big = inputs.config(name, order=order)
+    g = pc.from_config(big, precision=precision)
+    kw = dict(mpl=small["mpl"], rho_gamma0=small["rho_gamma0"], rho_m0=small["rho_m0"], precision=precision)
+    o = oracle.Oracle(base, small["L"], small["nfields"], small["model"], small["p"], order=order, dt=small["dt"], **kw)
     dev = g.device
-    tp = torch.from_numpy(phi_s).to(dev).repeat(1, r, r, r).contiguous()
-    tq = torch.from_numpy(pi_s).to(dev).repeat(1, r, r, r).contiguous()
-    assert tp.numel() == 2 ** 31
+    tp, tq = replicate_on_device(phi_s, r, dev), replicate_on_device(pi_s, r, dev)
     g.set_fields(tp, tq)
     del tp, tq
-    g.set_background(1.0)
+    torch.cuda.empty_cache()
+    # the radiation background of cfg3 is derived from H0, not from the lattice: set a, p_a explicitly on both
     o.set_fields(phi_s, pi_s)
     o.set_background(1.0)
-    g.step(1); o.step(1)
+    p_a_small = o.energies().p_a
+    g.set_background(1.0, p_a_small * r ** 3)                # p_a is extensive: -6 V_L mpl^2 a'
     geo = g.kick_geometry()
-    assert geo["blocks"] >= 16384 and geo["tma_stages"] > 0
+    assert geo["variant"] == variant and geo["tma_stages"] > 0, geo
+    g.step(steps); o.step(steps)
     po, qo = o.read_fields()
-    pg, qg = g.read_fields_device()
     eg, eo = g.energies(), o.energies()
-    assert rel(eg.a, eo.a) < 1e-6 and rel(eg.p_a / r ** 3, eo.p_a) < 1e-5
-    assert rel(eg.kin[0], eo.kin[0]) < 1e-5 and rel(eg.grad[1], eo.grad[1]) < 1e-4 and rel(eg.pot, eo.pot) < 1e-5
-    for arr_g, arr_o in ((pg, po), (qg, qo)):
-        for f in range(2):
-            want = torch.from_numpy(arr_o[f]).to(dev)
-            rms = float(want.double().pow(2).mean().sqrt())
-            den = torch.clamp(want.abs(), min=rms)
-            blocks = arr_g[f].view(r, base, r, base, r, base)
-            worst = 0.0
-            for iz in range(r):                              # every replica, every site
-                d = (blocks[iz] - want[:, None, :, None, :]).abs() / den[:, None, :, None, :]
-                worst = max(worst, float(d.max()))
-            assert worst <= 1e-5, (f, worst)
+    ts = 1e-10 if precision == 64 else 1e-4
+    nf = small["nfields"]
+    assert rel(eg.a, eo.a) < (1e-12 if precision == 64 else 1e-6) and rel(eg.p_a / r ** 3, eo.p_a) < ts
+    assert rel(eg.kin[0], eo.kin[0]) < ts and rel(eg.grad[nf - 1], eo.grad[nf - 1]) < 10 * ts and rel(eg.pot, eo.pot) < ts
+    pg, qg = g.read_fields_device()
+    e_phi = worst_replica_error(pg, po, r, base, dev)
+    del pg
+    e_pi = worst_replica_error(qg, qo, r, base, dev)
+    print("%s %d^3 order %d fp%d variant %d zc %d: per-site error phi %.2e pi %.2e after %d step(s)"
+          % (name, N, order, precision, geo["variant"], geo["zchunk"], e_phi, e_pi, steps))
+    assert e_phi <= tol and e_pi <= tol, (e_phi, e_pi)
+
+
+def test_context_on_a_second_device(pc):
+    """A Lattice made while ANOTHER device is current, and two Lattices on two GPUs driven from one thread: the
+    library records the device of the work buffer and switches to it for every call (shared-memory opt-in and
+    occupancy are per context, not per process).  Needs two GPUs."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    cfg = inputs.config("cfg0_chaotic32", N=72, dt=0.002)
+    phi, pi = inputs.make_initial(cfg)
+    torch.cuda.set_device(0)
+    a = pc.from_config(cfg, device="cuda:0")
+    b = pc.from_config(cfg, device="cuda:1")                 # made while cuda:0 is current
+    outs = []
+    for g in (a, b):
+        g.set_fields(phi, pi); g.set_background(1.0)
+        g.step(2)
+        outs.append(g.read_fields())
+    assert torch.cuda.current_device() == 0
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
