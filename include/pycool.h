@@ -136,6 +136,21 @@ int pycool_init_fields(pycool_ctx*, unsigned long long seed, const pycool_spectr
  * reproducible from run to run.  Applies a pending closing drift first.  Synchronises. */
 int pycool_field_spectrum(pycool_ctx*, int field, int which, int nbins, double* power_host, double* count_host);
 
+/* Number-density and energy-density spectra of one field (the paper's post-processing writes
+ * "field, number density and energy density spectra that are used in LATTICEEASY", and defines none of
+ * them: reading G24).  They are the spectra of the DISCRETE Hamiltonian (2.20) that the step integrates: with
+ * F^phi_k, F^pi_k as in pycool_field_spectrum, the canonical pair u_k = a F^phi_k, v_k = F^pi_k / a and
+ *     w_k^2 = k_eff^2(n) / dx^2 + a^2 m_eff2,   -k_eff^2 = eigenvalue of the stencil (2.7) on the mode,
+ *     n_k   = 1/2 (w_k |u_k|^2 + |v_k|^2 / w_k)     (0 where w_k^2 <= 0),      rho_k = 1/2 (|v_k|^2 + w_k^2 |u_k|^2),
+ * number[i], energy[i], count[i] = sums over the modes of the full spectrum with round(|n|) = i, i < nbins <= 2048.
+ * Then (2 / (a^4 L^3)) sum_i energy[i] = kin[f] + grad[f] + 1/2 m_eff2 <phi_f^2> of pycool_energies exactly
+ * (Parseval), and a vacuum state made by pycool_init_fields (|phi_k|^2 = 1/(2 w_k)) has number/count = 1/2.
+ * a is the current (time-synchronised) scale factor; m_eff2 is the caller's effective mass squared of the field
+ * (e.g. d^2V/dphi^2 at the mean field).  Two cuFFT D2Z transforms; applies a pending closing drift first.
+ * Synchronises. */
+int pycool_mode_spectra(pycool_ctx*, int field, double m_eff2, int nbins, double* number_host, double* energy_host,
+                        double* count_host);
+
 /* Set a (> 0) and p_a.  p_a = NaN asks the library to solve the first Friedmann equation (2.18) on the
  * current lattice, expanding branch (reading G10): p_a = -6 V_L mpl a^2 sqrt(rho/3); needs fields and a
  * finite mpl.  With mpl = +INF pass p_a = 0. */
@@ -181,6 +196,19 @@ int pycool_device_fields(pycool_ctx*, void** d_phi, void** d_pi, size_t layout[4
  * Synchronises. */
 int pycool_energies(pycool_ctx*, pycool_energy* out);
 
+/* Energy log: "How frequently to calculate the energy densities and to write them to a file is decided by the
+ * user".  every > 0: after every `every`-th completed step (counted from this call) pycool_step
+ * enqueues an energy read-out of the state that step ends in -- the lattice sums seen through the step's closing
+ * half drift, at the scale factor of that instant, finished on the device (rho, P, H, residual) -- and appends it
+ * to a device ring buffer of `capacity` entries.  No host synchronisation, and the step sequence itself is
+ * untouched: fields and scalars are bitwise those of an unlogged run, and every entry is bitwise what
+ * pycool_energies returns for a run stopped at that step.  every = 0 switches the log off and frees it.
+ * pycool_read_energy_log copies the newest min(logged, capacity, max_entries) entries, oldest first, to host memory
+ * (*n_out of them; *total, if not NULL, = entries logged since the cadence was set).  Synchronises. */
+int pycool_set_energy_cadence(pycool_ctx*, int every, int capacity);
+int pycool_read_energy_log(pycool_ctx*, pycool_energy* out_host, int max_entries, int* n_out,
+                           unsigned long long* total);
+
 int pycool_destroy(pycool_ctx*);
 
 /* Library-owned, NUL-terminated description of the last error of this context (valid until the next call
@@ -216,9 +244,11 @@ int pycool_set_fused_tail(pycool_ctx*, int on);
  * the current stage drains and wait (griddepcontrol.wait) until it has completed before they read anything it
  * wrote.  Hides launch latency and prologue on small lattices; results are unchanged. */
 int pycool_set_overlap(pycool_ctx*, int on);
-/* pycool_energies kernel: 1 (default) = TMA-fed z-march (even N, at most two fields; G from the identity
- * 2 G[psi] = D[psi^2] - 2 psi D[psi]); 0 = the plain one-thread-per-site kernel that evaluates (2.8) term by term
- * (always used for odd N or more than two fields).  They agree to rounding. */
+/* pycool_energies kernel: 1 (default) = TMA-fed z-march (even N, at most two fields; sum_x G[phi] through the paper's
+ * identity (2.17), sum_x G = -sum_x psi D[psi] with psi = phi - one lattice-wide reference value per field);
+ * 0 = the plain one-thread-per-site kernel that evaluates (2.8) term by term (always used for odd N or more than two
+ * fields).  They agree to rounding.  2, 3, 4 pick the TMA kernel's tile (64x16 with 2x2 sites per thread; 32x16 with
+ * 2x1 sites and two blocks per SM; 32x16 with 2x2 sites) instead of the automatic choice. */
 int pycool_set_energy_kernel(pycool_ctx*, int tma);
 /* Persistent launch of the TMA-fed kernel (default on): as many blocks as fit on the device at once; a block's
  * first work item (x-y tile, z-chunk) is its index, every further one is claimed from a device counter

@@ -23,7 +23,7 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
            "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_init_fields",
-           "pycool_field_spectrum")
+           "pycool_field_spectrum", "pycool_mode_spectra", "pycool_set_energy_cadence", "pycool_read_energy_log")
 
 
 class Params(C.Structure):
@@ -101,6 +101,9 @@ def lib():
         L.pycool_set_overlap.argtypes = [vp, ip]
         L.pycool_field_spectrum.argtypes = [vp, ip, ip, ip, C.POINTER(d), C.POINTER(d)]
         L.pycool_init_fields.argtypes = [vp, C.c_ulonglong, C.POINTER(Spectrum), C.POINTER(Spectrum)]
+        L.pycool_mode_spectra.argtypes = [vp, ip, d, ip, C.POINTER(d), C.POINTER(d), C.POINTER(d)]
+        L.pycool_set_energy_cadence.argtypes = [vp, ip, ip]
+        L.pycool_read_energy_log.argtypes = [vp, C.POINTER(Energy), ip, C.POINTER(ip), C.POINTER(C.c_ulonglong)]
         _lib = L
     return _lib
 
@@ -214,6 +217,26 @@ class Lattice:
         p, c = (C.c_double * nbins)(), (C.c_double * nbins)()
         self._chk(lib().pycool_field_spectrum(self._h, field, which, nbins, p, c))
         return np.array(p[:]), np.array(c[:])
+
+    def mode_spectra(self, field, m_eff2, nbins=None):
+        """(number, energy, count) per shell round(|n|) of one field; see pycool_mode_spectra (reading G24)."""
+        nbins = nbins or int(math.floor(math.sqrt(3.0) * self.N / 2.0 + 0.5)) + 1
+        n, e, c = (C.c_double * nbins)(), (C.c_double * nbins)(), (C.c_double * nbins)()
+        self._chk(lib().pycool_mode_spectra(self._h, field, float(m_eff2), nbins, n, e, c))
+        return np.array(n[:]), np.array(e[:]), np.array(c[:])
+
+    def set_energy_cadence(self, every, capacity=1024):
+        """Log the energies on the device after every `every`-th step (0: off); see pycool_set_energy_cadence."""
+        self._chk(lib().pycool_set_energy_cadence(self._h, int(every), int(capacity)))
+
+    def read_energy_log(self, max_entries=1 << 20):
+        """(list of Energy, oldest first; total number logged since the cadence was set)."""
+        n, total = C.c_int(), C.c_ulonglong()
+        self._chk(lib().pycool_read_energy_log(self._h, None, 0, C.byref(n), C.byref(total)))
+        have = min(int(total.value), max_entries)
+        buf = (Energy * max(have, 1))()
+        self._chk(lib().pycool_read_energy_log(self._h, buf, have, C.byref(n), C.byref(total)))
+        return [buf[i] for i in range(n.value)], int(total.value)
 
     def set_background(self, a=1.0, p_a=math.nan):
         self._chk(lib().pycool_set_background(self._h, a, p_a))

@@ -46,10 +46,19 @@ struct pycool_ctx {
   double* partials = nullptr;   // max(3 * kick blocks, 13 * kMaxSumBlocks) doubles
   size_t partials_cap = 0;
   double* sums = nullptr;       // 16 doubles: reduced rows
+  pycool_energy* d_energy = nullptr;   // the latest energy read-out, finished on the device (energy_finish)
+  bool energy_through_drift = false;   // the next energy launch sees phi through the pending closing half drift
+  // energy log (pycool_set_energy_cadence): every `log_every` completed steps an energy read-out is appended to a
+  // device ring buffer by kernels enqueued from pycool_step, without a host synchronisation
+  pycool_energy* d_log = nullptr;
+  int log_every = 0, log_cap = 0;
+  unsigned long long log_n = 0;        // entries written since the cadence was set
+  unsigned long long steps_done = 0;   // completed steps since the cadence was set
   pycool::Scalars* sc = nullptr;
   unsigned int* ticket = nullptr;   // blocks-done counter of the fused stage tail (zero between launches)
   bool overlap_launch = true;       // kick_tma launched with programmatic stream serialization (PDL)
-  bool energy_tma = true;           // pycool_energies through the TMA-fed kernel where the layout allows
+  int energy_tma = 1;               // pycool_energies through the TMA-fed kernel where the layout allows (0: plain;
+                                    //   1: automatic variant; 2-4: a given variant, pycool_set_energy_kernel)
   int energy_nb = 0;                // blocks (= partial sums per quantity) of the latest energy launch
   bool persistent = true;           // kick_tma: one block per resident slot, the TMA ring runs on across items
   int blocks_launched = 0;          // grid size of the latest kick launch
@@ -59,7 +68,7 @@ struct pycool_ctx {
   int device = 0, sms = 0;          // the CUDA device this context lives on and its SM count
   int resident[16];                 // blocks of the kick variant that fit on the device at once (-1: not asked yet);
                                     //   asking also opts the instance in to its dynamic shared memory ON THIS DEVICE
-  bool energy_attr[2] = {false, false};
+  bool energy_attr[3] = {false, false, false};
   bool own_mem = false, own_stream = false;
   void* owned_block = nullptr;  // one allocation when own_mem
   cudaStream_t stream = nullptr;

@@ -182,7 +182,7 @@ int kick_resident_m(pycool_ctx* c, int tile_) {
 template <typename Real, class Model, class T>
 int launch_energy_tma(pycool_ctx* c) {
   constexpr size_t smem = EnergySmem<Real, Model, T>::TOTAL;
-  bool& attr_done = c->energy_attr[T::TX == 64 ? 0 : 1];       // per context, i.e. per device
+  bool& attr_done = c->energy_attr[T::TX == 64 ? 0 : (T::J == 1 ? 1 : 2)];   // per context, i.e. per device
   if (!attr_done) {
     CUDA_TRY(c, cudaFuncSetAttribute(energy_tma<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_done = true;
@@ -191,6 +191,9 @@ int launch_energy_tma(pycool_ctx* c) {
   if (int st = encode_one(c, c->phi[c->cur], T::TX, T::TY, &tm_phi)) return st;
   if (int st = encode_one(c, c->pi[c->cur], T::TX, T::TY, &tm_pi)) return st;
   EnergyArgs<Real> g;
+  g.phi = (const Real*)c->phi[c->cur];
+  g.pi = (const Real*)c->pi[c->cur];
+  g.sc = c->energy_through_drift ? c->sc : nullptr;
   g.partials = c->partials;
   g.L = c->lay;
   g.zc = c->N < 32 ? c->N : 32;
@@ -209,13 +212,17 @@ template <typename Real, class Model>
 int launch_energy_m(pycool_ctx* c, int nb) {
   if constexpr (Model::NF <= 2) {
     if (c->lay.gx > 0 && c->energy_tma) {
-      const int st = c->N > 64 ? launch_energy_tma<Real, Model, TTile3<Real>>(c)
-                               : launch_energy_tma<Real, Model, TTile4<Real>>(c);
+      // 32 x 16 tile with 2 x 1 sites per thread, two blocks per SM (16 warps) above N = 64; 2: 64 x 16, 2 x 2 sites
+      const int v = c->energy_tma == 1 ? (c->N > 64 ? 3 : 4) : c->energy_tma;
+      const int st = v == 2 ? launch_energy_tma<Real, Model, TmaTile<Real, 64, 16, 3, 2, 1>>(c)
+                   : v == 3 ? launch_energy_tma<Real, Model, TTile7<Real>>(c)
+                            : launch_energy_tma<Real, Model, TTile4<Real>>(c);
       if (st >= 0) return st;
     }
   }
   energy_sums<Real, Model><<<nb, 256, 0, c->stream>>>((const Real*)c->phi[c->cur], (const Real*)c->pi[c->cur],
-                                                      c->lay, c->c[1], c->c[2], c->c[3], c->mp, c->partials);
+                                                      c->lay, c->c[1], c->c[2], c->c[3], c->mp, c->partials,
+                                                      c->energy_through_drift ? c->sc : nullptr);
   CUDA_TRY(c, cudaGetLastError());
   c->energy_nb = nb;
   return PYCOOL_OK;

@@ -5,14 +5,15 @@
 // (TX + 2G) x (TY + 2) x NF box of phi and of pi per z-plane into a ring of S shared-memory stages, halo included,
 // ghost images making every box a plain in-bounds box), same register queue along z for the 27-point stencil.
 //
-// G[phi](x) = 1/2 sum_alpha c_d(alpha) (phi(alpha) - phi(x))^2 needs the centre value of the OUTPUT site in every
-// term, so it does not decompose plane by plane as written.  Expanding the square and using sum_alpha c_d = 0
-// (c0 = -(6c1 + 12c2 + 8c3), alpha running over all 27 points) gives the identity used here:
-//     2 G[psi](x) = D[psi^2](x) - 2 psi(x) D[psi](x),
-// i.e. the same stencil applied to psi^2, which marches along z with a second pair of accumulators.  psi = phi - ref
-// (ref block-uniform): G and D are invariant under psi -> psi + const, and with psi of the size of the field's
-// variation across the tile neither term cancels against the homogeneous part.  All arithmetic in double, also for
-// fp32 fields (reading G16).
+// The gradient energy needs sum_x G[phi](x), G of (2.8).  G carries the centre value of the OUTPUT site in every term,
+// so it does not decompose plane by plane; but the paper's own identity (2.17),
+//     sum_x G[phi](x) = - sum_x phi(x) D[phi](x)        (summation by parts on the periodic lattice),
+// does, and D annihilates constants (c0 = -(6c1 + 12c2 + 8c3)), so with psi = phi - ref, ref ONE value per field for
+// the whole lattice (the field at site (0,0,0)): sum_x G[phi] = - sum_x psi D[psi], every term of which is of the size
+// of the fluctuations -- no cancellation against the homogeneous part (the plain sum_x phi D[phi], kept as the third
+// sum, loses ~6 digits on a preheating lattice).  One stencil, the kick's register queue, all arithmetic in double
+// also for fp32 fields (reading G16).  The plain kernel (kernels.cuh: energy_sums) evaluates (2.8) term by term; the
+// two agree to rounding (tested).
 #pragma once
 #include "kick_tma.cuh"
 
@@ -20,6 +21,9 @@ namespace pycool {
 
 template <typename Real>
 struct EnergyArgs {
+  const Real* phi;        // the state arrays (for the lattice-wide reference value of each field)
+  const Real* pi;
+  const Scalars* sc;      // not NULL: the sums see phi' = phi + c_close pi (the pending closing half drift)
   double* partials;       // [3 NF + 1][nitems]
   Layout L;
   int zc;                 // planes per z-chunk
@@ -36,7 +40,7 @@ struct EnergySmem {
 };
 
 template <typename Real, class Model, class T>
-__global__ void __launch_bounds__(T::NT, 1)
+__global__ void __launch_bounds__(T::NT, T::MINB)
 energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_pi,
            const EnergyArgs<Real> g) {
   using R2 = typename Vec2T<Real>::type;
@@ -80,6 +84,8 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
 
   const double c1 = g.c1, c2 = g.c2, c3 = g.c3;
   const double c0 = -(6.0 * c1 + 12.0 * c2 + 8.0 * c3);
+  const bool drift = g.sc != nullptr;                          // block-uniform
+  const Real cd = drift ? Real(g.sc->c_close) : Real(0);
   const typename Model::template Coef<double> coef(g.mp);
 
   bool valid[J];
@@ -101,18 +107,19 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
     halo_sm[k] = h < T::NHP ? row * PX + col : -1;
   }
 
-  // per site: value pair of plane p-1 (phi, pi), accumulators of D[psi] (A, B) and of D[psi^2] (A2, B2)
-  double2 pphi[NF][J], ppi[NF][J], A[NF][J], B[NF][J], A2[NF][J], B2[NF][J];
+  // per site: value pair of plane p-1 (phi, pi), accumulators of D[psi] (A, B)
+  double2 pphi[NF][J], ppi[NF][J], A[NF][J], B[NF][J];
   Real ref[NF];
   double acc[NQ];
 #pragma unroll
   for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
-    ref[f] = Real(0);
+    // one reference value per field for the WHOLE lattice: the field at site (0,0,0) as a flushed state holds it
+    const size_t o0 = L.at(f, 0, 0, 0);
+    ref[f] = drift ? fma(cd, g.pi[o0], g.phi[o0]) : g.phi[o0];
 #pragma unroll
-    for (int j = 0; j < J; ++j)
-      pphi[f][j] = ppi[f][j] = A[f][j] = B[f][j] = A2[f][j] = B2[f][j] = double2{0.0, 0.0};
+    for (int j = 0; j < J; ++j) pphi[f][j] = ppi[f][j] = A[f][j] = B[f][j] = double2{0.0, 0.0};
   }
 
   __syncthreads();                                             // barriers initialised before anyone waits
@@ -124,10 +131,6 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
     const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
     Real* pb = psi + (size_t)(i & 1) * (SM::BOXA / sizeof(Real));
     mbar_wait(bars + 8u * s, (uint32_t)((i / S) & 1));
-    if (p == -1) {
-#pragma unroll
-      for (int f = 0; f < NF; ++f) ref[f] = rphi[f * PLANE + PX + G];
-    }
 
     // ---- 1. psi = phi - ref into shared memory (own pairs and halo ring); keep phi, pi of the own sites
     double2 cphi[NF][J], cpi[NF][J];
@@ -136,8 +139,9 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
 #pragma unroll
       for (int j = 0; j < J; ++j) {
         const int o = f * PLANE + own_sm + j * PX;
-        const R2 a = *reinterpret_cast<const R2*>(rphi + o);
+        R2 a = *reinterpret_cast<const R2*>(rphi + o);
         const R2 b = *reinterpret_cast<const R2*>(rpi + o);
+        if (drift) { a.x = fma(cd, b.x, a.x); a.y = fma(cd, b.y, a.y); }     // as drift_flush would store it
         cphi[f][j] = double2{(double)a.x, (double)a.y};
         cpi[f][j] = double2{(double)b.x, (double)b.y};
         *reinterpret_cast<R2*>(pb + o) = R2{a.x - ref[f], a.y - ref[f]};
@@ -146,7 +150,11 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
       for (int k = 0; k < NHT; ++k)
         if (halo_sm[k] >= 0) {
           const int o = f * PLANE + halo_sm[k];
-          const R2 a = *reinterpret_cast<const R2*>(rphi + o);
+          R2 a = *reinterpret_cast<const R2*>(rphi + o);
+          if (drift) {
+            const R2 b = *reinterpret_cast<const R2*>(rpi + o);
+            a.x = fma(cd, b.x, a.x); a.y = fma(cd, b.y, a.y);
+          }
           *reinterpret_cast<R2*>(pb + o) = R2{a.x - ref[f], a.y - ref[f]};
         }
     }
@@ -158,31 +166,23 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
     for (int f = 0; f < NF; ++f) {
       const Real* sp = pb + f * PLANE + own_sm - PX;           // row above the first own row
       double Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];       // psi: side sums and centres of x-outputs 0, 1
-      double Sx[J + 2], Qx[J + 2], Sy[J + 2], Qy[J + 2];       // psi^2: the same
 #pragma unroll
       for (int r = 0; r < J + 2; ++r) {
         const double l = (double)sp[r * PX - 1];
         const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
         const double mx = (double)m.x, my = (double)m.y;
         const double rr = (double)sp[r * PX + 2];
-        const double l2 = l * l, mx2 = mx * mx, my2 = my * my, rr2 = rr * rr;
         Rx[r] = l + my; Cx[r] = mx; Ry[r] = mx + rr; Cy[r] = my;
-        Sx[r] = l2 + my2; Qx[r] = mx2; Sy[r] = mx2 + rr2; Qy[r] = my2;
       }
 #pragma unroll
       for (int j = 0; j < J; ++j) {
-        double Dx, Dy, D2x, D2y;
+        double Dx, Dy;
         {
           const double P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
           const double up = fma(c3, P2, fma(c2, P1, c1 * P0));
           Dx = A[f][j].x + up;
           A[f][j].x = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].x)));
           B[f][j].x = up;
-          const double Q0 = Qx[j + 1], Q1 = Sx[j + 1] + (Qx[j] + Qx[j + 2]), Q2 = Sx[j] + Sx[j + 2];
-          const double up2 = fma(c3, Q2, fma(c2, Q1, c1 * Q0));
-          D2x = A2[f][j].x + up2;
-          A2[f][j].x = fma(c2, Q2, fma(c1, Q1, fma(c0, Q0, B2[f][j].x)));
-          B2[f][j].x = up2;
         }
         {
           const double P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
@@ -190,19 +190,14 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
           Dy = A[f][j].y + up;
           A[f][j].y = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].y)));
           B[f][j].y = up;
-          const double Q0 = Qy[j + 1], Q1 = Sy[j + 1] + (Qy[j] + Qy[j + 2]), Q2 = Sy[j] + Sy[j + 2];
-          const double up2 = fma(c3, Q2, fma(c2, Q1, c1 * Q0));
-          D2y = A2[f][j].y + up2;
-          A2[f][j].y = fma(c2, Q2, fma(c1, Q1, fma(c0, Q0, B2[f][j].y)));
-          B2[f][j].y = up2;
         }
         if (p >= 1 && valid[j]) {                              // output plane p-1 (an own plane: 0 .. nz-1)
           const double rf = (double)ref[f];
           const double px = pphi[f][j].x, py = pphi[f][j].y;   // phi
           const double sx = px - rf, sy = py - rf;             // psi
           acc[3 * f] = fma(ppi[f][j].x, ppi[f][j].x, fma(ppi[f][j].y, ppi[f][j].y, acc[3 * f]));
-          acc[3 * f + 1] += 0.5 * (fma(-2.0 * sx, Dx, D2x) + fma(-2.0 * sy, Dy, D2y));   // G = (D[psi^2] - 2 psi D[psi])/2
-          acc[3 * f + 2] = fma(px, Dx, fma(py, Dy, acc[3 * f + 2]));
+          acc[3 * f + 1] = fma(-sx, Dx, fma(-sy, Dy, acc[3 * f + 1]));     // sum G = - sum psi D[psi]   (2.17)
+          acc[3 * f + 2] = fma(px, Dx, fma(py, Dy, acc[3 * f + 2]));       // sum phi D[phi] as written
         }
       }
     }

@@ -138,6 +138,55 @@ bin_shells(const double2* __restrict__ F, int N, double norm2, int nbins, double
   for (int i = threadIdx.x; i < 2 * nbins; i += blockDim.x) part[(size_t)blockIdx.x * 2 * nbins + i] = hist[i];
 }
 
+// Number- and energy-density spectra of one field (reading G24): with F^phi_k, F^pi_k
+// the D2Z transforms scaled by norm = L^1.5 / (sqrt 2 N^3), u = a F^phi, v = F^pi / a,
+//   w_k^2 = k_eff^2(n)/dx^2 + a^2 m_eff^2,  -k_eff^2 = eigenvalue of the stencil (2.7) on the mode,
+//   n_k = 1/2 (w |u|^2 + |v|^2 / w)  (0 where w^2 <= 0),   rho_k = 1/2 (|v|^2 + w^2 |u|^2),
+// added into the shell round(|n|) with the half-spectrum weight (2, or 1 on the planes ix = 0 and ix = N/2).
+// hist: [nbins] number, [nbins] energy, [nbins] counts.
+struct ModeSpectrumArgs {
+  double norm2, a2, m_eff2, inv_dx2, c0, c1, c2, c3;
+};
+__global__ void __launch_bounds__(256)
+bin_mode_spectra(const double2* __restrict__ Fphi, const double2* __restrict__ Fpi, int N, ModeSpectrumArgs g,
+                 int nbins, double* __restrict__ part /* [grid][3 nbins] */) {
+  extern __shared__ double hist[];
+  for (int i = threadIdx.x; i < 3 * nbins; i += blockDim.x) hist[i] = 0.0;
+  __syncthreads();
+  const int H = N / 2 + 1;
+  const unsigned long long nmodes = (unsigned long long)N * N * H;
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  const double inv_n = 2.0 / (double)N;
+  for (unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; j < nmodes; j += stride) {
+    const int ix = (int)(j % H);
+    const unsigned long long zy = j / H;
+    const int iy = (int)(zy % N), iz = (int)(zy / N);
+    const int nz = iz <= N / 2 ? iz : iz - N, ny = iy <= N / 2 ? iy : iy - N;
+    const long long n2 = (long long)nz * nz + (long long)ny * ny + (long long)ix * ix;
+    const int shell = (int)floor(sqrt((double)n2) + 0.5);
+    if (shell >= nbins) continue;
+    const double Cx = cospi(inv_n * ix), Cy = cospi(inv_n * iy), Cz = cospi(inv_n * iz);
+    const double keff2 = -(g.c0 + 2.0 * g.c1 * (Cx + Cy + Cz) + 4.0 * g.c2 * (Cx * Cy + Cy * Cz + Cz * Cx) +
+                           8.0 * g.c3 * Cx * Cy * Cz);
+    const double w2 = keff2 * g.inv_dx2 + g.a2 * g.m_eff2;
+    const double2 fp = Fphi[j], fq = Fpi[j];
+    const double u2 = g.norm2 * g.a2 * fma(fp.x, fp.x, fp.y * fp.y);
+    const double v2 = g.norm2 * fma(fq.x, fq.x, fq.y * fq.y) / g.a2;
+    const double wgt = (ix == 0 || (N % 2 == 0 && ix == N / 2)) ? 1.0 : 2.0;
+    const double rho = 0.5 * (v2 + w2 * u2);
+    double num = 0.0;
+    if (w2 > 0.0) {
+      const double w = sqrt(w2);
+      num = 0.5 * (w * u2 + v2 / w);
+    }
+    atomicAdd(&hist[shell], wgt * num);
+    atomicAdd(&hist[nbins + shell], wgt * rho);
+    atomicAdd(&hist[2 * nbins + shell], wgt);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < 3 * nbins; i += blockDim.x) part[(size_t)blockIdx.x * 3 * nbins + i] = hist[i];
+}
+
 __global__ void __launch_bounds__(256) reduce_shells(const double* __restrict__ part, int nblocks, int n, double* __restrict__ out) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;

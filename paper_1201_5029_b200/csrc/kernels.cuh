@@ -73,6 +73,10 @@ struct Scalars {          // device-resident; one per context
   double eta;             // conformal time: sum of the completed steps' lengths
   int nonfinite;          // sticky: a lattice sum was NaN/Inf
   int pad;
+  // the time-synchronised state at the end of the latest completed step (a and p_a above already carry the opening
+  // half flows of the next stage while a pycool_step call is under way): what an energy read-out at that instant
+  // sees, and the closing half drift phi += c_close pi that makes phi synchronous with it (the energy log)
+  double a_sync, pa_sync, c_close;
 };
 
 struct ScalarConst {
@@ -154,7 +158,10 @@ __device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k,
     flow_H2_pa(s, k, e);                       // H2(h/2), scalar part (pi is constant in H2: post-kick sum)
     c1 = drift_coef(s, e);                     //          field part, applied by the next kernel
     flow_H1(s, k, e);                          // H1(h/2)
-    if (len.ends_step) s.eta = __dadd_rn(s.eta, step_len);
+    if (len.ends_step) {
+      s.eta = __dadd_rn(s.eta, step_len);
+      s.a_sync = s.a; s.pa_sync = s.p_a; s.c_close = c1;
+    }
   }
   if (len.w_next != 0.0) {
     double next_len = step_len;
@@ -525,13 +532,20 @@ __global__ void __launch_bounds__(256) sumsq(const Real* __restrict__ v, Layout 
 template <typename Real, class Model>
 __global__ void __launch_bounds__(256)
 energy_sums(const Real* __restrict__ phi, const Real* __restrict__ pi, Layout L, double c1, double c2, double c3,
-            ModelParams mp, double* __restrict__ partials) {
+            ModelParams mp, double* __restrict__ partials, const Scalars* __restrict__ sc /* NULL: phi as stored */) {
   constexpr int NF = Model::NF, NQ = 3 * NF + 1;
   __shared__ double sh[NQ * 8];
   const int N = L.N;
   const size_t V = (size_t)N * N * N;
   const typename Model::template Coef<double> coef(mp);
   const double cw[4] = {0.0, c1, c2, c3};
+  // with sc: the state seen through the pending closing half drift, phi' = phi + c_close pi, formed
+  // in Real exactly as drift_flush would store it
+  const bool drift = sc != nullptr;
+  const Real cd = drift ? Real(sc->c_close) : Real(0);
+  auto at = [&](const Real* pf, const Real* qf, size_t i) -> double {
+    return drift ? (double)fma(cd, qf[i], pf[i]) : (double)pf[i];
+  };
   double acc[NQ];
 #pragma unroll
   for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
@@ -545,8 +559,9 @@ energy_sums(const Real* __restrict__ phi, const Real* __restrict__ pi, Layout L,
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       const Real* pf = phi + f * L.field;
+      const Real* qf = pi + f * L.field;
       const size_t ic = L.at(0, z, y, x);
-      const double ctr = (double)pf[ic];
+      const double ctr = at(pf, qf, ic);
       double s[4] = {0, 0, 0, 0}, q2[4] = {0, 0, 0, 0};
 #pragma unroll
       for (int dz = 0; dz < 3; ++dz)
@@ -556,7 +571,7 @@ energy_sums(const Real* __restrict__ phi, const Real* __restrict__ pi, Layout L,
           for (int dx = 0; dx < 3; ++dx) {
             const int d = (dx != 1) + (dy != 1) + (dz != 1);
             if (d == 0) continue;
-            const double df = (double)pf[L.at(0, zs[dz], ys[dy], xs[dx])] - ctr;
+            const double df = at(pf, qf, L.at(0, zs[dz], ys[dy], xs[dx])) - ctr;
             s[d] += df;
             q2[d] = fma(df, df, q2[d]);
           }

@@ -133,7 +133,7 @@ WorkLayout work_layout(int N, int nf, size_t esize) {
   w.arr = align_up(L.total * esize, 256);
   size_t o = 4 * w.arr;
   w.off_part = o; o += align_up(partials_capacity(N) * sizeof(double), 256);
-  w.off_sums = o; o += 256;
+  w.off_sums = o; o += 512;      // 16 reduced rows, then one pycool_energy (the latest read-out)
   w.off_sc = o; o += 256;
   w.total = o;
   return w;
@@ -345,18 +345,19 @@ int launch_fill_ghosts(pycool_ctx* c, void* arr) {
   return PYCOOL_OK;
 }
 
-// sums[0 .. 3 nf] <- per field (sum pi^2, sum G, sum phi D phi), then sum V; synchronises
-int energy_sums_host(pycool_ctx* c, double* out /* 3 nf + 1 */) {
-  const int nq = 3 * c->nf + 1;
+// One energy read-out, kernels only (no host synchronisation): the lattice sums of the current buffers -- seen through
+// the pending closing half drift when `through_drift` -- then energy_finish into *d_out (device).
+int enqueue_energy(pycool_ctx* c, bool through_drift, pycool_energy* d_out) {
   int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)kMaxSumBlocks);
+  c->energy_through_drift = through_drift;
   int st = (int)dispatch(c, OP_ENERGY, nb);
+  c->energy_through_drift = false;
   if (st != PYCOOL_OK) return st;
-  nb = c->energy_nb;
-  reduce_rows<<<nq, kReduceThreads, 0, c->stream>>>(c->partials, nb, c->sums);
+  EnergyConst k;
+  k.V = (double)c->V; k.dx2 = c->dx * c->dx; k.mpl = c->mpl; k.rho_g = c->rho_g; k.rho_m = c->rho_m; k.nf = c->nf;
+  energy_finish<<<1, kReduceThreads, 0, c->stream>>>(c->partials, c->energy_nb, c->sc, k, d_out);
   CUDA_TRY(c, cudaGetLastError());
   c->counts[3] += 2;
-  CUDA_TRY(c, cudaMemcpyAsync(out, c->sums, nq * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   return PYCOOL_OK;
 }
 
@@ -370,21 +371,14 @@ int read_scalars(pycool_ctx* c, Scalars* s) {
   return PYCOOL_OK;
 }
 
-struct Averages { double K[4], Gr[4], GrD[4], Vbar; };
-
-// lattice averages entering rho and P at scale factor a: (2.16), (2.8), (2.17)
-int averages(pycool_ctx* c, double a, Averages* av) {
-  double s[16];
-  int st = energy_sums_host(c, s);
+// The energies of the time-synchronised state on the host: flush, read-out on the device, one D2H copy; synchronises.
+int energies_now(pycool_ctx* c, pycool_energy* o) {
+  int st = ensure_flushed(c);
+  if (st == PYCOOL_OK) st = enqueue_energy(c, false, c->d_energy);
   if (st != PYCOOL_OK) return st;
-  const double a2 = a * a, a6 = a2 * a2 * a2, Vs = (double)c->V, dx2 = c->dx * c->dx;
-  for (int f = 0; f < c->nf; ++f) {
-    av->K[f] = s[3 * f] / (2.0 * a6 * Vs);
-    av->Gr[f] = s[3 * f + 1] / (2.0 * a2 * dx2 * Vs);
-    av->GrD[f] = -s[3 * f + 2] / (2.0 * a2 * dx2 * Vs);
-  }
-  av->Vbar = s[3 * c->nf] / Vs;
-  return PYCOOL_OK;
+  CUDA_TRY(c, cudaMemcpyAsync(o, c->d_energy, sizeof(pycool_energy), cudaMemcpyDeviceToHost, c->stream));
+  Scalars s;
+  return read_scalars(c, &s);
 }
 
 // ---- cuFFT, loaded on first use (pycool_init_fields only): a library FFT is a step the scope allows; loading it
@@ -536,6 +530,7 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
   c->partials = (double*)(work + w.off_part);
   c->partials_cap = partials_capacity(N);
   c->sums = (double*)(work + w.off_sums);
+  c->d_energy = (pycool_energy*)(work + w.off_sums + 256);
   c->sc = (Scalars*)(work + w.off_sc);
   c->ticket = (unsigned int*)(work + w.off_sc + 128);
   c->tile = auto_tile(c);
@@ -659,6 +654,85 @@ int pycool_init_fields(pycool_ctx* c, unsigned long long seed, const pycool_spec
   return launch_sum_pi2(c);
 }
 
+namespace {
+
+// D2Z transform of one array of the current state (phi or pi of one field) into `scratch` (N^2 (N/2+1) complex).
+int transform_array(pycool_ctx* c, const CufftApi& fft, cufftHandle plan, int field, int which, double2* scratch) {
+  const int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)c->sms * 64);
+  const void* base = which == 0 ? c->phi[c->cur] : c->pi[c->cur];
+  if (c->precision == 32)
+    gather_real<float><<<nb, 256, 0, c->stream>>>((double*)scratch, (const float*)base + (size_t)field * c->lay.field, c->lay);
+  else
+    gather_real<double><<<nb, 256, 0, c->stream>>>((double*)scratch, (const double*)base + (size_t)field * c->lay.field, c->lay);
+  CUDA_TRY(c, cudaGetLastError());
+  c->counts[3]++;
+  if (fft.exec_d2z(plan, (cufftDoubleReal*)scratch, (cufftDoubleComplex*)scratch) != CUFFT_SUCCESS)
+    return fail(c, PYCOOL_ECUDA, "cufftExecD2Z failed");
+  return PYCOOL_OK;
+}
+
+// Shell sums of one (kind 0: |F|^2 of one array; kind 1: number and energy density of one field) spectrum.
+int shell_spectrum(pycool_ctx* c, int field, int which, int kind, double m_eff2, int nbins, double* out0, double* out1,
+                   double* count_host) {
+  const CufftApi& fft = cufft_api();
+  if (!fft.ok) return fail(c, PYCOOL_ECUDA, "cuFFT (libcufft.so.11) could not be loaded");
+  const int N = c->N, rows = kind == 0 ? 2 : 3;
+  const size_t nmodes = (size_t)N * N * (N / 2 + 1);
+  const int nblk = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)c->sms * 8);
+  Scalars sc;
+  int st = read_scalars(c, &sc);                           // the time-synchronised a (the state has been flushed)
+  if (st != PYCOOL_OK) return st;
+  double2* scratch = nullptr;
+  double* part = nullptr;
+  if (cudaMalloc(&scratch, (kind == 0 ? 1 : 2) * nmodes * sizeof(double2)) != cudaSuccess ||
+      cudaMalloc(&part, ((size_t)nblk + 1) * rows * nbins * sizeof(double)) != cudaSuccess) {
+    cudaGetLastError();
+    if (scratch) cudaFree(scratch);
+    return fail(c, PYCOOL_ENOMEM, "out of device memory for the spectrum scratch");
+  }
+  cufftHandle plan = 0;
+  if (fft.plan3d(&plan, N, N, N, CUFFT_D2Z) != CUFFT_SUCCESS || fft.set_stream(plan, c->stream) != CUFFT_SUCCESS) {
+    cudaFree(scratch); cudaFree(part);
+    return fail(c, PYCOOL_ENOMEM, "cufftPlan3d(%d^3, D2Z) failed", N);
+  }
+  const double norm = c->L * std::sqrt(c->L) / (std::sqrt(2.0) * (double)N * (double)N * (double)N);
+  std::vector<double> h((size_t)rows * nbins);
+  auto run = [&]() -> int {
+    if (kind == 0) {
+      if (int e = transform_array(c, fft, plan, field, which, scratch)) return e;
+      bin_shells<<<nblk, 256, 2 * nbins * sizeof(double), c->stream>>>(scratch, N, norm * norm, nbins, part);
+    } else {
+      if (int e = transform_array(c, fft, plan, field, 0, scratch)) return e;
+      if (int e = transform_array(c, fft, plan, field, 1, scratch + nmodes)) return e;
+      ModeSpectrumArgs g;
+      g.norm2 = norm * norm; g.a2 = sc.a_sync * sc.a_sync; g.m_eff2 = m_eff2; g.inv_dx2 = 1.0 / (c->dx * c->dx);
+      g.c0 = c->c[0]; g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
+      bin_mode_spectra<<<nblk, 256, 3 * nbins * sizeof(double), c->stream>>>(scratch, scratch + nmodes, N, g, nbins, part);
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    double* out = part + (size_t)nblk * rows * nbins;
+    reduce_shells<<<(rows * nbins + 255) / 256, 256, 0, c->stream>>>(part, nblk, rows * nbins, out);
+    CUDA_TRY(c, cudaGetLastError());
+    c->counts[3] += 2;
+    CUDA_TRY(c, cudaMemcpyAsync(h.data(), out, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return PYCOOL_OK;
+  };
+  st = run();
+  if (st != PYCOOL_OK) cudaStreamSynchronize(c->stream);
+  fft.destroy(plan);
+  cudaFree(scratch); cudaFree(part);
+  if (st != PYCOOL_OK) return st;
+  for (int i = 0; i < nbins; ++i) {
+    out0[i] = h[i];
+    if (kind != 0) out1[i] = h[nbins + i];
+    count_host[i] = h[(size_t)(rows - 1) * nbins + i];
+  }
+  return PYCOOL_OK;
+}
+
+}  // namespace
+
 int pycool_field_spectrum(pycool_ctx* c, int field, int which, int nbins, double* power_host, double* count_host) {
   if (!c) return PYCOOL_EINVAL;
   OnDevice on_device(c);
@@ -668,45 +742,20 @@ int pycool_field_spectrum(pycool_ctx* c, int field, int which, int nbins, double
     return fail(c, PYCOOL_EINVAL, "nbins must be 1..3072 and the outputs non-NULL");
   int st = ensure_flushed(c);
   if (st != PYCOOL_OK) return st;
-  const CufftApi& fft = cufft_api();
-  if (!fft.ok) return fail(c, PYCOOL_ECUDA, "cuFFT (libcufft.so.11) could not be loaded");
-  const int N = c->N;
-  const size_t nmodes = (size_t)N * N * (N / 2 + 1);
-  const int nblk = (int)std::min<size_t>((nmodes + 255) / 256, (size_t)c->sms * 8);
-  double2* scratch = nullptr;
-  double* part = nullptr;
-  CUDA_TRY(c, cudaMalloc(&scratch, nmodes * sizeof(double2)));
-  if (cudaMalloc(&part, ((size_t)nblk + 1) * 2 * nbins * sizeof(double)) != cudaSuccess) {
-    cudaFree(scratch);
-    return fail(c, PYCOOL_ENOMEM, "out of device memory");
-  }
-  cufftHandle plan = 0;
-  if (fft.plan3d(&plan, N, N, N, CUFFT_D2Z) != CUFFT_SUCCESS || fft.set_stream(plan, c->stream) != CUFFT_SUCCESS) {
-    cudaFree(scratch); cudaFree(part);
-    return fail(c, PYCOOL_ENOMEM, "cufftPlan3d(%d^3, D2Z) failed", N);
-  }
-  const int nb = (int)std::min<size_t>((c->V + 255) / 256, (size_t)c->sms * 64);
-  const void* base = which == 0 ? c->phi[c->cur] : c->pi[c->cur];
-  if (c->precision == 32)
-    gather_real<float><<<nb, 256, 0, c->stream>>>((double*)scratch, (const float*)base + (size_t)field * c->lay.field, c->lay);
-  else
-    gather_real<double><<<nb, 256, 0, c->stream>>>((double*)scratch, (const double*)base + (size_t)field * c->lay.field, c->lay);
-  cufftResult fr = fft.exec_d2z(plan, (cufftDoubleReal*)scratch, (cufftDoubleComplex*)scratch);
-  const double norm = c->L * std::sqrt(c->L) / (std::sqrt(2.0) * (double)N * (double)N * (double)N);
-  bin_shells<<<nblk, 256, 2 * nbins * sizeof(double), c->stream>>>(scratch, N, norm * norm, nbins, part);
-  double* out = part + (size_t)nblk * 2 * nbins;
-  reduce_shells<<<(2 * nbins + 255) / 256, 256, 0, c->stream>>>(part, nblk, 2 * nbins, out);
-  cudaError_t e = cudaGetLastError();
-  std::vector<double> h(2 * (size_t)nbins);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), out, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  fft.destroy(plan);
-  cudaFree(scratch); cudaFree(part);
-  c->counts[3] += 3;
-  if (fr != CUFFT_SUCCESS) return fail(c, PYCOOL_ECUDA, "cufftExecD2Z failed");
-  CUDA_TRY(c, e);
-  for (int i = 0; i < nbins; ++i) { power_host[i] = h[i]; count_host[i] = h[nbins + i]; }
-  return PYCOOL_OK;
+  return shell_spectrum(c, field, which, 0, 0.0, nbins, power_host, nullptr, count_host);
+}
+
+int pycool_mode_spectra(pycool_ctx* c, int field, double m_eff2, int nbins, double* number_host, double* energy_host,
+                        double* count_host) {
+  if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
+  if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "spectrum before set_fields");
+  if (field < 0 || field >= c->nf || !std::isfinite(m_eff2)) return fail(c, PYCOOL_EINVAL, "bad field or m_eff2");
+  if (nbins < 1 || nbins > 2048 || !number_host || !energy_host || !count_host)   // 3 nbins doubles of shared memory
+    return fail(c, PYCOOL_EINVAL, "nbins must be 1..2048 and the outputs non-NULL");
+  int st = ensure_flushed(c);
+  if (st != PYCOOL_OK) return st;
+  return shell_spectrum(c, field, 0, 1, m_eff2, nbins, number_host, energy_host, count_host);
 }
 
 int pycool_set_background(pycool_ctx* c, double a, double p_a) {
@@ -717,15 +766,14 @@ int pycool_set_background(pycool_ctx* c, double a, double p_a) {
   if (std::isnan(p_a)) {                                   // reading G10: (2.18), expanding branch
     if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "p_a = NaN needs fields (call set_fields first)");
     if (std::isinf(c->mpl)) return fail(c, PYCOOL_EINVAL, "p_a = NaN with a static background (mpl = INF)");
-    Averages av;
-    int st = averages(c, a, &av);
+    set_scalars<<<1, 1, 0, c->stream>>>(c->sc, a, 0.0, 0);   // rho at the new a
+    CUDA_TRY(c, cudaGetLastError());
+    pycool_energy e;
+    int st = energies_now(c, &e);
     if (st != PYCOOL_OK) return st;
-    const double a2 = a * a;
-    double rho = av.Vbar + c->rho_g / (a2 * a2) + c->rho_m / (a2 * a);
-    for (int f = 0; f < c->nf; ++f) rho += av.K[f] + av.Gr[f];
-    if (!(rho >= 0)) return fail(c, PYCOOL_EINVAL, "negative or non-finite energy density");
-    const double ap = a2 * (double)sqrtl((long double)(rho / 3.0)) / c->mpl;      // (2.18)
-    p_a = -6.0 * (double)c->V * c->mpl * c->mpl * ap;                              // (2.11)
+    if (!(e.rho >= 0)) return fail(c, PYCOOL_EINVAL, "negative or non-finite energy density");
+    const double ap = a * a * (double)sqrtl((long double)(e.rho / 3.0)) / c->mpl;   // (2.18)
+    p_a = -6.0 * (double)c->V * c->mpl * c->mpl * ap;                                // (2.11)
   }
   set_scalars<<<1, 1, 0, c->stream>>>(c->sc, a, p_a, 1);
   CUDA_TRY(c, cudaGetLastError());
@@ -777,6 +825,13 @@ int pycool_step(pycool_ctx* c, int nsteps) {
     if (!c->fused_tail) {
       st = launch_scalar(c, len, 1);
       if (st != PYCOOL_OK) return st;
+    }
+    if (len.ends_step && c->log_every > 0 && ++c->steps_done % (unsigned long long)c->log_every == 0) {
+      // energy log: a read-out of the state this step ends in (its closing half drift applied on the fly, the
+      // scale factor of that instant), appended on the device; the step sequence itself is untouched
+      st = enqueue_energy(c, true, c->d_log + (c->log_n % (unsigned long long)c->log_cap));
+      if (st != PYCOOL_OK) return st;
+      c->log_n++;
     }
   }
   c->pending_drift = true;
@@ -846,28 +901,47 @@ int pycool_energies(pycool_ctx* c, pycool_energy* o) {
   OnDevice on_device(c);
   if (!o) return fail(c, PYCOOL_EINVAL, "out is NULL");
   if (!c->have_fields) return fail(c, PYCOOL_ESTATE, "energies before set_fields");
-  int st = ensure_flushed(c);
-  if (st != PYCOOL_OK) return st;
-  Scalars s;
-  st = read_scalars(c, &s);
-  if (st != PYCOOL_OK) return st;
-  Averages av;
-  st = averages(c, s.a, &av);
-  if (st != PYCOOL_OK) return st;
-  std::memset(o, 0, sizeof *o);
-  const double a = s.a, a2 = a * a;
-  double rho = av.Vbar + c->rho_g / (a2 * a2) + c->rho_m / (a2 * a);               // (2.16) + (2.20)
-  double P = -av.Vbar + c->rho_g / (3.0 * a2 * a2);
-  for (int f = 0; f < c->nf; ++f) {
-    rho += av.K[f] + av.Gr[f];
-    P += av.K[f] - av.Gr[f] / 3.0;
-    o->kin[f] = av.K[f]; o->grad[f] = av.Gr[f]; o->sum_phiDphi[f] = av.GrD[f];
+  return energies_now(c, o);
+}
+
+int pycool_set_energy_cadence(pycool_ctx* c, int every, int capacity) {
+  if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
+  if (every < 0 || (every > 0 && capacity < 1) || capacity > (1 << 24))
+    return fail(c, PYCOOL_EINVAL, "every must be >= 0 and capacity 1 .. 2^24");
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (c->d_log) cudaFree(c->d_log);
+  c->d_log = nullptr;
+  c->log_every = 0; c->log_cap = 0; c->log_n = 0; c->steps_done = 0;
+  if (every == 0) return PYCOOL_OK;
+  if (cudaMalloc(&c->d_log, (size_t)capacity * sizeof(pycool_energy)) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(c, PYCOOL_ENOMEM, "cudaMalloc of the energy log (%d entries) failed", capacity);
   }
-  const double ap = -s.p_a / (6.0 * (double)c->V * c->mpl * c->mpl);               // (2.14)
-  const double H = ap / a2;
-  o->a = a; o->p_a = s.p_a; o->eta = s.eta;
-  o->pot = av.Vbar; o->rho = rho; o->pressure = P; o->hubble = H;
-  o->residual = std::isinf(c->mpl) ? 0.0 : std::fabs(rho / (3.0 * c->mpl * c->mpl * H * H) - 1.0);   // (3.1)
+  c->log_every = every; c->log_cap = capacity;
+  return PYCOOL_OK;
+}
+
+int pycool_read_energy_log(pycool_ctx* c, pycool_energy* out_host, int max_entries, int* n_out,
+                           unsigned long long* total) {
+  if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
+  if (!n_out || max_entries < 0 || (max_entries > 0 && !out_host)) return fail(c, PYCOOL_EINVAL, "bad output arguments");
+  *n_out = 0;
+  if (total) *total = c->log_n;
+  if (!c->d_log) return PYCOOL_OK;
+  const unsigned long long have = std::min<unsigned long long>(c->log_n, (unsigned long long)c->log_cap);
+  const int n = (int)std::min<unsigned long long>(have, (unsigned long long)max_entries);
+  // the newest n entries, oldest first; entry number j (0-based since the cadence was set) sits in slot j % capacity
+  for (int i = 0; i < n; ++i) {
+    const unsigned long long j = c->log_n - (unsigned long long)n + (unsigned long long)i;
+    CUDA_TRY(c, cudaMemcpyAsync(out_host + i, c->d_log + (j % (unsigned long long)c->log_cap), sizeof(pycool_energy),
+                                cudaMemcpyDeviceToHost, c->stream));
+  }
+  Scalars s;
+  int st = read_scalars(c, &s);            // synchronises; reports a non-finite sum
+  if (st != PYCOOL_OK) return st;
+  *n_out = n;
   return PYCOOL_OK;
 }
 
@@ -876,6 +950,7 @@ int pycool_destroy(pycool_ctx* c) {
   OnDevice on_device(c);
   if (c->stream || !c->own_stream) cudaStreamSynchronize(c->stream);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->d_log) cudaFree(c->d_log);
   if (c->own_stream) cudaStreamDestroy(c->stream);
   if (c->owned_block) cudaFree(c->owned_block);
   delete c;
@@ -951,7 +1026,8 @@ int pycool_set_overlap(pycool_ctx* c, int on) {
 int pycool_set_energy_kernel(pycool_ctx* c, int tma) {
   if (!c) return PYCOOL_EINVAL;
   OnDevice on_device(c);
-  c->energy_tma = tma != 0;
+  if (tma < 0 || tma > 4) return fail(c, PYCOOL_EINVAL, "energy kernel must be 0 (plain), 1 (automatic) or 2..4 (a TMA variant)");
+  c->energy_tma = tma;
   return PYCOOL_OK;
 }
 
