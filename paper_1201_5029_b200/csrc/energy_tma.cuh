@@ -115,9 +115,13 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
   for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
-    // one reference value per field for the WHOLE lattice: the field at site (0,0,0) as a flushed state holds it
+    // one reference value per field for the WHOLE lattice: the field at site (0,0,0) as a flushed state holds it.
+    // fp32 fields: psi is stored in shared memory as a float, and phi - ref is exact in float only next to ref
+    // (a mean-zero field would pick up 6e-8 relative per site, which D does not annihilate), so no reference is
+    // subtracted: the stencil runs in double on the exact float values (loses 5 of 16 digits, far below fp32).
     const size_t o0 = L.at(f, 0, 0, 0);
-    ref[f] = drift ? fma(cd, g.pi[o0], g.phi[o0]) : g.phi[o0];
+    if constexpr (sizeof(Real) == 4) ref[f] = Real(0);
+    else ref[f] = drift ? fma(cd, g.pi[o0], g.phi[o0]) : g.phi[o0];
 #pragma unroll
     for (int j = 0; j < J; ++j) pphi[f][j] = ppi[f][j] = A[f][j] = B[f][j] = double2{0.0, 0.0};
   }

@@ -337,8 +337,8 @@ def test_one_field_variant_two_by_four_sites_per_thread(pc, N, zc):
                                     ("cfg3_qball256", 40), ("cfg3_qball256", 6)])
 @pytest.mark.parametrize("precision", [64, 32])
 def test_energy_kernels_agree_with_each_other_and_the_oracle(pc, name, N, precision):
-    """pycool_energies through the TMA-fed z-march (G from 2 G[psi] = D[psi^2] - 2 psi D[psi]) and through the plain
-    kernel that evaluates (2.8) term by term, after a few steps, against the oracle's direct evaluation; ragged
+    """pycool_energies through the TMA-fed z-march (sum G = - sum psi D[psi], the paper's identity (2.17)) and through
+    the plain kernel that evaluates (2.8) term by term, after a few steps, against the oracle's direct evaluation; ragged
     tiles, several z-chunks (N = 70, 136) and a lattice smaller than a tile (N = 6)."""
     cfg = inputs.config(name, N=N)
     cfg["L"] = cfg["L"] * N / inputs.config(name)["N"]
@@ -360,7 +360,9 @@ def test_energy_kernels_agree_with_each_other_and_the_oracle(pc, name, N, precis
     for f in range(cfg["nfields"]):
         assert rel(a.grad[f], b.grad[f]) <= (1e-12 if precision == 64 else 1e-6)
         # sum phi D[phi] = phi_0 sum D + sum dphi D with sum D = 0 up to rounding: the order of the sum shows at 1e-10
-        assert rel(a.kin[f], b.kin[f]) <= 1e-13 and rel(a.sum_phiDphi[f], b.sum_phiDphi[f]) <= 1e-9
+        # (condition number sum|phi D| / |sum phi D| ~ 3e5 on this lattice; fp32 fields: compared at fp32 accuracy)
+        assert rel(a.kin[f], b.kin[f]) <= 1e-13
+        assert rel(a.sum_phiDphi[f], b.sum_phiDphi[f]) <= (1e-9 if precision == 64 else 1e-6)
         assert rel(a.grad[f], a.sum_phiDphi[f]) <= (1e-9 if precision == 64 else 1e-4)      # (2.17)
     assert rel(a.pot, b.pot) <= 1e-13 and rel(a.rho, b.rho) <= 1e-12
 
