@@ -23,7 +23,13 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
            "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_init_fields",
-           "pycool_field_spectrum", "pycool_mode_spectra", "pycool_set_energy_cadence", "pycool_read_energy_log")
+           "pycool_field_spectrum", "pycool_mode_spectra", "pycool_set_energy_cadence", "pycool_read_energy_log",
+           # include/pycool_linear.h
+           "pycool_linear_create", "pycool_linear_num_classes", "pycool_linear_set_background",
+           "pycool_linear_set_perturbations", "pycool_linear_set_modes", "pycool_linear_step", "pycool_linear_read_modes",
+           "pycool_linear_read_perturbations", "pycool_linear_background_state", "pycool_linear_growth",
+           "pycool_linear_time_ms", "pycool_linear_destroy", "pycool_linear_last_error")
+GROWTH, NAIVE = 0, 1
 
 
 class Params(C.Structure):
@@ -48,6 +54,12 @@ class Energy(C.Structure):
             v = getattr(self, name)
             d[name] = list(v) if hasattr(v, "__len__") else v
         return d
+
+
+class LinearBackground(C.Structure):
+    _fields_ = [("a", C.c_double), ("p_a", C.c_double), ("eta", C.c_double), ("phi0", C.c_double * 4),
+                ("pi0", C.c_double * 4), ("kin", C.c_double), ("pot", C.c_double), ("rho", C.c_double),
+                ("hubble", C.c_double), ("residual", C.c_double)]
 
 
 class PycoolError(RuntimeError):
@@ -104,6 +116,22 @@ def lib():
         L.pycool_mode_spectra.argtypes = [vp, ip, d, ip, C.POINTER(d), C.POINTER(d), C.POINTER(d)]
         L.pycool_set_energy_cadence.argtypes = [vp, ip, ip]
         L.pycool_read_energy_log.argtypes = [vp, C.POINTER(Energy), ip, C.POINTER(ip), C.POINTER(C.c_ulonglong)]
+        dp = C.POINTER(d)
+        L.pycool_linear_create.argtypes = [C.POINTER(vp), ip, d, ip, pp, ip, d]
+        L.pycool_linear_num_classes.argtypes = [ip]
+        L.pycool_linear_num_classes.restype = C.c_size_t
+        L.pycool_linear_set_background.argtypes = [vp, d, d, dp, dp]
+        L.pycool_linear_set_perturbations.argtypes = [vp, vp, vp]
+        L.pycool_linear_set_modes.argtypes = [vp, vp, vp]
+        L.pycool_linear_step.argtypes = [vp, ip, ip]
+        L.pycool_linear_read_modes.argtypes = [vp, vp, vp]
+        L.pycool_linear_read_perturbations.argtypes = [vp, vp, vp]
+        L.pycool_linear_background_state.argtypes = [vp, C.POINTER(LinearBackground)]
+        L.pycool_linear_growth.argtypes = [vp, vp, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.pycool_linear_time_ms.argtypes = [vp, dp]
+        L.pycool_linear_destroy.argtypes = [vp]
+        L.pycool_linear_last_error.argtypes = [vp]
+        L.pycool_linear_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -347,6 +375,98 @@ class Lattice:
     def close(self):
         if self._h:
             lib().pycool_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class LinearLattice:
+    """The linearised solver (include/pycool_linear.h): homogeneous background + Fourier-space perturbations on a CUDA
+    device, double precision.  Same call names as the C ABI; the library owns its device memory and stream."""
+
+    def __init__(self, N, L, nfields, model, p=(), order=4, dt=0.01, device=None, **kw):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1201_5029_b200 needs a CUDA device (no CPU fallback)")
+        self.N, self.L, self.nf, self.order = N, L, nfields, order
+        self.device = torch.device("cuda:0" if device is None else device)
+        self._mp = make_params(model, p, **kw)
+        self._h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            st = lib().pycool_linear_create(C.byref(self._h), N, L, nfields, C.byref(self._mp), order, dt)
+        if st != OK:
+            raise PycoolError(st, lib().pycool_linear_last_error(None).decode())
+        self.nclasses = int(lib().pycool_linear_num_classes(N))
+
+    def _chk(self, st):
+        if st != OK:
+            raise PycoolError(st, lib().pycool_linear_last_error(self._h).decode())
+
+    def _real(self, x):
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        if x.size != self.nf * self.N ** 3:
+            raise PycoolError(EINVAL, "real-space buffer has %d elements" % x.size)
+        return x
+
+    def _modes_shape(self):
+        return (self.nf, self.N, self.N, self.N // 2 + 1)
+
+    def set_background(self, a, p_a, phi0, pi0):
+        if len(phi0) != self.nf or len(pi0) != self.nf:
+            raise PycoolError(EINVAL, "phi0 / pi0 need one value per field")
+        u, v = (C.c_double * self.nf)(*map(float, phi0)), (C.c_double * self.nf)(*map(float, pi0))
+        self._chk(lib().pycool_linear_set_background(self._h, float(a), float(p_a), u, v))
+
+    def set_perturbations(self, dphi, dpi):
+        dphi, dpi = self._real(dphi), self._real(dpi)
+        self._chk(lib().pycool_linear_set_perturbations(self._h, dphi.ctypes.data, dpi.ctypes.data))
+
+    def set_modes(self, dPhi, dPi):
+        """Half spectra [nf, N, N, N/2+1] complex (plain DFT convention, numpy.fft.rfftn layout)."""
+        a = np.ascontiguousarray(dPhi, dtype=np.complex128)
+        b = np.ascontiguousarray(dPi, dtype=np.complex128)
+        if a.shape != self._modes_shape() or b.shape != self._modes_shape():
+            raise PycoolError(EINVAL, "half spectra must have shape %s" % (self._modes_shape(),))
+        self._chk(lib().pycool_linear_set_modes(self._h, a.ctypes.data, b.ctypes.data))
+
+    def step(self, n=1, method=GROWTH):
+        self._chk(lib().pycool_linear_step(self._h, int(n), int(method)))
+
+    def read_modes(self):
+        a, b = np.empty(self._modes_shape(), np.complex128), np.empty(self._modes_shape(), np.complex128)
+        self._chk(lib().pycool_linear_read_modes(self._h, a.ctypes.data, b.ctypes.data))
+        return a, b
+
+    def read_perturbations(self):
+        shape = (self.nf, self.N, self.N, self.N)
+        a, b = np.empty(shape, np.float64), np.empty(shape, np.float64)
+        self._chk(lib().pycool_linear_read_perturbations(self._h, a.ctypes.data, b.ctypes.data))
+        return a, b
+
+    def background(self):
+        out = LinearBackground()
+        self._chk(lib().pycool_linear_background_state(self._h, C.byref(out)))
+        return out
+
+    def growth(self):
+        """Growth matrices [classes, 2 nf, 2 nf] of the latest GROWTH step call."""
+        M = np.empty((self.nclasses, 2 * self.nf, 2 * self.nf), np.float64)
+        n = C.c_size_t()
+        self._chk(lib().pycool_linear_growth(self._h, M.ctypes.data, self.nclasses, C.byref(n)))
+        return M
+
+    def time_ms(self):
+        ms = (C.c_double * 3)()
+        self._chk(lib().pycool_linear_time_ms(self._h, ms))
+        return dict(background=ms[0], growth=ms[1], modes=ms[2])
+
+    def close(self):
+        if self._h:
+            lib().pycool_linear_destroy(self._h)
             self._h = C.c_void_p()
 
     def __del__(self):

@@ -19,9 +19,9 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpycool.so")
 PTXAS_LOG = os.path.join(OBJ, "libpycool.ptxas.txt")
-SOURCES = [os.path.join(CSRC, "pycool.cu")] + sorted(glob.glob(os.path.join(CSRC, "models_*.cu")))
+SOURCES = [os.path.join(CSRC, "pycool.cu"), os.path.join(CSRC, "linear.cu")] + sorted(glob.glob(os.path.join(CSRC, "models_*.cu")))
 DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + sorted(glob.glob(os.path.join(CSRC, "*.h"))) + \
-    [os.path.join(os.path.dirname(HERE), "include", "pycool.h"), os.path.abspath(__file__)]
+    sorted(glob.glob(os.path.join(os.path.dirname(HERE), "include", "*.h"))) + [os.path.abspath(__file__)]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 CFLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xptxas", "-v",
           "-Xcompiler", "-fPIC,-fvisibility=hidden"]

@@ -21,10 +21,10 @@
 
 #include <cuda.h>
 #include <cuda_runtime.h>
-#include <cufft.h>      // types only: the library is loaded on demand (dlopen), not linked
 #include <dlfcn.h>
 
 #include "context.h"
+#include "cufft_api.h"
 #include "init_fields.cuh"
 #include "scalar_kernels.cuh"
 #include "potentials.cuh"
@@ -381,17 +381,9 @@ int energies_now(pycool_ctx* c, pycool_energy* o) {
   return read_scalars(c, &s);
 }
 
-// ---- cuFFT, loaded on first use (pycool_init_fields only): a library FFT is a step the scope allows; loading it
-// lazily keeps the hot path free of it and fails loudly when it is missing.
-struct CufftApi {
-  cufftResult (*plan3d)(cufftHandle*, int, int, int, cufftType) = nullptr;
-  cufftResult (*set_stream)(cufftHandle, cudaStream_t) = nullptr;
-  cufftResult (*exec_z2d)(cufftHandle, cufftDoubleComplex*, cufftDoubleReal*) = nullptr;
-  cufftResult (*exec_d2z)(cufftHandle, cufftDoubleReal*, cufftDoubleComplex*) = nullptr;
-  cufftResult (*destroy)(cufftHandle) = nullptr;
-  bool ok = false;
-};
-const CufftApi& cufft_api() {
+// ---- cuFFT, loaded on first use (cufft_api.h)
+}  // namespace
+const CufftApi& pycool::cufft_api() {
   static CufftApi api;
   static bool tried = false;
   if (tried) return api;
@@ -410,6 +402,7 @@ const CufftApi& cufft_api() {
   api.ok = api.plan3d && api.set_stream && api.exec_z2d && api.exec_d2z && api.destroy;
   return api;
 }
+namespace {
 
 template <typename Real>
 int init_one_array(pycool_ctx* c, const CufftApi& fft, cufftHandle plan, double2* scratch, Real* dst,
@@ -538,7 +531,7 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
     // padding and ghosts start as zeros (the closing drift sweeps the whole padded arrays)
     Scalars s0;
     std::memset(&s0, 0, sizeof s0);
-    s0.a = 1.0;
+    s0.a = 1.0; s0.a_sync = 1.0;
     if (cudaMemsetAsync(work, 0, 4 * w.arr, c->stream) != cudaSuccess ||
         cudaMemsetAsync(work + w.off_sc, 0, 256, c->stream) != cudaSuccess ||
         cudaMemcpyAsync(c->sc, &s0, sizeof s0, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||

@@ -19,9 +19,12 @@ def L():
 
 
 def _declared():
-    src = open(os.path.join(ROOT, "include", "pycool.h")).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return set(re.findall(r"\b(pycool_[a-z0-9_]+)\s*\(", src))
+    names = set()
+    for h in ("pycool.h", "pycool_linear.h"):
+        src = open(os.path.join(ROOT, "include", h)).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names |= set(re.findall(r"\b(pycool_[a-z0-9_]+)\s*\(", src))
+    return names
 
 
 def test_header_symbols_all_exported(L):
@@ -42,17 +45,45 @@ def test_only_abi_symbols_are_exported(L):
 
 
 def test_struct_sizes_match_header():
-    """ctypes mirrors of pycool_params / pycool_energy against a C compiler's view of the header."""
+    """ctypes mirrors of pycool_params / pycool_energy / pycool_linear_background against a C compiler's view of the
+    headers."""
     import subprocess
     import tempfile
     from paper_1201_5029_b200 import binding
-    code = '#include <stdio.h>\n#include "pycool.h"\nint main(){printf("%zu %zu\\n", sizeof(pycool_params), sizeof(pycool_energy));return 0;}\n'
+    code = ('#include <stdio.h>\n#include "pycool_linear.h"\nint main(){printf("%zu %zu %zu\\n", sizeof(pycool_params), '
+            'sizeof(pycool_energy), sizeof(pycool_linear_background));return 0;}\n')
     with tempfile.TemporaryDirectory() as d:
         src, exe = os.path.join(d, "s.c"), os.path.join(d, "s")
         open(src, "w").write(code)
         subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), src, "-o", exe], check=True)
-        a, b = map(int, subprocess.run([exe], capture_output=True, text=True).stdout.split())
-    assert a == C.sizeof(binding.Params) and b == C.sizeof(binding.Energy)
+        a, b, c = map(int, subprocess.run([exe], capture_output=True, text=True).stdout.split())
+    assert a == C.sizeof(binding.Params) and b == C.sizeof(binding.Energy) and c == C.sizeof(binding.LinearBackground)
+
+
+def test_linear_create_validates_then_needs_a_gpu(L):
+    """include/pycool_linear.h: argument validation on the host, class count (reading G28), no CPU path."""
+    import torch
+    from paper_1201_5029_b200 import binding
+    h = C.c_void_p()
+
+    def create(N=8, Lbox=1.0, nf=1, model=binding.FREE, order=4, dt=0.1, **kw):
+        mp = binding.make_params(model, kw.pop("p", (1.0,)), **kw)
+        return L.pycool_linear_create(C.byref(h), N, Lbox, nf, C.byref(mp), order, dt)
+
+    for bad in (dict(N=2), dict(Lbox=-1.0), dict(nf=5), dict(order=3), dict(dt=0.0), dict(model=9),
+                dict(model=binding.CHAOTIC, nf=1), dict(model=binding.OSCILLON, nf=2), dict(mpl=-1.0),
+                dict(stencil=(-5.0, 1.0, 0.0, 0.0)), dict(precision=32)):
+        assert create(**bad) == binding.EINVAL, bad
+        assert h.value is None and len(L.pycool_linear_last_error(None)) > 0
+    for N in (3, 4, 7, 8, 256, 1024):
+        M = N // 2
+        assert L.pycool_linear_num_classes(N) == (M + 1) * (M + 2) * (M + 3) // 6
+    assert L.pycool_linear_num_classes(2) == 0
+    if not torch.cuda.is_available():
+        assert create() == binding.ECUDA
+        with pytest.raises(RuntimeError):
+            binding.LinearLattice(8, 1.0, 1, binding.FREE, (1.0,))
+    assert L.pycool_linear_step(None, 1, 0) == binding.EINVAL and L.pycool_linear_destroy(None) == binding.EINVAL
 
 
 def test_stage_weights_host_logic(L, golden_dir):

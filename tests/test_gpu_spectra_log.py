@@ -49,16 +49,17 @@ def test_mode_spectra_match_the_oracle(pc, N, precision, stencil):
     po, qo = o.read_fields()
     a = o.energies().a
     st = DEFAULT_STENCIL if stencil == (0, 0, 0, 0) else stencil
-    tol = 1e-10 if precision == 64 else 2e-4
+    # fp32 fields: the removed zero mode comes back at the rounding level of a float (1e-8 of the spectrum's peak)
+    tol, floor = (1e-10, 1e-300) if precision == 64 else (2e-4, 1e-8)
     for f, m2 in ((0, 1.0), (1, 1.0e4 * 0.9676 ** 2)):
         want_n, want_e, want_c = spectra.mode_spectra(po[f].astype(np.float64), qo[f].astype(np.float64), cfg["L"], a, m2, st)
         got_n, got_e, got_c = g.mode_spectra(f, m2)
         assert len(got_c) == len(want_c) and np.array_equal(got_c, want_c) and got_c.sum() == N ** 3
-        assert np.max(np.abs(got_n - want_n) / (np.abs(want_n) + 1e-300)) < tol, f
-        assert np.max(np.abs(got_e - want_e) / (np.abs(want_e) + 1e-300)) < tol, f
+        assert np.max(np.abs(got_n - want_n) / (np.abs(want_n) + floor * want_n.max())) < tol, f
+        assert np.max(np.abs(got_e - want_e) / (np.abs(want_e) + floor * want_e.max())) < tol, f
         # a short output: the shells beyond nbins are dropped, the others unchanged
         n8, e8, c8 = g.mode_spectra(f, m2, nbins=8)
-        assert np.array_equal(c8, want_c[:8]) and np.max(np.abs(n8 - want_n[:8]) / want_n[:8]) < tol
+        assert np.array_equal(c8, want_c[:8]) and np.max(np.abs(n8 - want_n[:8]) / (want_n[:8] + floor * want_n.max())) < tol
 
 
 def test_energy_spectrum_sums_to_the_energies_on_the_device(pc):
@@ -90,8 +91,10 @@ def test_spectrum_argument_checks(pc):
     with pytest.raises(pc.PycoolError) as ei:
         g.field_spectrum(0, 0, nbins=4096)                   # more than 48 KB of shared-memory histogram
     assert ei.value.code == pc.EINVAL
-    n, e, c = g.mode_spectra(0, 0.0)                         # massless: the zero mode has w = 0 -> n = 0, rho = |v|^2/2 = 0
-    assert n[0] == 0.0 and e[0] == 0.0 and c[0] == 1
+    # massless: the zero mode has w^2 = k_eff^2(0)/dx^2 = 0 up to the rounding of c0 + 6 c1 + 12 c2 + 8 c3 (1e-16), so
+    # n = 0 and rho = |v|^2/2 + w^2 |u|^2/2 = 0 to that rounding
+    n, e, c = g.mode_spectra(0, 0.0)
+    assert n[0] == 0.0 and abs(e[0]) < 1e-13 and c[0] == 1
 
 
 # ------------------------------------------------------------------------------------- energy log
@@ -103,7 +106,8 @@ def test_energy_log_entries_are_the_synchronous_read_outs(pc, name, N, precision
     of an unlogged run -- the log does not touch the step sequence; (ii) every entry is bitwise what pycool_energies
     returns for a run stopped at that step (the flushed state and the on-the-fly closing drift see the same phi);
     (iii) each entry matches the oracle at that step.  TMA kernel (even N) and plain kernel (odd N)."""
-    cfg = inputs.config(name, N=N)
+    # cfg0's literal dt = L/N/20 is stable at N = 32 only (reading G19): the other sizes take the resolved step
+    cfg = inputs.config(name, N=N) if (name != "cfg0_chaotic32" or N == 32) else inputs.config(name, N=N, dt=0.0025)
     cfg["L"] = cfg["L"] * N / inputs.config(name)["N"] if name != "cfg0_chaotic32" else cfg["L"]
     nf = cfg["nfields"]
     phi, pi = inputs.make_initial(cfg, precision=precision)
@@ -144,7 +148,7 @@ def test_energy_log_entries_are_the_synchronous_read_outs(pc, name, N, precision
 
 
 def test_energy_log_ring_and_switch_off(pc):
-    cfg = inputs.config("cfg0_chaotic32", N=16)
+    cfg = inputs.config("cfg0_chaotic32", N=16, dt=0.0025)        # L/N/20 is unstable below N = 32 (reading G19)
     phi, pi = inputs.make_initial(cfg)
     g = pc.from_config(cfg)
     g.set_fields(phi, pi); g.set_background(1.0)
