@@ -52,11 +52,13 @@ def parse():
     ap.add_argument("--precision", type=int, default=64, choices=[32, 64])
     ap.add_argument("--tile", type=int, default=-1)
     ap.add_argument("--zchunk", type=int, default=0)
+    ap.add_argument("--item-order", type=int, default=-1, help="tiles per region of the item order (0: plain x-y-z; -1: library's)")
     ap.add_argument("--persistent", type=int, default=-1, help="1/0: persistent launch of the TMA kernel on/off (default: library's)")
     ap.add_argument("--fused-tail", type=int, default=-1, help="1/0: fused stage tail on/off (default: library's)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-init", action="store_true", help="skip the on-device initial-conditions timing")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-linear", action="store_true", help="skip the linearised-solver block (SURVEY 8(f) rank 4)")
     ap.add_argument("--device-init", action="store_true",
                     help="initial conditions from pycool_init_fields instead of host arrays (no e2e): for 1024^3 captures")
     ap.add_argument("--sweep", default=None, choices=["cfg4"], help="print the configs[4] matrix, one JSON line per cell")
@@ -77,7 +79,7 @@ COUNTER_COLUMNS = ("dram_bytes", "duration_us", "dram_pct", "fp64_pct", "issue_p
 
 
 def geometry_key(workload, precision, geo):
-    return "%s/fp%d/tile%d/zc%d" % (workload, precision, geo["variant"], geo["zchunk"])
+    return "%s/fp%d/tile%d/zc%d/region%dx%d" % ((workload, precision, geo["variant"], geo["zchunk"]) + tuple(geo["region"]))
 
 
 def recorded_counters(key):
@@ -269,6 +271,45 @@ def roofline_block(lat, workload, precision, N, nf, steps, barrier):
     return roof
 
 
+def linear_block(dev, N=256, steps=20):
+    """SURVEY 8(f) rank 4, on demand: the linearised solver (include/pycool_linear.h) on the two-field chaotic model,
+    N^3 modes, order 4: `steps` steps through the growth matrices (2.51) against the same steps with every mode on
+    its own -- the comparison behind the paper's "roughly 15 times faster".  Device times of the
+    kernels from CUDA events inside the library; second of two identical calls."""
+    import numpy as np
+    from paper_1201_5029_b200 import binding
+    peak, _ = measured_peaks()
+    out = {"workload": "chaotic model, %d^3, 2 fields, order 4, %d steps per call" % (N, steps)}
+    rng = np.random.default_rng(11)
+    shape = (2, N, N, N // 2 + 1)
+    P = (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)) * 1e-6
+    for name, method in (("growth", binding.GROWTH), ("naive", binding.NAIVE)):
+        g = binding.LinearLattice(N, 10.0, 2, binding.CHAOTIC, (1.0, 1.0e4), order=4, dt=10.0 / N / 20.0, device=dev)
+        g.set_background(1.0, float("nan"), (0.9676, 0.0), (-0.71371, 0.0))
+        g.set_modes(P, P)
+        g.step(steps, method)
+        g.step(steps, method)
+        t = g.time_ms()
+        t["total"] = t["background"] + t["growth"] + t["modes"]
+        out[name + "_ms"] = t
+        if method == binding.GROWTH:
+            nmodes, ncls = N * N * (N // 2 + 1), g.nclasses
+            # lin_apply: 2 nf complex read + written per mode, one (2 nf)^2 matrix read per class (the gathers of the
+            # ~23 modes of a class hit L2)
+            alg = nmodes * 4 * 16 * 2 + ncls * 16 * 8
+            out["apply"] = {"algorithmic_bytes": alg, "achieved": alg / (t["modes"] * 1e-3) / 1e9, "unit": "GB/s",
+                            "frac": alg / (t["modes"] * 1e-3) / 1e9 / peak, "bound": "hbm"}
+            # lin_growth: per class, column and stage 2 nf + nf (1 + nf) = 10 fp64 FMAs (nf = 2)
+            fma = ncls * 4 * steps * 3 * 10
+            out["growth_kernel"] = {"fp64_fma": fma, "achieved": 2 * fma / (t["growth"] * 1e-3) / 1e12, "unit": "TFLOP/s",
+                                    "bound": "alu"}
+            out["classes"], out["modes"] = ncls, nmodes
+        g.close()
+    out["speedup_growth_over_naive"] = out["naive_ms"]["total"] / out["growth_ms"]["total"]
+    out["paper"] = "roughly 15 times faster than the naive version (PAPER.md:403, Fermi-class GPU)"
+    return out
+
+
 def sweep_cfg4(a, dev, barrier):
     """BASELINE.json configs[4]: the two-field chaotic model at 512^3 and 1024^3, fp64 and fp32, order 2/4/6, 50
     steps each.  Initial conditions are generated on the device (pycool_init_fields: no 34 GB host arrays), so the
@@ -373,6 +414,8 @@ def main():
         lat.set_tile(a.tile)
     if a.zchunk > 0:
         lat.set_zchunk(a.zchunk)
+    if a.item_order >= 0:
+        lat.set_item_order(a.item_order)
     if a.persistent >= 0:
         lat.set_persistent(a.persistent)
     if a.fused_tail >= 0:
@@ -475,6 +518,8 @@ def main():
         line["init_fields"] = init
     if e2e:
         line["e2e"] = e2e
+    if not a.no_linear and world == 1:
+        line["linear"] = linear_block(dev)
     if not a.no_cpu_baseline and world == 1:
         stages = {2: 1, 4: 3, 6: 7, 8: 15}[order]
         v, _, sample = time_oracle(cfg, order, max(1, round(100 / stages)), 1, a.precision)     # ~13 s of CPU work

@@ -231,8 +231,9 @@ int pycool_kick_time_ms(pycool_ctx*, double* total_ms, unsigned long long* launc
  * tile[4] = work items (x-y tile, z-chunk) per launch -- the grid size of a one-block-per-item launch; a persistent
  * launch uses min(items, resident blocks) blocks; tile[5] = dynamic shared memory bytes; tile[6] = variant index
  * (pycool_set_tile);
- * tile[7] = TMA ring stages (0 = the register-prefetch kernel). */
-int pycool_kick_geometry(const pycool_ctx*, int tile[8]);
+ * tile[7] = TMA ring stages (0 = the register-prefetch kernel); tile[8], tile[9] = region of the item order in tiles
+ * (x: always the whole row; y: rows per region; pycool_set_item_order; the whole x-y tile grid = plain order). */
+int pycool_kick_geometry(const pycool_ctx*, int tile[10]);
 /* Override the z-chunk length (planes per block; 0 = automatic) before the next step. */
 int pycool_set_zchunk(pycool_ctx*, int planes);
 /* Fused stage tail (default on): the block of a drift+kick launch that finishes last adds the per-block partial
@@ -244,6 +245,14 @@ int pycool_set_fused_tail(pycool_ctx*, int on);
  * the current stage drains and wait (griddepcontrol.wait) until it has completed before they read anything it
  * wrote.  Hides launch latency and prologue on small lattices; results are unchanged. */
 int pycool_set_overlap(pycool_ctx*, int on);
+/* Order in which the persistent TMA-fed kernel hands out its work items (x-y tile, z-chunk).  -1 (default): the x-y
+ * tile grid is cut into regions of whole tile rows holding about as many tiles as there are blocks in flight, and a
+ * region is taken through ALL its z-chunks before the next region, so the blocks that finish z-chunk k of a region
+ * go on with z-chunk k+1 of the same tiles and the two planes consecutive chunks share are read from L2 the second
+ * time; 0: plain order (every tile of z-chunk 0, then z-chunk 1, ...); n > 0: regions of about n tiles.
+ * Fields do not depend on the order; the lattice sums are added in item-index order, so they change in the last
+ * bits with it (each order is reproducible bit for bit). */
+int pycool_set_item_order(pycool_ctx*, int tiles_per_region);
 /* pycool_energies kernel: 1 (default) = TMA-fed z-march (even N, at most two fields; sum_x G[phi] through the paper's
  * identity (2.17), sum_x G = -sum_x psi D[psi] with psi = phi - one lattice-wide reference value per field);
  * 0 = the plain one-thread-per-site kernel that evaluates (2.8) term by term (always used for odd N or more than two

@@ -22,7 +22,7 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
-           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_init_fields",
+           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_set_item_order", "pycool_init_fields",
            "pycool_field_spectrum", "pycool_mode_spectra", "pycool_set_energy_cadence", "pycool_read_energy_log",
            # include/pycool_linear.h
            "pycool_linear_create", "pycool_linear_num_classes", "pycool_linear_set_background",
@@ -111,6 +111,7 @@ def lib():
         L.pycool_set_adaptive.argtypes = [vp, ip]
         L.pycool_set_energy_kernel.argtypes = [vp, ip]
         L.pycool_set_overlap.argtypes = [vp, ip]
+        L.pycool_set_item_order.argtypes = [vp, ip]
         L.pycool_field_spectrum.argtypes = [vp, ip, ip, ip, C.POINTER(d), C.POINTER(d)]
         L.pycool_init_fields.argtypes = [vp, C.c_ulonglong, C.POINTER(Spectrum), C.POINTER(Spectrum)]
         L.pycool_mode_spectra.argtypes = [vp, ip, d, ip, C.POINTER(d), C.POINTER(d), C.POINTER(d)]
@@ -341,10 +342,10 @@ class Lattice:
         return ms.value, int(n.value)
 
     def kick_geometry(self):
-        t = (C.c_int * 8)()
+        t = (C.c_int * 10)()
         self._chk(lib().pycool_kick_geometry(self._h, t))
         return dict(tx=t[0], ty=t[1], zchunk=t[2], threads=t[3], blocks=t[4], items=t[4], smem_bytes=t[5], variant=t[6],
-                    tma_stages=t[7])
+                    tma_stages=t[7], region=(t[8], t[9]))
 
     def set_zchunk(self, planes):
         self._chk(lib().pycool_set_zchunk(self._h, planes))
@@ -355,6 +356,10 @@ class Lattice:
 
     def set_overlap(self, on=True):
         self._chk(lib().pycool_set_overlap(self._h, 1 if on else 0))
+
+    def set_item_order(self, tiles_per_region=-1):
+        """-1: automatic regions; 0: plain x-y-z order; n: regions of about n tiles (pycool_set_item_order)."""
+        self._chk(lib().pycool_set_item_order(self._h, int(tiles_per_region)))
 
     def set_energy_kernel(self, tma=True):
         self._chk(lib().pycool_set_energy_kernel(self._h, 1 if tma else 0))

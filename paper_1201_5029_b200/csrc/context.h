@@ -75,6 +75,8 @@ struct pycool_ctx {
   // launch geometry
   int tile = -1, zc = 0, zc_user = 0;
   dim3 grid;
+  int region[2] = {1, 1};       // kick_tma item order: regions of region[0] x region[1] tiles (kick_tma.cuh: item_origin)
+  int region_user = -1;         // pycool_set_item_order: -1 automatic, 0 plain x-y-z order, n > 0 about n tiles per region
   // state
   bool have_fields = false, nonfinite_seen = false;
   bool pending_drift = false;   // the closing half drift of the last step call is still to be applied to phi

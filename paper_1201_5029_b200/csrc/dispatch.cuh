@@ -12,7 +12,8 @@ using Tile0 = Tile<32, 8, 2>;
 using Tile1 = Tile<32, 16, 2>;
 using Tile2 = Tile<64, 8, 2>;
 // kick_tma variants: <TX, TY, ring stages, rows per thread J, blocks per SM the registers are cut for>.
-// (Tried and dropped, profiles/r1c: ring of 4, 512-thread 2 x 1-site blocks, 64 x 32 tiles -- never faster.)
+// (Tried and dropped, profiles/: ring of 4, 512-thread 2 x 1-site blocks, 64 x 32 tiles; for the Q-ball model a ring of
+// 2 with three blocks per SM at 80 registers (620 bytes of spills): 384 us against 245 -- never faster.)
 template <typename Real> using TTile3 = TmaTile<Real, 64, 16, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 256 thr x (2 x 2 sites)
 template <typename Real> using TTile4 = TmaTile<Real, 32, 16, 3, 2, 1>;   // 128 threads x (2 x 2 sites): small N
 template <typename Real> using TTile5 = TmaTile<Real, 128, 8, 3, 2, sizeof(Real) == 4 ? 2 : 1>;   // 1 KB rows
@@ -108,6 +109,7 @@ int launch_tma_t(pycool_ctx* c) {
   g.zc = c->zc;
   g.nbx = (int)c->grid.x; g.nby = (int)c->grid.y;
   g.nitems = (int)(c->grid.x * c->grid.y * c->grid.z);
+  g.ry = c->region[1];
   g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
   g.mp = c->mp;
   // persistent: one block per resident slot, every further item claimed from a device counter (kick_tma.cuh);

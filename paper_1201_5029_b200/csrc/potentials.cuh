@@ -27,7 +27,7 @@ template <> __device__ __forceinline__ float min_normal<float>() { return FLT_MI
 
 // Natural logarithm of a positive finite double, for the Q-ball potential (3.4).  CUDA's log() costs ~150
 // instructions per call in this kernel (slow-path branches, integer work), which made the Q-ball kick ALU-bound;
-// this one is ~45: x = 2^e m with m in [sqrt(1/2), sqrt(2)), s = (m-1)/(m+1), ln m = 2 s sum_k s^(2k)/(2k+1)
+// this one is ~40: x = 2^e m with m in [sqrt(1/2), sqrt(2)), s = (m-1)/(m+1), ln m = 2 s sum_k s^(2k)/(2k+1)
 // (|s| <= 0.1716, 11 terms: truncation 2e-19), ln x = e ln2_hi + (e ln2_lo + ln m) with the two-part ln 2 of
 // fdlibm.  Error <= 2.1 ulp against logl over [1e-300, 1e300], near 1 and at the sqrt 2 switch
 // (tests/test_abi_cpu.py compiles this very function for the host, tests/log_pos_check.cu, and checks it).
@@ -53,7 +53,20 @@ __host__ __device__ __forceinline__ double log_pos(double x) {
   double m;
   memcpy(&m, &bits, sizeof m);
 #endif
-  const double s = (m - 1.0) / (m + 1.0);
+  // s = (m - 1)/(m + 1) without the compiler's division (its slow-path test costs a divergent call per site):
+  // r ~ 1/d from the hardware's 20-bit seed (a float reciprocal on the host), two Newton steps (2^-80), then one
+  // correction of the quotient -- the quotient is within 1 ulp, d = m + 1 is in [1.7, 2.42), nothing can overflow
+  const double d = m + 1.0, n = m - 1.0;
+#if defined(__CUDA_ARCH__)
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+#else
+  double r = (double)(1.0f / (float)d);
+#endif
+  r = fma(fma(-d, r, 1.0), r, r);
+  r = fma(fma(-d, r, 1.0), r, r);
+  double s = n * r;
+  s = fma(fma(-d, s, n), r, s);
   const double z = s * s;
   // sum_{k=0..10} z^k / (2k + 3), Estrin's scheme: 5 dependent operations instead of Horner's 11 (the kick
   // has two of these chains per thread in flight and few warps to hide them behind)

@@ -270,6 +270,22 @@ int set_geometry(pycool_ctx* c) {
   while (3 * (size_t)blocks_xy(c->N, c->tile) * (size_t)((c->N + zc - 1) / zc) > c->partials_cap) ++zc;
   c->zc = zc;
   c->grid = dim3((c->N + t.tx - 1) / t.tx, (c->N + t.ty - 1) / t.ty, (c->N + zc - 1) / zc);
+  // item order (kick_tma.cuh: item_origin): regions of whole tile rows with about as many tiles as there are blocks
+  // in flight (never more), the rows spread evenly over the regions; a layer that does not fit in flight even as a
+  // single row, or a lattice whose whole x-y plane does, keeps the plain x-y-z order
+  {
+    const int nbx = (int)c->grid.x, nby = (int)c->grid.y;
+    int ry = nby;
+    if (t.stages > 0 && c->region_user != 0) {
+      int R = (int)dispatch(c, OP_RESIDENT, c->tile);
+      if (R < 1) R = c->sms;
+      const int want = c->region_user > 0 ? c->region_user : R;
+      const int ry_max = std::max(1, want / nbx);
+      const int nreg = (nby + ry_max - 1) / ry_max;
+      ry = (nby + nreg - 1) / nreg;
+    }
+    c->region[0] = nbx; c->region[1] = ry;
+  }
   if (t.stages > 0) return encode_maps(c);
   return PYCOOL_OK;
 }
@@ -990,7 +1006,7 @@ int pycool_kick_time_ms(pycool_ctx* c, double* total_ms, unsigned long long* lau
   return PYCOOL_OK;
 }
 
-int pycool_kick_geometry(const pycool_ctx* c, int tile[8]) {
+int pycool_kick_geometry(const pycool_ctx* c, int tile[10]) {
   if (!c || !tile) return PYCOOL_EINVAL;
   const TileInfo& t = kTiles[c->tile];
   tile[0] = t.tx; tile[1] = t.ty; tile[2] = c->zc; tile[3] = t.nt;
@@ -998,6 +1014,7 @@ int pycool_kick_geometry(const pycool_ctx* c, int tile[8]) {
   tile[5] = (int)dispatch(const_cast<pycool_ctx*>(c), OP_SMEM, c->tile);
   tile[6] = c->tile;
   tile[7] = t.stages;
+  tile[8] = c->region[0]; tile[9] = c->region[1];
   return PYCOOL_OK;
 }
 
@@ -1006,6 +1023,14 @@ int pycool_set_zchunk(pycool_ctx* c, int planes) {
   OnDevice on_device(c);
   if (planes < 0) return fail(c, PYCOOL_EINVAL, "planes < 0");
   c->zc_user = planes;
+  return set_geometry(c);
+}
+
+int pycool_set_item_order(pycool_ctx* c, int tiles_per_region) {
+  if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
+  if (tiles_per_region < -1) return fail(c, PYCOOL_EINVAL, "tiles_per_region must be -1 (automatic), 0 (plain order) or > 0");
+  c->region_user = tiles_per_region;
   return set_geometry(c);
 }
 

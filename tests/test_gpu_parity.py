@@ -270,6 +270,45 @@ def test_fused_tail_equals_separate_scalar_update(pc, tile, N):
     assert rel(ea.a, eb.a) < 1e-14 and rel(ea.p_a, eb.p_a) < 1e-13
 
 
+@pytest.mark.parametrize("tile,N,zc,precision", [(3, 200, 7, 64), (4, 136, 3, 64), (7, 136, 5, 64), (5, 264, 6, 32)])
+def test_item_orders_agree(pc, tile, N, zc, precision):
+    """pycool_set_item_order: the order in which (x-y tile, z-chunk) items are handed out -- plain x-y-z, regions of one
+    tile row, ragged regions (tile rows not divisible by the region height), the automatic regions -- changes which
+    block computes what and the index of every partial sum, nothing else: after one stage the fields are bitwise
+    equal, after several steps every order matches the oracle."""
+    cfg = inputs.config("cfg0_chaotic32", N=N, dt=0.002, order=2)
+    phi, pi = inputs.make_initial(cfg, precision=precision)
+    nrows = lambda g: (N + g.kick_geometry()["ty"] - 1) // g.kick_geometry()["ty"]
+    outs, seen = [], set()
+    for order in (0, 1, -1, 40, 100):
+        g = pc.from_config(cfg, precision=precision)
+        g.set_tile(tile); g.set_zchunk(zc); g.set_item_order(order)
+        geo = g.kick_geometry()
+        assert geo["items"] > 148 * 3 and 1 <= geo["region"][1] <= nrows(g)
+        if order == 0:
+            assert geo["region"][1] == nrows(g)
+        seen.add(geo["region"][1])
+        g.set_fields(phi, pi); g.set_background(1.0)
+        g.step(1)
+        outs.append(g.read_fields())
+    assert len(seen) >= 3                                          # really different orders, one of them ragged
+    for p_, q_ in outs[1:]:
+        assert np.array_equal(p_, outs[0][0]) and np.array_equal(q_, outs[0][1])
+    cfg4 = inputs.config("cfg0_chaotic32", N=N if N < 150 else 72, dt=0.002, order=4)
+    phi, pi = inputs.make_initial(cfg4, precision=precision)
+    for order in (1, 40):
+        g, o = make_pair(pc, cfg4, precision=precision)
+        g.set_tile(tile); g.set_zchunk(3); g.set_item_order(order)
+        start(g, o, phi, pi)
+        g.step(2); o.step(2)
+        if precision == 64:
+            compare(g, o, 2, 2e-12)
+        else:       # fp32 fields: the gradient energy of 1e-6 fluctuations is not resolved to 1e-5; fields and a are
+            (pg, qg), (po, qo) = g.read_fields(), o.read_fields()
+            assert rel_err_per_site(pg, po) <= 2e-5 and rel_err_per_site(qg, qo) <= 2e-5
+            assert rel(g.energies().a, o.energies().a) <= 1e-6
+
+
 @pytest.mark.parametrize("tile,N,zc", [(3, 136, 5), (4, 70, 1), (5, 260, 4), (7, 136, 1), (8, 72, 1)])
 def test_persistent_launch_is_bitwise_the_one_block_per_item_launch(pc, tile, N, zc):
     """More work items than resident blocks (short z-chunks): every block walks several items with its TMA ring
