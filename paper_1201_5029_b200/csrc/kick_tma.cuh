@@ -95,7 +95,7 @@ struct TmaArgs {
   double* partials;       // [3][nitems]: SD, SV, Spi2
   StageTail tail;         // fused reduction + scalar update by the last block
   Layout L;
-  int zc;                 // planes per z-chunk
+  int zc;                 // planes per z-chunk, at most (chunks are balanced: item_origin)
   int nbx, nby, nitems;   // work items = (x tile, y tile, z chunk): nitems = nbx nby nbz
   int ry;                 // item order: regions of ry rows of tiles, see item_origin (ry = nby: plain x-y-z order)
   double c1, c2, c3;
@@ -111,8 +111,10 @@ struct TmaArgs {
 // order (ry = nby) the second read comes ~1.7 rounds (> 300 MB of traffic) later, always from DRAM: 12.5 % of the
 // reads at 16-plane chunks (measured at 512^3: 4.88 -> 4.40 GB read per launch, 1.454 -> 1.405 ms, profiles/r2).
 // Blocks in flight are still x-y neighbours within their layer (halo rows hit L2 as before).
+// z-chunks are balanced: chunk bz of nbz owns planes [bz N / nbz, (bz + 1) N / nbz), lengths differing by one at most
+// (128^3 on 148 SMs: 9 chunks of 14-15 planes x 16 tiles = 144 items in one round, instead of 8 x 16).
 template <typename Real, int TX, int TY>
-__device__ __forceinline__ void item_origin(const TmaArgs<Real>& g, int item, int& x0, int& y0, int& z0) {
+__device__ __forceinline__ void item_origin(const TmaArgs<Real>& g, int item, int& x0, int& y0, int& z0, int& nz) {
   const int nbz = g.nitems / (g.nbx * g.nby);
   const int per_region = g.ry * g.nbx * nbz;                   // every region but the last is full
   const int reg = item / per_region, r = item - reg * per_region;
@@ -120,7 +122,9 @@ __device__ __forceinline__ void item_origin(const TmaArgs<Real>& g, int item, in
   const int layer = min(g.ry, g.nby - row0) * g.nbx;           // tiles of one z-layer of this region
   const int bz = r / layer, t = r - bz * layer;
   const int ty = t / g.nbx, tx = t - ty * g.nbx;
-  x0 = tx * TX; y0 = (row0 + ty) * TY; z0 = bz * g.zc;
+  x0 = tx * TX; y0 = (row0 + ty) * TY;
+  z0 = (int)(((long long)bz * g.L.N) / nbz);
+  nz = (int)(((long long)(bz + 1) * g.L.N) / nbz) - z0;
 }
 
 // The z-march of one work item.  EDGE (compile time) = the item touches a lattice face or a ragged edge: only
@@ -357,8 +361,9 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   int claimed = 0x7fffffff;                                    // thread 0: the next item (none unless dyn)
   auto pr_decode = [&]() {
     if (pr_item < g.nitems) {
-      item_origin<Real, TX, TY>(g, pr_item, pr_x0, pr_y0, pr_z0);
-      pr_nload = min(g.zc, N - pr_z0) + 2;
+      int nz_;
+      item_origin<Real, TX, TY>(g, pr_item, pr_x0, pr_y0, pr_z0, nz_);
+      pr_nload = nz_ + 2;
     }
     pr_i = 0;
   };
@@ -430,9 +435,8 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   int cs_seq = 0;
 #pragma unroll 1
   for (int item = blockIdx.x; item < g.nitems; item = item_ring[++cs_seq & 3]) {
-    int x0, y0, z0;
-    item_origin<Real, TX, TY>(g, item, x0, y0, z0);
-    const int nz = min(g.zc, N - z0);
+    int x0, y0, z0, nz;
+    item_origin<Real, TX, TY>(g, item, x0, y0, z0, nz);
     const bool edge_blk = (x0 < L.gx) | (x0 + TX > N - L.gx) | (y0 == 0) | (y0 + TY >= N);
     double sD = 0.0, sV = 0.0, sP = 0.0;
     if (edge_blk)

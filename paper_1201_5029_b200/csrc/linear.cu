@@ -96,6 +96,7 @@ int step_t(pycool_linear_ctx* c, int nsteps, int method) {
   const size_t nst = (size_t)nsteps * c->nstages;
   if (int st = ensure_table(c, nst)) return st;
   LinStage<NF>* table = (LinStage<NF>*)c->table;
+  const size_t plane = (size_t)c->N * (c->N / 2 + 1);          // modes of one i_z plane: the x extent of the mode grids
   LIN_TRY(c, cudaEventRecord(c->ev[0], c->stream));
   lin_background<NF><<<1, 1, 0, c->stream>>>(c->bg, c->k, c->d_w, c->nstages, nsteps, c->dt, table);
   LIN_TRY(c, cudaGetLastError());
@@ -106,13 +107,14 @@ int step_t(pycool_linear_ctx* c, int nsteps, int method) {
         table, nst, c->sc, c->N, c->nclasses, c->M);
     LIN_TRY(c, cudaGetLastError());
     LIN_TRY(c, cudaEventRecord(c->ev[2], c->stream));
-    lin_apply<NF><<<(unsigned)((c->nmodes + kLinThreads - 1) / kLinThreads), kLinThreads, 0, c->stream>>>(
-        c->dPhi, c->dPi, c->M, c->N, c->nmodes);
+    constexpr int kApplyThreads = LinApplyCfg<NF>::NT;
+    lin_apply<NF><<<dim3((unsigned)((plane + kApplyThreads - 1) / kApplyThreads), (unsigned)c->N), kApplyThreads, 0,
+                    c->stream>>>(c->dPhi, c->dPi, c->M, c->N, c->nmodes);
     LIN_TRY(c, cudaGetLastError());
     c->have_growth = true;
   } else {
     LIN_TRY(c, cudaEventRecord(c->ev[2], c->stream));
-    lin_naive<NF><<<(unsigned)((c->nmodes + kLinThreads - 1) / kLinThreads), kLinThreads, 0, c->stream>>>(
+    lin_naive<NF><<<dim3((unsigned)((plane + kLinThreads - 1) / kLinThreads), (unsigned)c->N), kLinThreads, 0, c->stream>>>(
         c->dPhi, c->dPi, table, nst, c->sc, c->N, c->nmodes);
     LIN_TRY(c, cudaGetLastError());
   }

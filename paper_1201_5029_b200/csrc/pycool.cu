@@ -233,14 +233,12 @@ int auto_tile(pycool_ctx* c) {
   return 1;
 }
 
-// Automatic z-chunk.  Short chunks keep the blocks in flight (x-y neighbours) within a few planes of each other,
-// so their halo rows hit L2; each chunk re-reads two halo planes and costs a fixed number of instructions.  Which
-// length wins depends on the board's power state (profiles/r1d): measured cold (a pause before every sample) the
-// fp64 64 x 16 kernel is fastest at 8 planes at 512^3 (1.446 ms; 16: 1.466; 32: 1.508) and 12 at 1024^3, but inside
-// a sustained run (bench.py: 60-140 launches back to back, sw_power_cap) 8 planes lose 7 % (4.83 vs 4.51-4.57
-// ms/step) and 16-24 are level (order 6: 24 best; 1024^3: 24 best, 37.9 vs 38.4 (16) and 39.1 (32) ms/step).
-// Chosen for the sustained case: 16 planes, 24 at N >= 1024; fp32 128 x 8 tile: 24 at 512^3, 16 at 1024^3 (cold:
-// 0.776 vs 0.785 ms, 6.19 vs 6.34 ms).  Small lattices: the chunk length that minimises
+// Automatic z-chunk.  Every chunk marches two halo planes on top of its own (instructions and L2 traffic; since the
+// region item order they are no longer DRAM traffic, kick_tma.cuh: item_origin), long chunks let x-y neighbours drift
+// apart (their halo rows then miss L2) and leave fewer items to balance.  Measured inside sustained runs (bench.py,
+// sw_power_cap, profiles/r2): fp64 64 x 16 tile at 512^3: 12 -> 0.903, 16 -> 0.920-0.924, 20 -> 0.931, 24 -> 0.927,
+// 32 -> 0.902 of peak; at 1024^3: 16 -> 0.874, 24 -> 0.886, 32 -> 0.860; fp32 128 x 8 tile at 512^3: 16 -> 0.826,
+// 24 -> 0.848, 32 -> 0.828; at 1024^3: 16 -> 0.794, 24 -> 0.809.  Small lattices: the chunk length that minimises
 // rounds x (planes + 2 halo planes) + pipeline fill over the resident blocks.
 int auto_zchunk(pycool_ctx* c) {
   const int N = c->N, bxy = blocks_xy(N, c->tile);
@@ -248,16 +246,18 @@ int auto_zchunk(pycool_ctx* c) {
   int R = (int)dispatch(c, OP_RESIDENT, c->tile);
   if (R < 1) R = c->sms;
   int cap = 16;
-  if (c->precision == 64 && c->tile == 3) cap = N >= 1024 ? 24 : 16;
-  else if (c->precision == 32 && c->tile == 5) cap = N >= 1024 ? 16 : (N >= 512 ? 24 : 16);
+  if (c->precision == 64 && c->tile == 3) cap = N >= 1024 ? 24 : (N >= 512 ? 20 : 16);
+  else if (c->precision == 32 && c->tile == 5) cap = N >= 512 ? 24 : 16;
   auto items = [&](int zc) { return (long long)bxy * ((N + zc - 1) / zc); };
   if (items(cap) >= 4LL * R) return cap;
   int best = cap < N ? cap : N;
   long long best_cost = -1;
-  for (int zc = 2; zc <= N; zc += 2) {                        // tiny lattices: a few planes per block
-    const long long rounds = (items(zc) + R - 1) / R;
-    const long long cost = rounds * (zc + 2) + 4;
-    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = zc; }
+  for (int zc = N; zc >= 2; --zc) {                           // small lattices: few planes per block; chunks are
+    const int nbz = (N + zc - 1) / zc;                        // balanced, so what counts is the longest, ceil(N / nbz)
+    const int len = (N + nbz - 1) / nbz;
+    const long long rounds = ((long long)bxy * nbz + R - 1) / R;
+    const long long cost = rounds * (len + 2) + 4;
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = len; }
   }
   return best;
 }

@@ -685,3 +685,61 @@ def test_context_on_a_second_device(pc):
         outs.append(g.read_fields())
     assert torch.cuda.current_device() == 0
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+# ------------------------------------------------------------------------------------- memory safety without a sanitizer
+@pytest.mark.parametrize("name,N,tile,zc,precision", [("cfg0_chaotic32", 72, 3, 5, 64), ("cfg0_chaotic32", 40, 4, 3, 64),
+                                                      ("cfg0_chaotic32", 72, 5, 7, 32), ("cfg3_qball256", 40, 7, 3, 64),
+                                                      ("cfg2_oscillon256", 130, 9, 9, 64), ("cfg0_chaotic32", 21, -1, 0, 64)])
+def test_nothing_is_written_outside_the_work_buffer_and_nothing_uninitialised_is_read(pc, name, N, tile, zc, precision):
+    """compute-sanitizer is closed on this pool (profiles/r2_sanitizer.md), so the two properties it would check are
+    tested directly through the C ABI with a caller-owned work buffer (pycool_create_ext): (i) guard bands of 1 MiB on
+    both sides of the buffer, filled with a byte pattern, are intact after uploads, steps with the energy log, both
+    energy kernels, spectra and downloads; (ii) the buffer itself starts as NaN bytes (0xFF), so any element the
+    library reads without having written it first would surface as a non-finite field or sum."""
+    import ctypes as C
+    import torch
+    cfg = inputs.config(name, N=N, order=2) if name != "cfg0_chaotic32" else inputs.config(name, N=N, order=2, dt=0.0025)
+    if name != "cfg0_chaotic32":
+        cfg["L"] = cfg["L"] * N / inputs.config(name)["N"]
+    nf = cfg["nfields"]
+    phi, pi = inputs.make_initial(cfg, precision=precision)
+    need = pc.work_bytes(N, nf, precision)
+    guard = 1 << 20
+    buf = torch.full((need + 2 * guard + 256,), 0xFF, dtype=torch.uint8, device="cuda:0")
+    base = (buf.data_ptr() + guard + 255) // 256 * 256
+    off = base - buf.data_ptr()
+    buf[:off] = 0xA5
+    buf[off + need:] = 0xA5
+    L = pc.lib()
+    mp = pc.make_params(cfg["model"], cfg["p"], mpl=cfg["mpl"], rho_gamma0=cfg["rho_gamma0"], rho_m0=cfg["rho_m0"],
+                        precision=precision)
+    h = C.c_void_p()
+    stream = torch.cuda.current_stream()
+    assert L.pycool_create_ext(C.byref(h), N, cfg["L"], nf, C.byref(mp), 2, cfg["dt"], base, need, stream.cuda_stream) == 0
+    try:
+        if tile >= 0:
+            assert L.pycool_set_tile(h, tile) == 0
+        if zc > 0:
+            assert L.pycool_set_zchunk(h, zc) == 0
+        assert L.pycool_set_fields(h, phi.ctypes.data, pi.ctypes.data) == 0
+        assert L.pycool_set_background(h, 1.0, math.nan) == 0
+        assert L.pycool_set_energy_cadence(h, 1, 4) == 0
+        assert L.pycool_step(h, 2) == 0 and L.pycool_step(h, 1) == 0
+        e = pc.Energy()
+        assert L.pycool_energies(h, C.byref(e)) == 0
+        assert L.pycool_set_energy_kernel(h, 0) == 0 and L.pycool_energies(h, C.byref(e)) == 0
+        if N % 2 == 0:
+            nb = int(math.floor(math.sqrt(3.0) * N / 2.0 + 0.5)) + 1
+            a, b, c_ = (C.c_double * nb)(), (C.c_double * nb)(), (C.c_double * nb)()
+            assert L.pycool_mode_spectra(h, 0, 1.0, nb, a, b, c_) == 0
+            assert all(math.isfinite(x) for x in a) and all(math.isfinite(x) for x in b)
+        out_phi, out_pi = np.empty_like(phi), np.empty_like(pi)
+        assert L.pycool_read_fields(h, out_phi.ctypes.data, out_pi.ctypes.data) == 0
+    finally:
+        L.pycool_destroy(h)
+    torch.cuda.synchronize()
+    assert bool((buf[:off] == 0xA5).all()) and bool((buf[off + need:] == 0xA5).all())
+    assert np.all(np.isfinite(out_phi)) and np.all(np.isfinite(out_pi))
+    for v in (e.a, e.p_a, e.rho, e.pressure, e.pot) + tuple(e.kin[:nf]) + tuple(e.grad[:nf]):
+        assert math.isfinite(v)
