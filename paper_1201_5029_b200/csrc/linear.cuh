@@ -180,11 +180,11 @@ __device__ __forceinline__ unsigned lin_class_of(int a, int b, int c) {   // any
   return (unsigned)(lin_tet((unsigned)hi) + lin_tri((unsigned)mid) + (unsigned)lo);
 }
 __device__ __forceinline__ void lin_class_triple(unsigned t, int& lo, int& mid, int& hi) {
-  int h = (int)cbrt(6.0 * (double)t);
+  int h = (int)__powf(6.0f * (float)t + 1.0f, 0.33333334f);   // a guess within a few units; corrected below
   while (lin_tet((unsigned)h + 1) <= t) ++h;
   while (h > 0 && lin_tet((unsigned)h) > t) --h;
   const unsigned rem = t - (unsigned)lin_tet((unsigned)h);
-  int m = (int)((sqrt(8.0 * (double)rem + 1.0) - 1.0) * 0.5);
+  int m = (int)((sqrtf(8.0f * (float)rem + 1.0f) - 1.0f) * 0.5f);
   while (lin_tri((unsigned)m + 1) <= rem) ++m;
   while (m > 0 && lin_tri((unsigned)m) > rem) --m;
   hi = h; mid = m; lo = (int)(rem - (unsigned)lin_tri((unsigned)m));
@@ -237,9 +237,9 @@ lin_growth(const LinStage<NF>* __restrict__ table, size_t nst, LinStencil sc, in
            double* __restrict__ M) {
   constexpr int W = 2 + NF * NF, C = 2 * NF;
   __shared__ double sh[kLinChunk * W];
-  const unsigned long long g = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const unsigned t = (unsigned)(g / C);
-  const int col = (int)(g % C);
+  const unsigned g = blockIdx.x * blockDim.x + threadIdx.x;    // < classes x 2 NF <= 1.5e9 at N = 2048
+  const unsigned t = g / C;
+  const int col = (int)(g - t * C);
   const bool live = t < nclasses;
   double k2 = 0.0;
   if (live) {
@@ -319,8 +319,8 @@ lin_apply(double2* __restrict__ dPhi, double2* __restrict__ dPi, const double* _
   double2 v[C];
 #pragma unroll
   for (int i = 0; i < NF; ++i) {
-    v[2 * i] = dPhi[(size_t)i * nmodes + m];
-    v[2 * i + 1] = dPi[(size_t)i * nmodes + m];
+    v[2 * i] = __ldcs(dPhi + (size_t)i * nmodes + m);          // the modes stream through once: evict-first, so that
+    v[2 * i + 1] = __ldcs(dPi + (size_t)i * nmodes + m);       // the matrix table (47 MB at 256^3) stays in L2
   }
   const double2* mat = wmat + lane * STR;
 #pragma unroll
@@ -332,8 +332,8 @@ lin_apply(double2* __restrict__ dPhi, double2* __restrict__ dPi, const double* _
       acc.x = fma(mm.x, v[2 * c2].x, acc.x); acc.y = fma(mm.x, v[2 * c2].y, acc.y);
       acc.x = fma(mm.y, v[2 * c2 + 1].x, acc.x); acc.y = fma(mm.y, v[2 * c2 + 1].y, acc.y);
     }
-    if (r & 1) dPi[(size_t)(r >> 1) * nmodes + m] = acc;
-    else dPhi[(size_t)(r >> 1) * nmodes + m] = acc;
+    if (r & 1) __stcs(dPi + (size_t)(r >> 1) * nmodes + m, acc);
+    else __stcs(dPhi + (size_t)(r >> 1) * nmodes + m, acc);
   }
 }
 

@@ -54,8 +54,8 @@ __host__ __device__ __forceinline__ double log_pos(double x) {
   memcpy(&m, &bits, sizeof m);
 #endif
   // s = (m - 1)/(m + 1) without the compiler's division (its slow-path test costs a divergent call per site):
-  // r ~ 1/d from the hardware's 20-bit seed (a float reciprocal on the host), two Newton steps (2^-80), then one
-  // correction of the quotient -- the quotient is within 1 ulp, d = m + 1 is in [1.7, 2.42), nothing can overflow
+  // r ~ 1/d from the hardware's seed (>= 20 bits; a float reciprocal on the host), one Newton step (2^-40), then one
+  // correction of the quotient (error 2^-40 x 2^-40) -- within 1 ulp; d = m + 1 is in [1.7, 2.42), nothing can overflow
   const double d = m + 1.0, n = m - 1.0;
 #if defined(__CUDA_ARCH__)
   double r;
@@ -63,7 +63,6 @@ __host__ __device__ __forceinline__ double log_pos(double x) {
 #else
   double r = (double)(1.0f / (float)d);
 #endif
-  r = fma(fma(-d, r, 1.0), r, r);
   r = fma(fma(-d, r, 1.0), r, r);
   double s = n * r;
   s = fma(fma(-d, s, n), r, s);
