@@ -12,7 +12,7 @@
 // periodic image(s) into the ghost columns / rows of the output buffer, which the next stage then reads as plain
 // in-bounds box elements.  z wraps through the box coordinate (one plane per box).  DESIGN.md "TMA path".
 //
-// Thread (tx2, ty2) owns the 2 x 2 sites x = 2 tx2 + {0,1}, y = 2 ty2 + {0,1} of the tile for all NF fields.
+// Thread (txw, tyj) owns XW x J sites of the tile for all NF fields (default 2 x 2: x = 2 txw + {0,1}, y = 2 tyj + {0,1}).
 #pragma once
 #include <cuda.h>
 
@@ -25,6 +25,12 @@ namespace pycool {
 template <typename Real> struct Vec2T;
 template <> struct Vec2T<double> { using type = double2; };
 template <> struct Vec2T<float> { using type = float2; };
+
+// XW consecutive sites along x, moved with one 8- or 16-byte access (float2, double2, float4).
+template <typename Real, int XW>
+struct alignas(XW * sizeof(Real) <= 16 ? XW * sizeof(Real) : 16) VecX {
+  Real v[XW];
+};
 
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -57,19 +63,21 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm,
       : "memory");
 }
 
-// Tile traits.  Thread (tx2, tyj) owns the x pair 2 tx2 + {0,1} of rows J tyj .. J tyj + J-1 for all fields;
+// Tile traits.  Thread (txw, tyj) owns the XW sites XW txw + {0 .. XW-1} of rows J tyj .. J tyj + J-1 for all
+// fields (XW = 2: an x pair; XW = 4: an x quad, fp32 only -- one 16-byte access either way);
 // MINB = blocks per SM the register budget is cut for (__launch_bounds__).
-template <typename Real, int TX_, int TY_, int S_, int J_ = 2, int MINB_ = 1>
+template <typename Real, int TX_, int TY_, int S_, int J_ = 2, int MINB_ = 1, int XW_ = 2>
 struct TmaTile {
-  static constexpr int TX = TX_, TY = TY_, S = S_, J = J_, MINB = MINB_;
+  static constexpr int TX = TX_, TY = TY_, S = S_, J = J_, MINB = MINB_, XW = XW_;
   static constexpr int G = 16 / (int)sizeof(Real);      // box halo / ghost columns on each side (16 bytes)
   static constexpr int PX = TX + 2 * G;                 // box row length
   static constexpr int RY = TY + 2;                     // box rows
   static constexpr int PLANE = PX * RY;                 // box elements per field
-  static constexpr int NT = (TX / 2) * (TY / J);        // threads: 2 x J sites each
+  static constexpr int NT = (TX / XW) * (TY / J);       // threads: XW x J sites each
   static constexpr int HR = (TX + 4) / 2;               // halo pairs in the top (and bottom) box row: x = -2 .. TX+1
   static constexpr int NHP = 2 * HR + 2 * TY;           // ring of halo pairs the stencil reads (x pairs)
-  static_assert(TX % 2 == 0 && TY % J == 0 && (J == 1 || J == 2 || J == 4), "2 x J sites per thread");
+  static_assert(TX % XW == 0 && TY % J == 0 && (J == 1 || J == 2 || J == 4), "XW x J sites per thread");
+  static_assert(XW == 2 || (XW == 4 && sizeof(Real) == 4), "x quads: 16 bytes, so fp32 only");
   static_assert(NT % 32 == 0 && NT <= 1024, "block size");
   static_assert(PX <= 256 && RY <= 256, "TMA box extents");
 };
@@ -137,7 +145,9 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
                                            const Real kD, const Real kV, const Real c0, const Real c1, const Real c2,
                                            const Real c3, const typename Model::template Coef<Real>& coef,
                                            double& sD, double& sV, double& sP) {
-  using R2 = typename Vec2T<Real>::type;
+  using R2 = typename Vec2T<Real>::type;                     // halo ring: always x pairs
+  constexpr int XW = T::XW;
+  using RV = VecX<Real, XW>;                                 // own sites: XW along x, one access
   using SM = TmaSmem<Real, Model, T>;
   constexpr int NF = Model::NF, TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J;
   constexpr int PLANE = T::PLANE;
@@ -146,7 +156,7 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
   const Layout& L = g.L;
   const int N = L.N;
   const int tid = threadIdx.x;
-  const int tx2 = tid % (TX / 2), tyj = tid / (TX / 2);
+  const int txw = tid % (TX / XW), tyj = tid / (TX / XW);
   const size_t plane_b = L.plane * ES, field_b = L.field * ES;
   (void)TY; (void)S; (void)tyj;
 
@@ -158,7 +168,8 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
   // Own sites.  Items that touch no lattice face and no ragged edge (block-uniform test) store through a
   // uniform plane pointer plus a 32-bit per-thread byte offset and nothing else; the others also write the
   // periodic images of their face sites into the ghost columns / rows and predicate ragged sites.
-  const int gx = x0 + 2 * tx2;
+  // (XW never exceeds the ghost width L.gx = 16 bytes of elements, so a group is all image or no image.)
+  const int gx = x0 + XW * txw;
   const bool okx = gx < N;
   int ximg = 0;                                              // element offset of the x image, 0 = none
   if (gx < L.gx) ximg = N; else if (gx >= N - L.gx) ximg = -N;
@@ -174,43 +185,44 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
     yimg[j] = 0;
     if (gy == 0) yimg[j] = (long long)N * L.pitch; else if (gy == N - 1) yimg[j] = -(long long)N * L.pitch;
   }
-  auto store_edge = [&](unsigned char* plane, int j, R2 v) { // one output pair and its periodic images
+  auto store_edge = [&](unsigned char* plane, int j, RV v) { // one output group and its periodic images
     Real* p = reinterpret_cast<Real*>(plane + own_off[j]);
-    *reinterpret_cast<R2*>(p) = v;
+    *reinterpret_cast<RV*>(p) = v;
     if (ximg) {
-      *reinterpret_cast<R2*>(p + ximg) = v;
-      if (ximg2) *reinterpret_cast<R2*>(p - ximg) = v;
+      *reinterpret_cast<RV*>(p + ximg) = v;
+      if (ximg2) *reinterpret_cast<RV*>(p - ximg) = v;
     }
     if (yimg[j]) {
-      *reinterpret_cast<R2*>(p + yimg[j]) = v;
+      *reinterpret_cast<RV*>(p + yimg[j]) = v;
       if (ximg) {
-        *reinterpret_cast<R2*>(p + yimg[j] + ximg) = v;
-        if (ximg2) *reinterpret_cast<R2*>(p + yimg[j] - ximg) = v;
+        *reinterpret_cast<RV*>(p + yimg[j] + ximg) = v;
+        if (ximg2) *reinterpret_cast<RV*>(p + yimg[j] - ximg) = v;
       }
     }
   };
-  auto store_own = [&](unsigned char* plane, int j, R2 v) {  // plain store (st.global.cs measured 9 % slower)
-    if constexpr (!EDGE) *reinterpret_cast<R2*>(plane + own_off[j]) = v;
+  auto store_own = [&](unsigned char* plane, int j, RV v) {  // plain store (st.global.cs measured 9 % slower)
+    if constexpr (!EDGE) *reinterpret_cast<RV*>(plane + own_off[j]) = v;
     else if (valid[j]) store_edge(plane, j, v);
   };
 
-  R2 qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
-  R2 A[NF][J], B[NF][J];                                     // stencil accumulators
+  RV qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
+  RV A[NF][J], B[NF][J];                                     // stencil accumulators
   Real ref[NF];                                              // item-uniform; D annihilates constants
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
     ref[f] = Real(0);
 #pragma unroll
-    for (int j = 0; j < J; ++j) {
-      A[f][j] = B[f][j] = qa_phi[f][j] = qa_pi[f][j] = qb_phi[f][j] = qb_pi[f][j] = R2{Real(0), Real(0)};
-    }
+    for (int j = 0; j < J; ++j)
+#pragma unroll
+      for (int k = 0; k < XW; ++k)
+        A[f][j].v[k] = B[f][j].v[k] = qa_phi[f][j].v[k] = qa_pi[f][j].v[k] = qb_phi[f][j].v[k] = qb_pi[f][j].v[k] = Real(0);
   }
 
   // One plane of the march: cphi/cpi receive plane p, pphi/ppi hold plane p-1 (finalised here).
   // EDGE (compile-time) = the item touches a lattice face or a ragged edge; interior items run a copy of the
   // march without any of the image / validity branches.
-  auto step = [&](const int p, const int par, R2 (&cphi)[NF][J], R2 (&cpi)[NF][J], const R2 (&pphi)[NF][J],
-                  const R2 (&ppi)[NF][J]) {
+  auto step = [&](const int p, const int par, RV (&cphi)[NF][J], RV (&cpi)[NF][J], const RV (&pphi)[NF][J],
+                  const RV (&ppi)[NF][J]) {
     const int s = slot;
     const Real* rphi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA);
     const Real* rpi = reinterpret_cast<const Real*>(raw + (size_t)s * 2 * SM::BOXA + SM::BOXA);
@@ -225,7 +237,7 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
       for (int f = 0; f < NF; ++f) ref[f] = rphi[f * PLANE + PX + G];
     }
 
-    // ---- 1. drift: phi' = phi + c_drift pi (own pairs and halo ring); psi = phi' - ref to shared memory
+    // ---- 1. drift: phi' = phi + c_drift pi (own groups and halo ring); psi = phi' - ref to shared memory
     const bool own_plane = (p >= 0) && (p < nz);
     unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)zwrap(p) * plane_b;
 #pragma unroll
@@ -233,14 +245,17 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
 #pragma unroll
       for (int j = 0; j < J; ++j) {
         const int o = f * PLANE + own_sm + j * PX;
-        const R2 a = *reinterpret_cast<const R2*>(rphi + o);
-        const R2 b = *reinterpret_cast<const R2*>(rpi + o);
-        R2 ph;
-        ph.x = fma(cd, b.x, a.x);
-        ph.y = fma(cd, b.y, a.y);
+        const RV a = *reinterpret_cast<const RV*>(rphi + o);
+        const RV b = *reinterpret_cast<const RV*>(rpi + o);
+        RV ph, ps;
+#pragma unroll
+        for (int k = 0; k < XW; ++k) {
+          ph.v[k] = fma(cd, b.v[k], a.v[k]);
+          ps.v[k] = ph.v[k] - ref[f];
+        }
         cphi[f][j] = ph; cpi[f][j] = b;
         if (own_plane) store_own(ophi + f * field_b, j, ph);
-        *reinterpret_cast<R2*>(pb + o) = R2{ph.x - ref[f], ph.y - ref[f]};
+        *reinterpret_cast<RV*>(pb + o) = ps;
       }
 #pragma unroll
       for (int k = 0; k < NHT; ++k)
@@ -255,34 +270,31 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
     issue_next(s);
 
     // ---- 2. in-plane sums of plane p; 3. finalise plane p-1
-    R2 D[NF][J];
+    RV D[NF][J];
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       const Real* sp = pb + f * PLANE + own_sm - PX;         // row above the first own row
-      Real Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];       // x-output 0 and 1: side sums and centres
+      Real Sd[J + 2][XW], Ce[J + 2][XW];                     // per row and x-output: side sum (left + right), centre
 #pragma unroll
       for (int r = 0; r < J + 2; ++r) {
-        const Real l = sp[r * PX - 1];
-        const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
-        const Real rr = sp[r * PX + 2];
-        Rx[r] = l + m.y; Cx[r] = m.x;
-        Ry[r] = m.x + rr; Cy[r] = m.y;
+        Real e[XW + 2];                                      // x = -1 .. XW of this row
+        e[0] = sp[r * PX - 1];
+        const RV m = *reinterpret_cast<const RV*>(sp + r * PX);
+#pragma unroll
+        for (int k = 0; k < XW; ++k) e[k + 1] = m.v[k];
+        e[XW + 1] = sp[r * PX + XW];
+#pragma unroll
+        for (int k = 0; k < XW; ++k) { Sd[r][k] = e[k] + e[k + 2]; Ce[r][k] = e[k + 1]; }
       }
 #pragma unroll
       for (int j = 0; j < J; ++j) {
-        {
-          const Real P0 = Cx[j + 1], P1 = Rx[j + 1] + (Cx[j] + Cx[j + 2]), P2 = Rx[j] + Rx[j + 2];
-          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0)); // weight of plane p in outputs p-1 and p+1
-          D[f][j].x = A[f][j].x + up;                        // output p-1 complete
-          A[f][j].x = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].x)));   // + weight of plane p in output p
-          B[f][j].x = up;
-        }
-        {
-          const Real P0 = Cy[j + 1], P1 = Ry[j + 1] + (Cy[j] + Cy[j + 2]), P2 = Ry[j] + Ry[j + 2];
-          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));
-          D[f][j].y = A[f][j].y + up;
-          A[f][j].y = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].y)));
-          B[f][j].y = up;
+#pragma unroll
+        for (int k = 0; k < XW; ++k) {
+          const Real P0 = Ce[j + 1][k], P1 = Sd[j + 1][k] + (Ce[j][k] + Ce[j + 2][k]), P2 = Sd[j][k] + Sd[j + 2][k];
+          const Real up = fma(c3, P2, fma(c2, P1, c1 * P0));  // weight of plane p in outputs p-1 and p+1
+          D[f][j].v[k] = A[f][j].v[k] + up;                  // output p-1 complete
+          A[f][j].v[k] = fma(c2, P2, fma(c1, P1, fma(c0, P0, B[f][j].v[k])));   // + weight of plane p in output p
+          B[f][j].v[k] = up;
         }
       }
     }
@@ -291,27 +303,22 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
 #pragma unroll
       for (int j = 0; j < J; ++j) {
         if (!EDGE || valid[j]) {
-          Real ph[NF], dV[NF];
-          R2 pn[NF];
+          RV pn[NF];
 #pragma unroll
-          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].x;
-          sV += (double)Model::template eval<Real>(coef, ph, dV);
+          for (int k = 0; k < XW; ++k) {
+            Real ph[NF], dV[NF];
 #pragma unroll
-          for (int f = 0; f < NF; ++f) {
-            pn[f].x = fma(kD, D[f][j].x, fma(-kV, dV[f], ppi[f][j].x));   // pi' = pi + kD D - kV dV
-            sD = fma((double)ph[f], (double)D[f][j].x, sD);
-            sP = fma((double)pn[f].x, (double)pn[f].x, sP);
+            for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].v[k];
+            sV += (double)Model::template eval<Real>(coef, ph, dV);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+              pn[f].v[k] = fma(kD, D[f][j].v[k], fma(-kV, dV[f], ppi[f][j].v[k]));   // pi' = pi + kD D - kV dV
+              sD = fma((double)ph[f], (double)D[f][j].v[k], sD);
+              sP = fma((double)pn[f].v[k], (double)pn[f].v[k], sP);
+            }
           }
 #pragma unroll
-          for (int f = 0; f < NF; ++f) ph[f] = pphi[f][j].y;
-          sV += (double)Model::template eval<Real>(coef, ph, dV);
-#pragma unroll
-          for (int f = 0; f < NF; ++f) {
-            pn[f].y = fma(kD, D[f][j].y, fma(-kV, dV[f], ppi[f][j].y));
-            sD = fma((double)ph[f], (double)D[f][j].y, sD);
-            sP = fma((double)pn[f].y, (double)pn[f].y, sP);
-            store_own(opi + f * field_b, j, pn[f]);
-          }
+          for (int f = 0; f < NF; ++f) store_own(opi + f * field_b, j, pn[f]);
         }
       }
     }
@@ -338,7 +345,7 @@ __global__ void __launch_bounds__(T::NT, T::MINB)
 kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUtensorMap tm_pi,
          const TmaArgs<Real> g) {
   using SM = TmaSmem<Real, Model, T>;
-  constexpr int TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J;
+  constexpr int TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J, XW = T::XW;
 
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* base = smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u);
@@ -350,7 +357,7 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   const Layout& L = g.L;
   const int N = L.N;
   const int tid = threadIdx.x;
-  const int tx2 = tid % (TX / 2), tyj = tid / (TX / 2);
+  const int txw = tid % (TX / XW), tyj = tid / (TX / XW);
 
   // ---- producer: the stream of loads, item after item, planes z0-1 .. z0+nz of each.  Every thread keeps the
   // (block-uniform) bookkeeping; only thread 0 touches the barriers, the TMA unit and the claim counter.
@@ -417,7 +424,7 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
 
   // box offsets: own pair of row j, and the halo pair(s) of this thread (top and bottom box rows x = -2 ..
   // TX+1, and the pairs left and right of every own row; 16-byte accesses, the outer element is unused)
-  const int own_sm = (J * tyj + 1) * PX + G + 2 * tx2;
+  const int own_sm = (J * tyj + 1) * PX + G + XW * txw;
   constexpr int NHT = (T::NHP + NT - 1) / NT;                  // halo pairs per thread
   int halo_sm[NHT];
 #pragma unroll

@@ -76,10 +76,10 @@ int pycool::fail(pycool_ctx* c, int code, const char* fmt, ...) {
 }
 
 //                                 generic kick_fused          | kick_tma (TX, TY, threads, ring stages)
-const TileInfo pycool::kTiles[kNumTiles] = {{32, 8, 128, 0}, {32, 16, 256, 0}, {64, 8, 256, 0},
-                                            {64, 16, 256, 3}, {32, 16, 128, 3}, {128, 8, 256, 3},
-                                            {128, 16, 512, 3}, {32, 16, 256, 3}, {64, 8, 256, 3}, {128, 16, 256, 3},
-                                            {32, 16, 256, 3}};
+const TileInfo pycool::kTiles[kNumTiles] = {{32, 8, 128, 0, 1}, {32, 16, 256, 0, 1}, {64, 8, 256, 0, 1},
+                                            {64, 16, 256, 3, 2}, {32, 16, 128, 3, 2}, {128, 8, 256, 3, 2},
+                                            {128, 16, 512, 3, 2}, {32, 16, 256, 3, 2}, {64, 8, 256, 3, 2},
+                                            {128, 16, 256, 3, 2}, {32, 16, 256, 3, 2}, {128, 8, 256, 3, 4}};
 
 namespace {
 
@@ -105,7 +105,11 @@ Layout make_layout(int N, int nf, size_t esize) {
   return L;
 }
 
-bool tile_allowed(const Layout& L, int tile) { return tile < kNumGeneric || L.gx > 0; }
+// TMA variants need the ghost layout (even N); x quads need whole quads inside the lattice (N a multiple of 4)
+bool tile_allowed(const Layout& L, int tile) {
+  if (tile < kNumGeneric) return true;
+  return L.gx > 0 && L.N % kTiles[tile].xw == 0;
+}
 
 int auto_tile(pycool_ctx* c);   // after dispatch(): needs the shared-memory size of a variant
 
@@ -212,14 +216,16 @@ long long dispatch(pycool_ctx* c, Op op, int arg) {
 // Automatic variant (measured on B200, profiles/): the register-prefetch kernel where the layout has no ghosts
 // (odd N); else the first TMA variant of a preference list whose ring fits in shared memory.
 //   two fields fp64, one field fp32: 64 x 16 tile; two or more fields fp32: 128 x 8 (512-byte rows; the fp32
-//   instances of both are cut for two blocks per SM, which is what fp32 needs: half the bytes per plane);
+//   instances of both are cut for two blocks per SM, which is what fp32 needs: half the bytes per plane), as x quads
+//   (variant 11: float4 accesses, 4 x 1 sites per thread; 2 % faster than the x pairs of variant 5 in one process at
+//   512^3 and 1024^3, profiles/r2) when N is a multiple of 4;
 //   one field fp64: 128 x 16 with 2 x 4 sites per thread (twice the work per plane and per barrier; a ring of 6
 //   with the 64 x 16 tile gains nothing, so it is the per-plane fixed cost, not the bytes in flight);
 //   Q-ball (the logarithm makes it ALU-heavy): 32 x 16 with 2 x 1 sites per thread, two blocks per SM.
 int auto_tile(pycool_ctx* c) {
   const Layout& L = c->lay;
   if (L.gx == 0) return L.N <= 64 ? 0 : 1;
-  static const int pref_default[] = {3, 4}, pref_one[] = {9, 6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {5, 3, 4},
+  static const int pref_default[] = {3, 4}, pref_one[] = {9, 6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {11, 5, 3, 4},
                    pref_small[] = {4, 10}, pref_many[] = {10, 4};
   const int* pref = pref_default;
   int n = 2;
@@ -227,9 +233,9 @@ int auto_tile(pycool_ctx* c) {
   else if (L.N <= 64) { pref = pref_small; n = 2; }
   else if (c->model == PYCOOL_QBALL && c->precision == 64) { pref = pref_alu; n = 2; }
   else if (c->nf == 1 && c->precision == 64) { pref = pref_one; n = 4; }
-  else if (c->precision == 32 && c->nf >= 2) { pref = pref_f32; n = 3; }
+  else if (c->precision == 32 && c->nf >= 2) { pref = pref_f32; n = 4; }
   for (int i = 0; i < n; ++i)
-    if (dispatch(c, OP_BUILT, pref[i])) return pref[i];
+    if (tile_allowed(L, pref[i]) && dispatch(c, OP_BUILT, pref[i])) return pref[i];
   return 1;
 }
 
@@ -238,7 +244,8 @@ int auto_tile(pycool_ctx* c) {
 // apart (their halo rows then miss L2) and leave fewer items to balance.  Measured inside sustained runs (bench.py,
 // sw_power_cap, profiles/r2): fp64 64 x 16 tile at 512^3: 12 -> 0.903, 16 -> 0.920-0.924, 20 -> 0.931, 24 -> 0.927,
 // 32 -> 0.902 of peak; at 1024^3: 16 -> 0.874, 24 -> 0.886, 32 -> 0.860; fp32 128 x 8 tile at 512^3: 16 -> 0.826,
-// 24 -> 0.848, 32 -> 0.828; at 1024^3: 16 -> 0.794, 24 -> 0.809.  Small lattices: the chunk length that minimises
+// 24 -> 0.848, 32 -> 0.828; at 1024^3: 16 -> 0.794, 24 -> 0.809; its x-quad form (variant 11) is best at 32 planes.
+// Small lattices: the chunk length that minimises
 // rounds x (planes + 2 halo planes) + pipeline fill over the resident blocks.
 int auto_zchunk(pycool_ctx* c) {
   const int N = c->N, bxy = blocks_xy(N, c->tile);
@@ -248,6 +255,7 @@ int auto_zchunk(pycool_ctx* c) {
   int cap = 16;
   if (c->precision == 64 && c->tile == 3) cap = N >= 1024 ? 24 : (N >= 512 ? 20 : 16);
   else if (c->precision == 32 && c->tile == 5) cap = N >= 512 ? 24 : 16;
+  else if (c->precision == 32 && c->tile == 11) cap = N >= 512 ? 32 : 16;
   auto items = [&](int zc) { return (long long)bxy * ((N + zc - 1) / zc); };
   if (items(cap) >= 4LL * R) return cap;
   int best = cap < N ? cap : N;
@@ -1068,7 +1076,7 @@ int pycool_set_tile(pycool_ctx* c, int tile) {
   OnDevice on_device(c);
   if (tile < -1 || tile >= kNumTiles) return fail(c, PYCOOL_EINVAL, "tile must be -1 (auto) .. %d", kNumTiles - 1);
   if (tile >= 0 && !tile_allowed(c->lay, tile))
-    return fail(c, PYCOOL_EINVAL, "tile %d is a TMA variant: it needs the ghost layout (even N >= 4)", tile);
+    return fail(c, PYCOOL_EINVAL, "tile %d is a TMA variant: it needs the ghost layout (even N >= 4; N %% 4 == 0 for x quads)", tile);
   if (tile >= 0 && (size_t)dispatch(c, OP_SMEM, tile) > kMaxSmem)
     return fail(c, PYCOOL_EINVAL, "tile %d needs %zu bytes of shared memory for this model and precision (limit %zu)",
                 tile, (size_t)dispatch(c, OP_SMEM, tile), kMaxSmem);

@@ -152,7 +152,7 @@ def set_tile_or_skip(pc, g, tile):
     try:
         g.set_tile(tile)
     except pc.PycoolError as e:
-        assert e.code == pc.EINVAL and tile in (6, 9) and ("shared memory" in str(e) or "not built" in str(e))
+        assert e.code == pc.EINVAL and tile in (6, 9, 11) and ("shared memory" in str(e) or "not built" in str(e))
         return False
     return True
 
@@ -215,7 +215,7 @@ def test_variants_agree_and_ghost_images_hold(pc, precision):
     cfg["init"], cfg["amp"] = "white", 1e-3
     phi, pi = inputs.make_initial(cfg, precision=precision)
     outs = []
-    for tile in range(11):
+    for tile in range(12):
         g = pc.from_config(cfg, precision=precision)
         if not set_tile_or_skip(pc, g, tile):
             assert precision == 64 or tile == 9
@@ -586,6 +586,41 @@ def test_fp32_one_step(pc, tile):
     check_scalars(g.energies(), o.energies(), 2, tol=1e-5)
 
 
+@pytest.mark.parametrize("N,zc", [(72, 5), (136, 7), (264, 0)])
+def test_fp32_x_quads(pc, N, zc):
+    """Variant 11 (fp32 only): 4 x 1 sites per thread, float4 accesses.  Same per-site arithmetic as the x-pair
+    variants, so after one stage the fields are bitwise those of variant 5; several steps against the fp32 oracle;
+    ragged tiles (N = 72: less than one tile wide; 136, 264: 128 + 8), lattice faces, z-chunks.  Needs N % 4 == 0."""
+    cfg = inputs.config("cfg0_chaotic32", N=N, dt=0.002, order=2)
+    phi, pi = inputs.make_initial(cfg, precision=32)
+    outs = []
+    for tile in (5, 11):
+        g = pc.from_config(cfg, precision=32)
+        g.set_tile(tile); g.set_zchunk(zc)
+        assert g.kick_geometry()["variant"] == tile
+        g.set_fields(phi, pi); g.set_background(1.0)
+        g.step(1)
+        outs.append(g.read_fields())
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    cfg4 = inputs.config("cfg0_chaotic32", N=min(N, 136), dt=0.002, order=4)
+    phi, pi = inputs.make_initial(cfg4, precision=32)
+    g, o = make_pair(pc, cfg4, precision=32)
+    g.set_tile(11); g.set_zchunk(zc)
+    start(g, o, phi, pi)
+    g.step(2); o.step(2)
+    (pg, qg), (po, qo) = g.read_fields(), o.read_fields()
+    assert rel_err_per_site(pg, po) <= 2e-5 and rel_err_per_site(qg, qo) <= 2e-5
+    assert rel(g.energies().a, o.energies().a) <= 1e-6
+    with pytest.raises(pc.PycoolError) as ei:                     # N = 70: even, but not whole quads
+        h = pc.from_config(inputs.config("cfg0_chaotic32", N=70, dt=0.002), precision=32)
+        h.set_tile(11)
+    assert ei.value.code == pc.EINVAL
+    with pytest.raises(pc.PycoolError) as ei:                     # fp64: not built
+        h = pc.from_config(inputs.config("cfg0_chaotic32", N=72, dt=0.002))
+        h.set_tile(11)
+    assert ei.value.code == pc.EINVAL
+
+
 # ------------------------------------------------------------------------------------- full size, bench configs
 def replicate_on_device(arr, r, dev):
     import torch
@@ -611,12 +646,12 @@ def worst_replica_error(big, small_np, r, base, dev):
 FULL_SIZE = [
     ("cfg4_chaotic512", 512, 32, 4, 64, 2e-12, 2, 3),       # the bench default
     ("cfg4_chaotic512", 512, 32, 6, 64, 4e-12, 1, 3),
-    ("cfg4_chaotic512", 512, 32, 4, 32, 1e-5, 1, 5),
+    ("cfg4_chaotic512", 512, 32, 4, 32, 1e-5, 1, 11),       # fp32: x quads
     ("cfg1_chaotic128", 128, 32, 6, 64, 2e-12, 2, 3),       # configs[1]: order 6 at its own size
     ("cfg2_oscillon256", 256, 32, 4, 64, 2e-12, 2, 9),      # configs[2]: one field, 2 x 4 sites per thread
     ("cfg3_qball256", 256, 32, 4, 64, 2 * QBALL_TOL_1STEP, 2, 7),   # configs[3]: QBall x (2 x 1 sites, 2 blocks/SM)
     ("cfg4_chaotic1024", 1024, 32, 4, 64, 2e-12, 1, 3),     # configs[4]: 69 GB of state, byte offsets > 2^34
-    ("cfg4_chaotic1024", 1024, 32, 4, 32, 1e-5, 1, 5),      # 2^31 elements per array
+    ("cfg4_chaotic1024", 1024, 32, 4, 32, 1e-5, 1, 11),     # 2^31 elements per array
 ]
 
 
