@@ -160,10 +160,9 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
   const size_t plane_b = L.plane * ES, field_b = L.field * ES;
   (void)TY; (void)S; (void)tyj;
 
-  auto zwrap = [&](int p) {
-    int gz = z0 + p;
-    return gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
-  };
+  // lattice planes of the outputs p (phi') and p-1 (pi'), carried along the march instead of being wrapped anew
+  // from z0 + p every plane
+  int gz_cur = z0 - 1 < 0 ? z0 - 1 + N : z0 - 1, gz_prev = gz_cur;   // plane p = -1
 
   // Own sites.  Items that touch no lattice face and no ragged edge (block-uniform test) store through a
   // uniform plane pointer plus a 32-bit per-thread byte offset and nothing else; the others also write the
@@ -239,7 +238,7 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
 
     // ---- 1. drift: phi' = phi + c_drift pi (own groups and halo ring); psi = phi' - ref to shared memory
     const bool own_plane = (p >= 0) && (p < nz);
-    unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)zwrap(p) * plane_b;
+    unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)gz_cur * plane_b;
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
 #pragma unroll
@@ -299,7 +298,7 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
       }
     }
     if (p >= 1) {
-      unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)zwrap(p - 1) * plane_b;
+      unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)gz_prev * plane_b;   // plane p-1
 #pragma unroll
       for (int j = 0; j < J; ++j) {
         if (!EDGE || valid[j]) {
@@ -322,6 +321,8 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
         }
       }
     }
+    gz_prev = gz_cur;                                        // on to plane p+1
+    if (++gz_cur == N) gz_cur = 0;
   };
 
 #pragma unroll 1
