@@ -307,6 +307,13 @@ lin_apply(double2* __restrict__ dPhi, double2* __restrict__ dPi, const double* _
   const int lane = threadIdx.x & 31;
   double2* wmat = smat + (threadIdx.x >> 5) * 32 * STR;
   const unsigned cls = live ? lin_class_of(ax, ay, az) : 0u;
+  // the mode loads go out first, so that they and the matrix gather are in flight together
+  double2 v[C];
+#pragma unroll
+  for (int i = 0; i < NF; ++i) {
+    v[2 * i] = live ? __ldcs(dPhi + (size_t)i * nmodes + m) : double2{0.0, 0.0};   // the modes stream through once:
+    v[2 * i + 1] = live ? __ldcs(dPi + (size_t)i * nmodes + m) : double2{0.0, 0.0}; // evict-first, the table stays in L2
+  }
   const double2* Mv = reinterpret_cast<const double2*>(M);
 #pragma unroll
   for (int k = 0; k < MW; ++k) {
@@ -316,12 +323,6 @@ lin_apply(double2* __restrict__ dPhi, double2* __restrict__ dPi, const double* _
   }
   __syncwarp();
   if (!live) return;
-  double2 v[C];
-#pragma unroll
-  for (int i = 0; i < NF; ++i) {
-    v[2 * i] = __ldcs(dPhi + (size_t)i * nmodes + m);          // the modes stream through once: evict-first, so that
-    v[2 * i + 1] = __ldcs(dPi + (size_t)i * nmodes + m);       // the matrix table (47 MB at 256^3) stays in L2
-  }
   const double2* mat = wmat + lane * STR;
 #pragma unroll
   for (int r = 0; r < C; ++r) {
