@@ -107,8 +107,8 @@ int step_t(pycool_linear_ctx* c, int nsteps, int method) {
         table, nst, c->sc, c->N, c->nclasses, c->M);
     LIN_TRY(c, cudaGetLastError());
     LIN_TRY(c, cudaEventRecord(c->ev[2], c->stream));
-    constexpr int kApplyThreads = LinApplyCfg<NF>::NT;
-    lin_apply<NF><<<dim3((unsigned)((plane + kApplyThreads - 1) / kApplyThreads), (unsigned)c->N), kApplyThreads, 0,
+    constexpr int kApplyModes = LinApplyCfg<NF>::MPB;
+    lin_apply<NF><<<dim3((unsigned)((plane + kApplyModes - 1) / kApplyModes), (unsigned)c->N), LinApplyCfg<NF>::NT, 0,
                     c->stream>>>(c->dPhi, c->dPi, c->M, c->N, c->nmodes);
     LIN_TRY(c, cudaGetLastError());
     c->have_growth = true;

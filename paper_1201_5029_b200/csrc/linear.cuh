@@ -285,57 +285,45 @@ __device__ __forceinline__ bool lin_mode_of_thread(int N, size_t& m, int& ax, in
 }
 
 // mode <- M(class of the mode) mode   (2.51).  dPhi, dPi: [NF][nmodes] complex.
-// The matrices are a gather: neighbouring modes belong to different classes, so a thread fetching its own (2 NF)^2
-// doubles makes every warp-wide load touch 32 different lines (measured: L1 95 % busy, 0.57 of the HBM roofline).
-// Instead a warp fetches the 32 matrices of its modes together -- consecutive lanes read consecutive 16 bytes of one
-// matrix, whole lines per request -- into shared memory (row stride odd in 16-byte units: conflict-free), and every
-// lane then reads its own matrix from there.
+// The matrices are a gather: neighbouring modes belong to different classes.  One thread per (mode, row of M): the
+// 2 NF threads of a mode read the 2 NF rows of its matrix -- together one contiguous (2 NF)^2 x 8 bytes, a whole line
+// at NF = 2 -- and each the mode's 2 NF complex values (the same addresses within the group: broadcast), and write one
+// complex each.  No shared memory, no shuffles: a thread-per-mode version fetching its matrix in 8 strided loads kept
+// L1 95 % busy (0.57 of the HBM roofline), one staging the matrices of a warp through shared memory stalled on the
+// shared-memory queue (0.63).  The update is in place, so the block synchronises between its reads and its writes.
 template <int NF> struct LinApplyCfg {
-  static constexpr int C = 2 * NF, MW = C * C / 2;            // double2 per matrix
-  static constexpr int STR = MW | 1;                          // shared-memory row stride, odd
-  static constexpr int NT = NF <= 2 ? 256 : 64;               // threads per block: 32 STR double2 per warp fit 48 KB
+  static constexpr int C = 2 * NF;                            // threads per mode = rows of M
+  static constexpr int NT = 256;
+  static constexpr int MPB = NT / C;                          // modes per block (NF = 3: 42, four threads idle)
 };
 template <int NF>
 __global__ void __launch_bounds__(LinApplyCfg<NF>::NT)
 lin_apply(double2* __restrict__ dPhi, double2* __restrict__ dPi, const double* __restrict__ M, int N, size_t nmodes) {
   using K = LinApplyCfg<NF>;
-  constexpr int C = K::C, MW = K::MW, STR = K::STR;
-  __shared__ double2 smat[(K::NT / 32) * 32 * STR];
-  size_t m;
-  int ax, ay, az;
-  const bool live = lin_mode_of_thread(N, m, ax, ay, az);
-  const int lane = threadIdx.x & 31;
-  double2* wmat = smat + (threadIdx.x >> 5) * 32 * STR;
-  const unsigned cls = live ? lin_class_of(ax, ay, az) : 0u;
-  // the mode loads go out first, so that they and the matrix gather are in flight together
-  double2 v[C];
-#pragma unroll
-  for (int i = 0; i < NF; ++i) {
-    v[2 * i] = live ? __ldcs(dPhi + (size_t)i * nmodes + m) : double2{0.0, 0.0};   // the modes stream through once:
-    v[2 * i + 1] = live ? __ldcs(dPi + (size_t)i * nmodes + m) : double2{0.0, 0.0}; // evict-first, the table stays in L2
-  }
-  const double2* Mv = reinterpret_cast<const double2*>(M);
-#pragma unroll
-  for (int k = 0; k < MW; ++k) {
-    const int e = lane + 32 * k, mi = e / MW, o = e - mi * MW;
-    const unsigned c = __shfl_sync(0xffffffffu, cls, mi);
-    wmat[mi * STR + o] = __ldg(Mv + (size_t)c * MW + o);
-  }
-  __syncwarp();
-  if (!live) return;
-  const double2* mat = wmat + lane * STR;
-#pragma unroll
-  for (int r = 0; r < C; ++r) {
-    double2 acc = {0.0, 0.0};
+  constexpr int C = K::C;
+  const unsigned nxh = (unsigned)N / 2 + 1, plane = (unsigned)N * nxh;
+  const unsigned ml = threadIdx.x / C, row = threadIdx.x - ml * C;
+  const unsigned q = blockIdx.x * K::MPB + ml;                // mode within the i_z plane: iy (N/2 + 1) + ix
+  const int iz = (int)blockIdx.y;
+  const bool live = ml < (unsigned)K::MPB && q < plane;
+  double2 acc = {0.0, 0.0};
+  size_t m = 0;
+  if (live) {
+    const unsigned iy = q / nxh;
+    const int ax = (int)(q - iy * nxh), ay = min((int)iy, N - (int)iy), az = min(iz, N - iz);
+    m = (size_t)iz * plane + q;
+    const double2* mrow = reinterpret_cast<const double2*>(M) + ((size_t)lin_class_of(ax, ay, az) * C + row) * NF;
 #pragma unroll
     for (int c2 = 0; c2 < NF; ++c2) {
-      const double2 mm = mat[r * NF + c2];                     // M[r][2 c2], M[r][2 c2 + 1]
-      acc.x = fma(mm.x, v[2 * c2].x, acc.x); acc.y = fma(mm.x, v[2 * c2].y, acc.y);
-      acc.x = fma(mm.y, v[2 * c2 + 1].x, acc.x); acc.y = fma(mm.y, v[2 * c2 + 1].y, acc.y);
+      const double2 mm = __ldg(mrow + c2);                     // M[row][2 c2], M[row][2 c2 + 1]
+      const double2 u = __ldcs(dPhi + (size_t)c2 * nmodes + m);   // the modes stream through once: evict-first, the
+      const double2 w = __ldcs(dPi + (size_t)c2 * nmodes + m);    // matrix table (47 MB at 256^3) stays in L2
+      acc.x = fma(mm.x, u.x, acc.x); acc.y = fma(mm.x, u.y, acc.y);
+      acc.x = fma(mm.y, w.x, acc.x); acc.y = fma(mm.y, w.y, acc.y);
     }
-    if (r & 1) __stcs(dPi + (size_t)(r >> 1) * nmodes + m, acc);
-    else __stcs(dPhi + (size_t)(r >> 1) * nmodes + m, acc);
   }
+  __syncthreads();                                             // every read of the block before its first write
+  if (live) __stcs(((row & 1) ? dPi : dPhi) + (size_t)(row >> 1) * nmodes + m, acc);
 }
 
 // Every mode through every stage on its own ("naive version").  Real coefficients: the real and
