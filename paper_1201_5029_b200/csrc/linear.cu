@@ -3,7 +3,7 @@
 // One pycool_linear_step(n, GROWTH) call enqueues, on the context's stream and without a host synchronisation:
 //     lin_background   (1 thread)   background through n x stages(order) stages + the per-stage coefficient table
 //     lin_growth       (thread per class x column)   growth matrices M(n dt, k_eff^2) of (2.51)
-//     lin_apply        (thread per mode)             every Fourier mode multiplied by its class's matrix
+//     lin_apply        (thread per mode x row of M)   every Fourier mode multiplied by its class's matrix
 // and with NAIVE: lin_background, then lin_naive (thread per mode through every stage).  Kernels: linear.cuh.
 #include <cmath>
 #include <cstdarg>
