@@ -54,6 +54,7 @@ def parse():
     ap.add_argument("--zchunk", type=int, default=0)
     ap.add_argument("--item-order", type=int, default=-1, help="tiles per region of the item order (0: plain x-y-z; -1: library's)")
     ap.add_argument("--persistent", type=int, default=-1, help="1/0: persistent launch of the TMA kernel on/off (default: library's)")
+    ap.add_argument("--cooperative", type=int, default=-1, help="1/0: multi-stage cooperative launches on small lattices on/off (default: library's)")
     ap.add_argument("--fused-tail", type=int, default=-1, help="1/0: fused stage tail on/off (default: library's)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-init", action="store_true", help="skip the on-device initial-conditions timing")
@@ -418,6 +419,8 @@ def main():
         lat.set_item_order(a.item_order)
     if a.persistent >= 0:
         lat.set_persistent(a.persistent)
+    if a.cooperative >= 0:
+        lat.set_cooperative(a.cooperative)
     if a.fused_tail >= 0:
         lat.set_fused_tail(a.fused_tail)
     if a.device_init:

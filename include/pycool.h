@@ -221,7 +221,8 @@ int pycool_stage_weights(int order, double* w, int cap);
 
 /* ---- instrumentation (does not change results) ---- */
 /* Number of kernels this context has launched so far, by kind:
- *   counts[0] fused drift+kick, [1] reduce+scalar update, [2] closing drift, [3] energy/sum kernels. */
+ *   counts[0] fused drift+kick (stages: a cooperative multi-stage launch counts each of its stages),
+ *   [1] reduce+scalar update, [2] closing drift, [3] energy/sum kernels. */
 int pycool_launch_counts(const pycool_ctx*, unsigned long long counts[4]);
 /* profiling on: bracket every fused drift+kick launch with CUDA events on the context stream. */
 int pycool_set_profiling(pycool_ctx*, int on);
@@ -241,6 +242,12 @@ int pycool_set_zchunk(pycool_ctx*, int planes);
  * so a stage is ONE launch.  Off: a separate reduce + scalar-update launch follows every kick.  Both orders of
  * summation are fixed; they differ from each other in the last bits only. */
 int pycool_set_fused_tail(pycool_ctx*, int on);
+/* Small lattices (default on): when every work item of a stage fits on the GPU at once (32^3 .. 128^3 on a B200) and
+ * the device supports cooperative launches, pycool_step runs up to 32 steps' worth of stages in ONE cooperative launch,
+ * with a grid-wide barrier between stages instead of a kernel boundary (the paper goes back to the CPU at every
+ * sub-step).  Results are bitwise those of the launch-per-stage path.  Off, while profiling, with the
+ * fused tail off or for larger lattices: one launch per stage.  pycool_launch_counts counts stages either way. */
+int pycool_set_cooperative(pycool_ctx*, int on);
 /* Programmatic dependent launch of the TMA-fed kernel (default on): the next stage's blocks are scheduled while
  * the current stage drains and wait (griddepcontrol.wait) until it has completed before they read anything it
  * wrote.  Hides launch latency and prologue on small lattices; results are unchanged. */

@@ -22,7 +22,7 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_read_fields", "pycool_read_fields_device", "pycool_device_fields", "pycool_energies", "pycool_destroy",
            "pycool_last_error", "pycool_stage_weights", "pycool_launch_counts", "pycool_set_profiling",
            "pycool_kick_time_ms", "pycool_kick_geometry", "pycool_set_zchunk", "pycool_set_tile",
-           "pycool_set_fused_tail", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_set_item_order", "pycool_init_fields",
+           "pycool_set_fused_tail", "pycool_set_cooperative", "pycool_set_persistent", "pycool_flush", "pycool_set_adaptive", "pycool_set_energy_kernel", "pycool_set_overlap", "pycool_set_item_order", "pycool_init_fields",
            "pycool_field_spectrum", "pycool_mode_spectra", "pycool_set_energy_cadence", "pycool_read_energy_log",
            # include/pycool_linear.h
            "pycool_linear_create", "pycool_linear_num_classes", "pycool_linear_set_background",
@@ -106,6 +106,7 @@ def lib():
         L.pycool_set_zchunk.argtypes = [vp, ip]
         L.pycool_set_tile.argtypes = [vp, ip]
         L.pycool_set_fused_tail.argtypes = [vp, ip]
+        L.pycool_set_cooperative.argtypes = [vp, ip]
         L.pycool_set_persistent.argtypes = [vp, ip]
         L.pycool_flush.argtypes = [vp]
         L.pycool_set_adaptive.argtypes = [vp, ip]
@@ -370,6 +371,10 @@ class Lattice:
 
     def set_persistent(self, on):
         self._chk(lib().pycool_set_persistent(self._h, 1 if on else 0))
+
+    def set_cooperative(self, on):
+        """Small lattices: several stages per cooperative launch (pycool_set_cooperative)."""
+        self._chk(lib().pycool_set_cooperative(self._h, 1 if on else 0))
 
     def set_fused_tail(self, on):
         self._chk(lib().pycool_set_fused_tail(self._h, 1 if on else 0))

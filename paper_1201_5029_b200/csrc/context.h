@@ -63,6 +63,10 @@ struct pycool_ctx {
   bool persistent = true;           // kick_tma: one block per resident slot, the TMA ring runs on across items
   int blocks_launched = 0;          // grid size of the latest kick launch
   bool fused_tail = true;           // last block of a kick reduces the partials and advances the scalars
+  bool cooperative = true;          // small lattices: several stages per cooperative launch (kick_tma_coop)
+  int coop_ok = -1;                 // the device supports cooperative launches (-1: not asked yet)
+  int coop_resident[16];            // co-resident blocks of kick_tma_coop per variant (-1: not asked yet, 0: not built)
+  pycool::CoopSchedule coop{};      // schedule of the next cooperative launch
   pycool::StageLen len{};                   // stage weights handed to the next kick launch
   bool adaptive = false;            // dt is a physical-time increment (pycool_set_adaptive)
   int device = 0, sms = 0;          // the CUDA device this context lives on and its SM count
@@ -122,7 +126,7 @@ extern const TileInfo kTiles[kNumTiles];
 int encode_one(pycool_ctx* c, void* ptr, int tx, int ty, CUtensorMap* out);
 
 // Kernel template instances live in one translation unit per model (models_*.cu); this is their one entry point.
-enum Op { OP_KICK, OP_ENERGY, OP_SMEM, OP_RESIDENT, OP_BUILT };
+enum Op { OP_KICK, OP_ENERGY, OP_SMEM, OP_RESIDENT, OP_BUILT, OP_KICK_COOP, OP_COOP_RESIDENT };
 template <typename Real, class Model>
 long long dispatch_one(pycool_ctx* c, Op op, int arg);
 

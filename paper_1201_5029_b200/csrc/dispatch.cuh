@@ -134,6 +134,74 @@ int launch_tma_t(pycool_ctx* c) {
   CUDA_TRY(c, cudaLaunchKernelEx(&cfg, kick_tma<Real, Model, T>, c->tm[c->cur][0], c->tm[c->cur][1], g));
   return PYCOOL_OK;
 }
+// ---- small lattices: several stages per cooperative launch (kick_tma_coop), variants 3 and 4 only
+template <class T> constexpr bool coop_tile() { return T::S == 3 && T::J == 2 && T::MINB == 1 && T::XW == 2 && T::TY == 16 && T::TX <= 64; }
+
+// Co-resident blocks of kick_tma_coop on this device (0: no cooperative launch here).
+template <typename Real, class Model, class T>
+int coop_resident(pycool_ctx* c, int tile_) {
+  if (c->coop_resident[tile_] >= 0) return c->coop_resident[tile_];
+  constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
+  int per_sm = 0, coop = 0;
+  cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device);
+  if (e == cudaSuccess && coop)
+    e = cudaFuncSetAttribute(kick_tma_coop<Real, Model, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess && coop)
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kick_tma_coop<Real, Model, T>, T::NT, smem);
+  if (e != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+  c->coop_resident[tile_] = coop ? per_sm * c->sms : 0;
+  return c->coop_resident[tile_];
+}
+
+// One cooperative launch of c->coop.nstages stages starting from buffer c->cur (the caller flips c->cur afterwards).
+template <typename Real, class Model, class T>
+int launch_tma_coop_t(pycool_ctx* c) {
+  constexpr size_t smem = TmaSmem<Real, Model, T>::TOTAL;
+  TmaArgs<Real> g;
+  g.phi_out = nullptr; g.pi_out = nullptr;                    // per stage: CoopArgs
+  g.sc = c->sc;
+  g.partials = c->partials;
+  g.tail.sc = c->sc;
+  g.tail.ticket = c->ticket;
+  g.tail.work = c->ticket + 1;
+  g.tail.fused = 1;
+  g.tail.k = c->kc;
+  g.tail.len = c->len;
+  g.L = c->lay;
+  g.zc = c->zc;
+  g.nbx = (int)c->grid.x; g.nby = (int)c->grid.y;
+  g.nitems = (int)(c->grid.x * c->grid.y * c->grid.z);
+  g.ry = c->region[1];
+  g.c1 = c->c[1]; g.c2 = c->c[2]; g.c3 = c->c[3];
+  g.mp = c->mp;
+  CoopArgs<Real> ca;
+  for (int b = 0; b < 2; ++b) { ca.phi[b] = (Real*)c->phi[b]; ca.pi[b] = (Real*)c->pi[b]; }
+  ca.cur0 = c->cur;
+  ca.release = c->ticket + 2;
+  CUDA_TRY(c, cudaMemsetAsync(ca.release, 0, sizeof(unsigned int), c->stream));
+  CoopSchedule sch = c->coop;
+  void* args[] = {(void*)&c->tm[0][0], (void*)&c->tm[0][1], (void*)&c->tm[1][0], (void*)&c->tm[1][1], (void*)&g, (void*)&ca,
+                  (void*)&sch};
+  CUDA_TRY(c, cudaLaunchCooperativeKernel((const void*)kick_tma_coop<Real, Model, T>, dim3((unsigned)g.nitems), dim3(T::NT),
+                                          args, smem, c->stream));
+  c->blocks_launched = g.nitems;
+  return PYCOOL_OK;
+}
+
+template <typename Real, class Model>
+long long coop_m(pycool_ctx* c, Op op, int tile_) {
+  switch (tile_) {
+#define X(ID, TT)                                                                                             \
+  case ID:                                                                                                    \
+    if constexpr (coop_tile<TT<Real>>() && tile_built<Real, Model, TT<Real>>())                               \
+      return op == OP_KICK_COOP ? launch_tma_coop_t<Real, Model, TT<Real>>(c) : coop_resident<Real, Model, TT<Real>>(c, tile_); \
+    else return op == OP_KICK_COOP ? PYCOOL_EINVAL : 0;
+    PYCOOL_TMA_TILES(X)
+#undef X
+    default: return op == OP_KICK_COOP ? PYCOOL_EINVAL : 0;
+  }
+}
+
 template <typename Real, class Model>
 int launch_kick_m(pycool_ctx* c) {
   const int tile_ = c->tile;
@@ -241,6 +309,8 @@ int launch_energy_m(pycool_ctx* c, int nb) {
 template <typename Real, class Model>
 long long dispatch_one(pycool_ctx* c, Op op, int arg) {
   if (op == OP_KICK) return launch_kick_m<Real, Model>(c);
+  if (op == OP_KICK_COOP) return coop_m<Real, Model>(c, op, c->tile);
+  if (op == OP_COOP_RESIDENT) return coop_m<Real, Model>(c, op, arg);
   if (op == OP_ENERGY) return launch_energy_m<Real, Model>(c, arg);
   if (op == OP_RESIDENT) return kick_resident_m<Real, Model>(c, arg);
   if (op == OP_BUILT) return tile_built_m<Real, Model>(arg) ? 1 : 0;

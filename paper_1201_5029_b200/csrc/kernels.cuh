@@ -129,6 +129,30 @@ __device__ __forceinline__ double block_sum_fixed(const double* v, int n, double
   return r;
 }
 
+// The three sums of a stage in one pass: the same per-quantity arithmetic as three block_sum_fixed calls (same strided
+// partial sums, same tree), but one set of loads in flight and one barrier per tree level instead of three.
+template <int T>
+__device__ __forceinline__ void block_sum_fixed3(const double* v, size_t stride, int n, double* sh /* 3 T doubles */,
+                                                 double (&out)[3]) {
+  static_assert((T & (T - 1)) == 0, "tree shape: power of two");
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+  for (int i = threadIdx.x; i < n; i += T) {
+    a0 += __ldcg(v + i); a1 += __ldcg(v + stride + i); a2 += __ldcg(v + 2 * stride + i);
+  }
+  sh[threadIdx.x] = a0; sh[T + threadIdx.x] = a1; sh[2 * T + threadIdx.x] = a2;
+  __syncthreads();
+  for (int s = T / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) {
+      sh[threadIdx.x] += sh[threadIdx.x + s];
+      sh[T + threadIdx.x] += sh[T + threadIdx.x + s];
+      sh[2 * T + threadIdx.x] += sh[2 * T + threadIdx.x + s];
+    }
+    __syncthreads();
+  }
+  out[0] = sh[0]; out[1] = sh[T]; out[2] = sh[2 * T];
+  __syncthreads();
+}
+
 // Lengths of a stage and of the one after it, as weights of the step length.
 struct StageLen {
   double w, w_next;   // stage weights (2.42)-(2.45), Table 1; w_next = 0: the call ends after this stage
@@ -136,6 +160,17 @@ struct StageLen {
   int adaptive;       // step length = dt / a(start of the step): "adaptive conformal step with constant
                       // increases in physical time"
   int ends_step;      // this stage is the last of its step
+};
+
+// Stage lengths of a multi-stage cooperative launch (kick_tma.cuh: kick_tma_coop): the device forms each StageLen.
+struct CoopSchedule {
+  double w[16];          // stage weights of one step (2.42)-(2.45), Table 1
+  int ns;                // stages per step
+  int first;             // index of this launch's first stage within the pycool_step call
+  int nstages;           // stages in this launch
+  int call_ends;         // the call ends with this launch: no stage follows the last one
+  double dt;
+  int adaptive;
 };
 
 // The scalar side of the step, one thread.
@@ -205,7 +240,7 @@ __device__ __forceinline__ void publish_partials(double* partials, unsigned npar
 // All threads, once per block, after thread 0 published the block's last partials.
 template <int NT>
 __device__ __forceinline__ void stage_finish(const StageTail& t, const double* partials, unsigned nparts,
-                                             double* sh /* >= NT doubles, free to overwrite */) {
+                                             double* sh /* >= 3 NT doubles, free to overwrite */) {
   __shared__ int is_last;
   if (threadIdx.x == 0) {
     __threadfence();
@@ -219,12 +254,11 @@ __device__ __forceinline__ void stage_finish(const StageTail& t, const double* p
   }
   if (!t.fused) return;
   __threadfence();
-  const double SD = block_sum_fixed<NT>(partials, (int)nparts, sh);
-  const double SV = block_sum_fixed<NT>(partials + nparts, (int)nparts, sh);
-  const double SP = block_sum_fixed<NT>(partials + 2 * (size_t)nparts, (int)nparts, sh);
+  double S3[3];
+  block_sum_fixed3<NT>(partials, (size_t)nparts, (int)nparts, sh, S3);
   if (threadIdx.x == 0) {
     Scalars s = *t.sc;
-    scalar_advance(s, t.k, t.len, 1, SD, SV, SP);
+    scalar_advance(s, t.k, t.len, 1, S3[0], S3[1], S3[2]);
     *t.sc = s;
   }
 }
@@ -292,7 +326,7 @@ struct Tile {
 template <typename Real, class Model, class T>
 constexpr size_t kick_smem_bytes() {
   size_t tile = 2 * (size_t)Model::NF * T::PLANE * sizeof(Real);
-  size_t red = (size_t)T::NT * sizeof(double);          // block_reduce scratch, then the tail's tree
+  size_t red = 3 * (size_t)T::NT * sizeof(double);      // block_reduce scratch, then the tail's three trees
   return tile > red ? tile : red;
 }
 

@@ -92,7 +92,7 @@ struct TmaSmem {
   static constexpr size_t RED = 3 * (T::NT / 32) * sizeof(double);             // per-item block reduction
   static constexpr size_t TOTAL = RAW + PSI + BARS + RED + 128;                // + slack to align the base
   static_assert(T::S * 8 <= BARS, "mbarriers fit");
-  static_assert(T::NT * sizeof(double) <= PSI, "the stage tail's tree fits in the psi buffers");
+  static_assert(3 * T::NT * sizeof(double) <= RAW + PSI, "the stage tail's three trees fit in the idle ring + psi");
 };
 
 template <typename Real>
@@ -138,8 +138,9 @@ __device__ __forceinline__ void item_origin(const TmaArgs<Real>& g, int item, in
 // The z-march of one work item.  EDGE (compile time) = the item touches a lattice face or a ragged edge: only
 // that copy carries the periodic-image stores and the validity predicates; interior items run branch-free.
 template <bool EDGE, typename Real, class Model, class T, class IssueF>
-__device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue_next, int& slot, uint32_t& phase,
-                                           unsigned char* raw, Real* psi, const uint32_t bars, const int x0,
+__device__ __forceinline__ void march_item(const TmaArgs<Real>& g, Real* phi_out, Real* pi_out, IssueF& issue_next,
+                                           int& slot, uint32_t& phase, unsigned char* raw, Real* psi,
+                                           const uint32_t bars, const int x0,
                                            const int y0, const int z0, const int nz, const int own_sm,
                                            const int (&halo_sm)[(T::NHP + T::NT - 1) / T::NT], const Real cd,
                                            const Real kD, const Real kV, const Real c0, const Real c1, const Real c2,
@@ -238,7 +239,7 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
 
     // ---- 1. drift: phi' = phi + c_drift pi (own groups and halo ring); psi = phi' - ref to shared memory
     const bool own_plane = (p >= 0) && (p < nz);
-    unsigned char* ophi = reinterpret_cast<unsigned char*>(g.phi_out) + (size_t)gz_cur * plane_b;
+    unsigned char* ophi = reinterpret_cast<unsigned char*>(phi_out) + (size_t)gz_cur * plane_b;
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
 #pragma unroll
@@ -298,7 +299,7 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, IssueF& issue
       }
     }
     if (p >= 1) {
-      unsigned char* opi = reinterpret_cast<unsigned char*>(g.pi_out) + (size_t)gz_prev * plane_b;   // plane p-1
+      unsigned char* opi = reinterpret_cast<unsigned char*>(pi_out) + (size_t)gz_prev * plane_b;   // plane p-1
 #pragma unroll
       for (int j = 0; j < J; ++j) {
         if (!EDGE || valid[j]) {
@@ -448,11 +449,11 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     const bool edge_blk = (x0 < L.gx) | (x0 + TX > N - L.gx) | (y0 == 0) | (y0 + TY >= N);
     double sD = 0.0, sV = 0.0, sP = 0.0;
     if (edge_blk)
-      march_item<true, Real, Model, T>(g, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz, own_sm, halo_sm, cd,
-                                       kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
+      march_item<true, Real, Model, T>(g, g.phi_out, g.pi_out, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz,
+                                       own_sm, halo_sm, cd, kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
     else
-      march_item<false, Real, Model, T>(g, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz, own_sm, halo_sm,
-                                        cd, kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
+      march_item<false, Real, Model, T>(g, g.phi_out, g.pi_out, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz,
+                                        own_sm, halo_sm, cd, kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
 
     // ---- the item's partial sums, fixed order.  The barrier inside block_reduce also separates this item's
     // last reads of the psi planes from the next item's first writes.
@@ -461,8 +462,169 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
     if (tid == 0) publish_partials(g.partials, (unsigned)g.nitems, (unsigned)item, v);
   }
 
-  __syncthreads();                                             // psi is free: the tail's tree uses it
-  stage_finish<NT>(g.tail, g.partials, (unsigned)g.nitems, reinterpret_cast<double*>(psi));
+  __syncthreads();                                             // ring (every load consumed) and psi are free: the tail's
+  stage_finish<NT>(g.tail, g.partials, (unsigned)g.nitems, reinterpret_cast<double*>(raw));   // trees use them
+}
+
+
+// ------------------------------------------------------------------------------------------------ small lattices
+// Several stages in ONE cooperative launch, for lattices whose work items all fit on the GPU at once (32^3 .. 128^3):
+// one block per item, and between stages a grid-wide barrier instead of a kernel boundary -- the blocks stay
+// resident, keep their shared-memory carve-up, barriers and per-thread tables, and a stage costs no launch
+// hand-over (the paper returns to the CPU at every sub-step).  The barrier is the stage tail itself:
+// every block publishes its partial sums and takes a ticket; the block that draws the last ticket adds the partials
+// in item order, advances the scalars (scalar_advance, as stage_finish does) and releases the others, which wait on a
+// counter in global memory.  Same items, same partial-sum indices, same order of the final sum as the launch-per-
+// stage path: results are bitwise identical (tested).  Needs cudaLaunchCooperativeKernel (co-residency).
+template <typename Real>
+struct CoopArgs {
+  Real* phi[2];          // the two state buffers; stage k reads buffer (cur0 + k) & 1 and writes the other
+  Real* pi[2];
+  int cur0;
+  unsigned int* release; // stages completed in this launch (zero at launch)
+};
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <typename Real, class Model, class T>
+__global__ void __launch_bounds__(T::NT, T::MINB)
+kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant__ CUtensorMap tm_pi0,
+              const __grid_constant__ CUtensorMap tm_phi1, const __grid_constant__ CUtensorMap tm_pi1,
+              const TmaArgs<Real> g, const CoopArgs<Real> ca, const CoopSchedule sch) {
+  using SM = TmaSmem<Real, Model, T>;
+  constexpr int TX = T::TX, TY = T::TY, S = T::S, G = T::G, PX = T::PX, NT = T::NT, J = T::J, XW = T::XW;
+
+  extern __shared__ unsigned char smem_dyn[];
+  unsigned char* base = smem_dyn + ((128u - (smem_addr(smem_dyn) & 127u)) & 127u);
+  unsigned char* raw = base;
+  Real* psi = reinterpret_cast<Real*>(base + SM::RAW);
+  const uint32_t bars = smem_addr(base + SM::RAW + SM::PSI);
+  double* red = reinterpret_cast<double*>(base + SM::RAW + SM::PSI + SM::BARS);
+  __shared__ int is_last;
+
+  const Layout& L = g.L;
+  const int N = L.N;
+  const int tid = threadIdx.x;
+  const int txw = tid % (TX / XW), tyj = tid / (TX / XW);
+  const int item = blockIdx.x;                                 // one item per block, the same in every stage
+  int x0, y0, z0, nz;
+  item_origin<Real, TX, TY>(g, item, x0, y0, z0, nz);
+  const bool edge_blk = (x0 < L.gx) | (x0 + TX > N - L.gx) | (y0 == 0) | (y0 + TY >= N);
+
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) mbar_init(bars + 8u * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  const Real c1 = Real(g.c1), c2 = Real(g.c2), c3 = Real(g.c3);
+  const Real c0 = -(Real(6) * c1 + Real(12) * c2 + Real(8) * c3);
+  const typename Model::template Coef<Real> coef(g.mp);
+  const int own_sm = (J * tyj + 1) * PX + G + XW * txw;
+  constexpr int NHT = (T::NHP + NT - 1) / NT;
+  int halo_sm[NHT];
+#pragma unroll
+  for (int k = 0; k < NHT; ++k) {
+    const int h = tid + k * NT;
+    int row, col;
+    if (h < T::HR) { row = 0; col = G - 2 + 2 * h; }
+    else if (h < 2 * T::HR) { row = TY + 1; col = G - 2 + 2 * (h - T::HR); }
+    else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 2; }
+    halo_sm[k] = h < T::NHP ? row * PX + col : -1;
+  }
+  int slot = 0;
+  uint32_t phase = 0;
+  __syncthreads();                                             // barriers initialised before anyone waits
+
+#pragma unroll 1
+  for (int k = 0; k < sch.nstages; ++k) {
+    const int cur = (ca.cur0 + k) & 1;
+    const CUtensorMap* tphi = cur ? &tm_phi1 : &tm_phi0;
+    const CUtensorMap* tpi = cur ? &tm_pi1 : &tm_pi0;
+    // the loads of this stage: planes z0-1 .. z0+nz of the block's item, S in flight
+    int pr_i = 0;
+    const int pr_nload = nz + 2;
+    auto issue_next = [&](int s) {
+      if (pr_i >= pr_nload) return;
+      if (tid == 0) {
+        const uint32_t bar = bars + 8u * s;
+        const uint32_t dst = smem_addr(raw + (size_t)s * 2 * SM::BOXA);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(bar, (uint32_t)(2 * SM::BOX));
+        int gz = z0 + pr_i - 1;
+        gz = gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+        tma_load_4d(dst, tphi, bar, x0, y0, gz, 0);
+        tma_load_4d(dst + (uint32_t)SM::BOXA, tpi, bar, x0, y0, gz, 0);
+      }
+      ++pr_i;
+    };
+    for (int s = 0; s < S; ++s) {                              // ring slots in consumption order from `slot`
+      int sl = slot + s; if (sl >= S) sl -= S;
+      issue_next(sl);
+    }
+    // the scalars the previous stage's tail left (other blocks wrote them: read through L2)
+    const Real cd = Real(__ldcg(&g.sc->c_drift)), kD = Real(__ldcg(&g.sc->kD)), kV = Real(__ldcg(&g.sc->kV));
+
+    double sD = 0.0, sV = 0.0, sP = 0.0;
+    Real* po = ca.phi[cur ^ 1];
+    Real* qo = ca.pi[cur ^ 1];
+    if (edge_blk)
+      march_item<true, Real, Model, T>(g, po, qo, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz, own_sm, halo_sm,
+                                       cd, kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
+    else
+      march_item<false, Real, Model, T>(g, po, qo, issue_next, slot, phase, raw, psi, bars, x0, y0, z0, nz, own_sm, halo_sm,
+                                        cd, kD, kV, c0, c1, c2, c3, coef, sD, sV, sP);
+    double v[3] = {sD, sV, sP};
+    block_reduce<3, NT>(v, red);
+
+    // ---- stage tail = grid barrier.  Thread 0 publishes, then takes a ticket (release: every store of this block,
+    // fields included, is ordered before it by the block barrier + fence).
+    __syncthreads();
+    if (tid == 0) {
+      publish_partials(g.partials, (unsigned)g.nitems, (unsigned)item, v);
+      __threadfence();
+      is_last = atomicAdd(g.tail.ticket, 1u) == (unsigned)(k + 1) * gridDim.x - 1u;
+    }
+    __syncthreads();
+    if (is_last) {                                             // every block has published: reduce, advance, release
+      __threadfence();
+      double* sh = reinterpret_cast<double*>(raw);             // ring idle (every load consumed), psi behind it
+      double S3[3];
+      block_sum_fixed3<NT>(g.partials, (size_t)g.nitems, g.nitems, sh, S3);
+      const double SD = S3[0], SV = S3[1], SP = S3[2];
+      if (tid == 0) {
+        const int i = sch.first + k;                           // stage index within the call
+        StageLen len;
+        len.dt = sch.dt; len.adaptive = sch.adaptive;
+        len.w = sch.w[i % sch.ns];
+        len.w_next = (k + 1 < sch.nstages || !sch.call_ends) ? sch.w[(i + 1) % sch.ns] : 0.0;
+        len.ends_step = (i % sch.ns) == sch.ns - 1;
+        Scalars s;                                             // through L2: another block wrote them last stage, and
+        {                                                      // this SM's L1 may still hold an older copy
+          const double* src = reinterpret_cast<const double*>(g.sc);
+          double* dst = reinterpret_cast<double*>(&s);
+          static_assert(sizeof(Scalars) % sizeof(double) == 0, "Scalars is copied as doubles");
+#pragma unroll
+          for (int q = 0; q < (int)(sizeof(Scalars) / sizeof(double)); ++q) dst[q] = __ldcg(src + q);
+        }
+        scalar_advance(s, g.tail.k, len, 1, SD, SV, SP);
+        *g.tail.sc = s;
+        if (k + 1 == sch.nstages) *g.tail.ticket = 0u;         // counters ready for the next launch
+        __threadfence();
+        st_release_u32(ca.release, (unsigned)(k + 1));
+      }
+    }
+    if (tid == 0) {
+      while (ld_acquire_u32(ca.release) < (unsigned)(k + 1)) __nanosleep(20);
+      asm volatile("fence.proxy.async;" ::: "memory");         // other blocks' stores before this block's TMA loads
+    }
+    __syncthreads();
+  }
 }
 
 }  // namespace pycool

@@ -260,7 +260,7 @@ int auto_zchunk(pycool_ctx* c) {
   if (items(cap) >= 4LL * R) return cap;
   int best = cap < N ? cap : N;
   long long best_cost = -1;
-  for (int zc = N; zc >= 2; --zc) {                           // small lattices: few planes per block; chunks are
+  for (int zc = N; zc >= 1; --zc) {                           // small lattices: few planes per block; chunks are
     const int nbz = (N + zc - 1) / zc;                        // balanced, so what counts is the longest, ceil(N / nbz)
     const int len = (N + nbz - 1) / nbz;
     const long long rounds = ((long long)bxy * nbz + R - 1) / R;
@@ -480,6 +480,7 @@ int create_common(pycool_ctx** out, int N, double L, int nf, const pycool_params
   pycool_ctx* c = new (std::nothrow) pycool_ctx();
   if (!c) return fail(nullptr, PYCOOL_ENOMEM, "host allocation failed");
   for (int& r : c->resident) r = -1;
+  for (int& r : c->coop_resident) r = -1;
   {
     // the context lives on the device of the caller's work buffer (ext), else on the current device
     int dev = 0;
@@ -828,7 +829,40 @@ int pycool_step(pycool_ctx* c, int nsteps) {
       c->ev.push_back(e);
     }
   }
-  for (long long i = 0; i < S; ++i) {
+  // Small lattices whose work items are all co-resident: several stages per cooperative launch, a grid barrier
+  // between stages instead of a kernel boundary (kick_tma.cuh: kick_tma_coop); same results bit for bit.
+  const long long nitems = (long long)c->grid.x * c->grid.y * c->grid.z;
+  const bool coop = c->cooperative && c->fused_tail && !c->profiling && kTiles[c->tile].stages > 0 &&
+                    dispatch(c, OP_COOP_RESIDENT, c->tile) >= nitems;
+  for (long long i = 0; i < S;) {
+    if (coop) {
+      // up to the end of the call, the next energy-log point, or 32 steps, whichever comes first
+      long long n = std::min<long long>(S - i, 32LL * ns);
+      if (c->log_every > 0) {
+        const long long to_step_end = ns - (i % ns);
+        const unsigned long long steps_to_log = (unsigned long long)c->log_every - c->steps_done % (unsigned long long)c->log_every;
+        n = std::min<long long>(n, to_step_end + (long long)(steps_to_log - 1) * ns);
+      }
+      CoopSchedule& sch = c->coop;
+      for (int k = 0; k < ns; ++k) sch.w[k] = c->w[k];
+      sch.ns = ns; sch.first = (int)(i % ns); sch.nstages = (int)n; sch.call_ends = (i + n == S) ? 1 : 0;
+      sch.dt = c->dt; sch.adaptive = c->adaptive ? 1 : 0;
+      st = (int)dispatch(c, OP_KICK_COOP, 0);
+      if (st != PYCOOL_OK) return st;
+      c->counts[0] += (unsigned long long)n;
+      if (n & 1) c->cur ^= 1;
+      const long long steps_ended = (i % ns + n) / ns;       // steps completed inside this launch
+      i += n;
+      if (c->log_every > 0 && steps_ended > 0) {
+        c->steps_done += (unsigned long long)steps_ended;
+        if (i % ns == 0 && c->steps_done % (unsigned long long)c->log_every == 0) {
+          st = enqueue_energy(c, true, c->d_log + (c->log_n % (unsigned long long)c->log_cap));
+          if (st != PYCOOL_OK) return st;
+          c->log_n++;
+        }
+      }
+      continue;
+    }
     len.w = c->w[i % ns];
     len.w_next = (i + 1 < S) ? c->w[(i + 1) % ns] : 0.0;      // stage weights are never zero
     len.ends_step = (i % ns) == ns - 1;
@@ -850,6 +884,7 @@ int pycool_step(pycool_ctx* c, int nsteps) {
       if (st != PYCOOL_OK) return st;
       c->log_n++;
     }
+    ++i;
   }
   c->pending_drift = true;
   return PYCOOL_OK;
@@ -1061,6 +1096,13 @@ int pycool_set_persistent(pycool_ctx* c, int on) {
   if (!c) return PYCOOL_EINVAL;
   OnDevice on_device(c);
   c->persistent = on != 0;
+  return PYCOOL_OK;
+}
+
+int pycool_set_cooperative(pycool_ctx* c, int on) {
+  if (!c) return PYCOOL_EINVAL;
+  OnDevice on_device(c);
+  c->cooperative = on != 0;
   return PYCOOL_OK;
 }
 

@@ -778,3 +778,48 @@ def test_nothing_is_written_outside_the_work_buffer_and_nothing_uninitialised_is
     assert np.all(np.isfinite(out_phi)) and np.all(np.isfinite(out_pi))
     for v in (e.a, e.p_a, e.rho, e.pressure, e.pot) + tuple(e.kin[:nf]) + tuple(e.grad[:nf]):
         assert math.isfinite(v)
+
+
+# ------------------------------------------------------------------------------------- cooperative multi-stage launches
+@pytest.mark.parametrize("name,N,order,precision,kw", [("cfg0_chaotic32", 32, 4, 64, {}), ("cfg1_chaotic128", 128, 6, 64, {}),
+                                                       ("cfg0_chaotic32", 64, 4, 32, {}), ("cfg2_oscillon256", 48, 4, 64, {}),
+                                                       ("cfg3_qball256", 40, 4, 64, {}), ("cfg0_chaotic32", 24, 8, 64, {"adaptive": True})])
+def test_cooperative_launch_is_bitwise_the_launch_per_stage_path(pc, name, N, order, precision, kw):
+    """Small lattices run several stages per cooperative launch with a grid barrier between stages
+    (pycool_set_cooperative, default on).  Same items, same partial-sum indices, same order of every sum: fields,
+    scalars, energies and the energy log are bitwise those of the launch-per-stage path, across split calls, odd and
+    even stage counts per launch (buffer parity) and log points in the middle of a call; and the default path really is
+    the cooperative one (checked through the oracle as well at N = 32)."""
+    cfg = inputs.config(name, N=N, order=order) if name != "cfg0_chaotic32" or N == 32 else inputs.config(name, N=N, order=order, dt=0.0025)
+    if name in ("cfg2_oscillon256", "cfg3_qball256"):
+        cfg["L"] = cfg["L"] * N / inputs.config(name)["N"]
+    nf = cfg["nfields"]
+    phi, pi = inputs.make_initial(cfg, precision=precision)
+
+    def run(coop):
+        g = pc.from_config(cfg, precision=precision)
+        g.set_cooperative(coop)
+        g.set_fields(phi, pi); g.set_background(1.0)
+        if kw.get("adaptive"):
+            g.set_adaptive(True)
+        g.set_energy_cadence(2, 8)
+        g.step(3); g.step(1); g.step(5)
+        log, total = g.read_energy_log()
+        e = g.energies()
+        return g.read_fields(), e, log, total, g.launch_counts()[0]
+
+    (pa, qa), ea, la, ta, na = run(True)
+    (pb, qb), eb, lb, tb, nb = run(False)
+    stages = {2: 1, 4: 3, 6: 7, 8: 15}[order]
+    assert na == nb == 9 * stages and ta == tb == 4
+    assert np.array_equal(pa, pb) and np.array_equal(qa, qb)
+    tup = lambda e: (e.a, e.p_a, e.eta, e.rho, e.pressure, e.pot, e.hubble) + tuple(e.kin[:nf]) + tuple(e.grad[:nf])
+    assert tup(ea) == tup(eb)
+    assert [tup(x) for x in la] == [tup(x) for x in lb]
+    if N == 32:
+        o = oracle.Oracle(N, cfg["L"], nf, cfg["model"], cfg["p"], order=order, dt=cfg["dt"], mpl=cfg["mpl"])
+        o.set_fields(phi, pi); o.set_background(1.0)
+        o.step(9)
+        po, qo = o.read_fields()
+        assert rel_err_per_site(pa, po) <= 1e-11 and rel_err_per_site(qa, qo) <= 1e-11
+        assert rel(ea.a, o.energies().a) <= 1e-12
