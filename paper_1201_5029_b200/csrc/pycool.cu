@@ -832,7 +832,7 @@ int pycool_step(pycool_ctx* c, int nsteps) {
   // Small lattices whose work items are all co-resident: several stages per cooperative launch, a grid barrier
   // between stages instead of a kernel boundary (kick_tma.cuh: kick_tma_coop); same results bit for bit.
   const long long nitems = (long long)c->grid.x * c->grid.y * c->grid.z;
-  const bool coop = c->cooperative && c->fused_tail && !c->profiling && kTiles[c->tile].stages > 0 &&
+  bool coop = c->cooperative && c->fused_tail && !c->profiling && kTiles[c->tile].stages > 0 &&
                     dispatch(c, OP_COOP_RESIDENT, c->tile) >= nitems;
   for (long long i = 0; i < S;) {
     if (coop) {
@@ -848,7 +848,12 @@ int pycool_step(pycool_ctx* c, int nsteps) {
       sch.ns = ns; sch.first = (int)(i % ns); sch.nstages = (int)n; sch.call_ends = (i + n == S) ? 1 : 0;
       sch.dt = c->dt; sch.adaptive = c->adaptive ? 1 : 0;
       st = (int)dispatch(c, OP_KICK_COOP, 0);
-      if (st != PYCOOL_OK) return st;
+      if (st != PYCOOL_OK) {                                 // e.g. the GPU is shared and the grid is not co-resident:
+        cudaGetLastError();                                  // nothing was launched; go on one launch per stage
+        coop = false;
+        c->cooperative = false;
+        continue;
+      }
       c->counts[0] += (unsigned long long)n;
       if (n & 1) c->cur ^= 1;
       const long long steps_ended = (i % ns + n) / ns;       // steps completed inside this launch
