@@ -17,7 +17,7 @@ namespace pycool {
 constexpr int kMaxSumBlocks = 1184;      // capacity (partial sums) of the sum / energy kernels: 8 blocks per SM, at most
 constexpr size_t kMaxSmem = 227 * 1024;  // dynamic shared memory one block may opt in to on sm_100
 constexpr int kNumGeneric = 3;           // kick_fused variants (any N, any layout)
-constexpr int kNumTiles = 12;            // + kick_tma variants (ghost layout only)
+constexpr int kNumTiles = 13;            // + kick_tma variants (ghost layout only)
 
 struct TileInfo { int tx, ty, nt, stages, xw; };   // stages > 0: TMA ring depth; xw: sites per thread along x (fp32)
 

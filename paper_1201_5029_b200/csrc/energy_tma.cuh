@@ -97,15 +97,7 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
   const int own_sm = (J * tyj + 1) * PX + G + 2 * tx2;
   constexpr int NHT = (T::NHP + NT - 1) / NT;
   int halo_sm[NHT];
-#pragma unroll
-  for (int k = 0; k < NHT; ++k) {
-    const int h = tid + k * NT;
-    int row, col;
-    if (h < T::HR) { row = 0; col = G - 2 + 2 * h; }
-    else if (h < 2 * T::HR) { row = TY + 1; col = G - 2 + 2 * (h - T::HR); }
-    else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 2; }
-    halo_sm[k] = h < T::NHP ? row * PX + col : -1;
-  }
+  halo_pairs_of_thread<T>(tid, halo_sm);
 
   // per site: value pair of plane p-1 (phi, pi), accumulators of D[psi] (A, B)
   double2 pphi[NF][J], ppi[NF][J], A[NF][J], B[NF][J];

@@ -82,6 +82,22 @@ struct TmaTile {
   static_assert(PX <= 256 && RY <= 256, "TMA box extents");
 };
 
+// Box offsets of the halo pairs this thread converts every plane: the top and bottom box rows (x = -2 .. TX+1 in pairs)
+// and the pairs left and right of every own row; -1 = none.  16-byte accesses in fp64, the outer element is unused.
+template <class T>
+__device__ __forceinline__ void halo_pairs_of_thread(int tid, int (&halo_sm)[(T::NHP + T::NT - 1) / T::NT]) {
+  constexpr int NHT = (T::NHP + T::NT - 1) / T::NT;
+#pragma unroll
+  for (int k = 0; k < NHT; ++k) {
+    const int h = tid + k * T::NT;
+    int row, col;
+    if (h < T::HR) { row = 0; col = T::G - 2 + 2 * h; }
+    else if (h < 2 * T::HR) { row = T::TY + 1; col = T::G - 2 + 2 * (h - T::HR); }
+    else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? T::G + T::TX : T::G - 2; }
+    halo_sm[k] = h < T::NHP ? row * T::PX + col : -1;
+  }
+}
+
 template <typename Real, class Model, class T>
 struct TmaSmem {
   static constexpr size_t BOX = (size_t)Model::NF * T::PLANE * sizeof(Real);   // bytes one bulk copy delivers
@@ -429,15 +445,7 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
   const int own_sm = (J * tyj + 1) * PX + G + XW * txw;
   constexpr int NHT = (T::NHP + NT - 1) / NT;                  // halo pairs per thread
   int halo_sm[NHT];
-#pragma unroll
-  for (int k = 0; k < NHT; ++k) {
-    const int h = tid + k * NT;
-    int row, col;
-    if (h < T::HR) { row = 0; col = G - 2 + 2 * h; }
-    else if (h < 2 * T::HR) { row = TY + 1; col = G - 2 + 2 * (h - T::HR); }
-    else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 2; }
-    halo_sm[k] = h < T::NHP ? row * PX + col : -1;
-  }
+  halo_pairs_of_thread<T>(tid, halo_sm);
   int slot = 0;                                                // ring slot and phase of the next plane to consume
   uint32_t phase = 0;
 
@@ -528,15 +536,7 @@ kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant
   const int own_sm = (J * tyj + 1) * PX + G + XW * txw;
   constexpr int NHT = (T::NHP + NT - 1) / NT;
   int halo_sm[NHT];
-#pragma unroll
-  for (int k = 0; k < NHT; ++k) {
-    const int h = tid + k * NT;
-    int row, col;
-    if (h < T::HR) { row = 0; col = G - 2 + 2 * h; }
-    else if (h < 2 * T::HR) { row = TY + 1; col = G - 2 + 2 * (h - T::HR); }
-    else { const int r = h - 2 * T::HR; row = 1 + (r >> 1); col = (r & 1) ? G + TX : G - 2; }
-    halo_sm[k] = h < T::NHP ? row * PX + col : -1;
-  }
+  halo_pairs_of_thread<T>(tid, halo_sm);
   int slot = 0;
   uint32_t phase = 0;
   __syncthreads();                                             // barriers initialised before anyone waits

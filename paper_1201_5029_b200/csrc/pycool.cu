@@ -79,7 +79,7 @@ int pycool::fail(pycool_ctx* c, int code, const char* fmt, ...) {
 const TileInfo pycool::kTiles[kNumTiles] = {{32, 8, 128, 0, 1}, {32, 16, 256, 0, 1}, {64, 8, 256, 0, 1},
                                             {64, 16, 256, 3, 2}, {32, 16, 128, 3, 2}, {128, 8, 256, 3, 2},
                                             {128, 16, 512, 3, 2}, {32, 16, 256, 3, 2}, {64, 8, 256, 3, 2},
-                                            {128, 16, 256, 3, 2}, {32, 16, 256, 3, 2}, {128, 8, 256, 3, 4}};
+                                            {128, 16, 256, 3, 2}, {32, 16, 256, 3, 2}, {128, 8, 256, 3, 4}, {32, 8, 128, 3, 2}};
 
 namespace {
 
@@ -221,17 +221,18 @@ long long dispatch(pycool_ctx* c, Op op, int arg) {
 //   512^3 and 1024^3, profiles/r2) when N is a multiple of 4;
 //   one field fp64: 128 x 16 with 2 x 4 sites per thread (twice the work per plane and per barrier; a ring of 6
 //   with the 64 x 16 tile gains nothing, so it is the per-plane fixed cost, not the bytes in flight);
-//   Q-ball (the logarithm makes it ALU-heavy): 32 x 16 with 2 x 1 sites per thread, two blocks per SM.
+//   Q-ball (bound by the latency of its dependent fp64 work): 32 x 8 with 2 x 1 sites per thread, four blocks per SM
+//   (variant 12; 32 x 16 with two blocks per SM, variant 7, is 9 % slower in one process).
 int auto_tile(pycool_ctx* c) {
   const Layout& L = c->lay;
   if (L.gx == 0) return L.N <= 64 ? 0 : 1;
-  static const int pref_default[] = {3, 4}, pref_one[] = {9, 6, 3, 4}, pref_alu[] = {7, 4}, pref_f32[] = {11, 5, 3, 4},
+  static const int pref_default[] = {3, 4}, pref_one[] = {9, 6, 3, 4}, pref_alu[] = {12, 7, 4}, pref_f32[] = {11, 5, 3, 4},
                    pref_small[] = {4, 10}, pref_many[] = {10, 4};
   const int* pref = pref_default;
   int n = 2;
   if (c->nf >= 3) { pref = c->precision == 64 ? pref_many : pref_small; n = 2; }   // 2 x 1 sites per thread in fp64
   else if (L.N <= 64) { pref = pref_small; n = 2; }
-  else if (c->model == PYCOOL_QBALL && c->precision == 64) { pref = pref_alu; n = 2; }
+  else if (c->model == PYCOOL_QBALL && c->precision == 64) { pref = pref_alu; n = 3; }
   else if (c->nf == 1 && c->precision == 64) { pref = pref_one; n = 4; }
   else if (c->precision == 32 && c->nf >= 2) { pref = pref_f32; n = 4; }
   for (int i = 0; i < n; ++i)
