@@ -278,7 +278,9 @@ int pycool_set_persistent(pycool_ctx*, int on);
  *   3..10: TMA-fed kernel (even N >= 4 only, else PYCOOL_EINVAL): tiles 64x16, 32x16, 128x8, 128x16 with 2 x 2
  *         sites per thread; 32x16, 64x8 with 2 x 1 sites per thread and two blocks per SM; 128x16 with 2 x 4
  *         sites per thread (one-field lattices); 32x16 with 2 x 1 sites per thread, one block per SM (three and
- *         four fp64 fields).
+ *         four fp64 fields);
+ *   11:   128x8 as x quads, 4 x 1 sites per thread with 16-byte float accesses (fp32 only, N a multiple of 4);
+ *   12:   32x8 with 2 x 1 sites per thread and four blocks per SM (the Q-ball model in fp64 only).
  * PYCOOL_EINVAL also if the variant's TMA ring does not fit in shared memory for this model and precision, or
  * if its per-thread state would not fit the register budget for this number of fields (such instances are not
  * compiled: no variant that spills is shipped). */
