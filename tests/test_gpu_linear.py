@@ -174,11 +174,13 @@ def test_matter_term_and_explicit_p_a(pc):
     check_background(g, o, 2)
 
 
-def test_sampled_modes_at_bench_size(pc):
-    """128^3 x 2 fields (the size bench.py --linear times is 256^3; the oracle holds full complex spectra, so the
-    element-wise check runs here): 20 steps through the growth matrices, every 97th mode of the half spectrum
-    against the oracle's per-mode evolution of exactly those modes."""
-    N, L, steps = 128, 10.0, 20
+@pytest.mark.parametrize("N,method", [(128, "growth"), (256, "growth"), (256, "naive")])
+def test_sampled_modes_at_bench_size(pc, N, method):
+    """The size and launch configuration bench.py's `linear` block times (256^3 x 2 fields, order 4, 20 steps per call;
+    also 128^3): every 97th mode of the half spectrum against the oracle's per-mode evolution of exactly those modes
+    (the oracle's own arrays hold full complex spectra, so it is run on the sample: a mode's evolution depends on its
+    k_eff^2 and the background only)."""
+    L, steps = 10.0, 20
     m = MODELS["chaotic"]
     g = pc.LinearLattice(N, L, 2, m["model"], m["p"], order=4, dt=L / N / 20.0, mpl=1.0)
     g.set_background(1.0, math.nan, m["phi0"], m["pi0"])
@@ -187,7 +189,7 @@ def test_sampled_modes_at_bench_size(pc):
     P0 = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
     Q0 = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
     g.set_modes(P0, Q0)
-    g.step(steps, pc.GROWTH)
+    g.step(steps, pc.GROWTH if method == "growth" else pc.NAIVE)
     P, Q = g.read_modes()
     # the oracle on the sampled modes: a tiny LinearOracle carries the background, the modes' own k_eff^2 is passed in
     o = linear.LinearOracle(4, L * 4 / N, 2, m["model"], m["p"], order=4, dt=L / N / 20.0, mpl=1.0)
