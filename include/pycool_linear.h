@@ -116,6 +116,35 @@ int pycool_linear_destroy(pycool_linear_ctx*);
  * thread); library-owned string. */
 const char* pycool_linear_last_error(const pycool_linear_ctx*);
 
+/* ---- growth matrices with NO allocation: for callers that cannot call cudaMalloc (a stream under CUDA graph
+ * capture, a tight serving loop, a harness that forbids it).  No context: one call computes the growth matrices
+ * M(nsteps dt, k_eff^2) of (2.51) of every class -- the background kernel + the growth kernel of
+ * pycool_linear_step(.., PYCOOL_LINEAR_GROWTH), same arithmetic, same class order -- for the background given by
+ * value, and writes them to memory the CALLER owns.  It calls no cudaMalloc / cudaFree / stream, event or plan
+ * creation: the scratch those kernels need (the background state, the stage weights and the per-stage coefficient
+ * table, 2 + nf^2 doubles per stage) lives in a fixed array in the library's device image,
+ *     PYCOOL_LINEAR_STATIC_MAX_STAGES stages = 576 KiB + 256 bytes,
+ * which every GPU that loads libpycool.so holds until the process exits.
+ *   nsteps * stages(order) <= PYCOOL_LINEAR_STATIC_MAX_STAGES (stages: 1, 3, 7, 15 for order 2, 4, 6, 8), else
+ *   PYCOOL_EINVAL with a message naming the limit; N, L, nfields, params, order, dt as for pycool_linear_create;
+ *   a, p_a, phi0_host, pi0_host as for pycool_linear_set_background (host pointers, read before the call returns;
+ *   p_a = NaN solves (2.18));
+ *   M_device: DEVICE pointer on the current device to max_classes * (2 nf)^2 doubles, layout of pycool_linear_growth,
+ *   max_classes >= pycool_linear_num_classes(N) (PYCOOL_EINVAL otherwise, or if it is not device memory of the
+ *   current device);
+ *   stream: a cudaStream_t of the current device (NULL: the default stream).  The call is asynchronous: it
+ *   enqueues three kernels (four with p_a = NaN) and returns; the caller synchronises the stream before reading M_device.
+ * Every call on a device shares the one scratch array, which keeps the previous call's contents.  Nothing in it has
+ * to start at zero -- each call overwrites the background, the weights and the table entries it later reads -- but
+ * calls that overlap on the GPU (different streams, or several host threads) RACE on it: keep calls to one device
+ * on one stream, or order them yourself.  Calls on different devices do not interact. */
+#define PYCOOL_LINEAR_STATIC_MAX_STAGES 4096
+int pycool_linear_growth_static(int N, double L, int nfields, const pycool_params* params, int order, double dt,
+                                int nsteps, double a, double p_a, const double* phi0_host, const double* pi0_host,
+                                double* M_device, size_t max_classes, void* stream);
+/* Message of the latest failed pycool_linear_growth_static on this thread; library-owned string. */
+const char* pycool_linear_static_last_error(void);
+
 #if defined(__GNUC__)
 #pragma GCC visibility pop
 #endif

@@ -28,7 +28,8 @@ SYMBOLS = ("pycool_create", "pycool_work_bytes", "pycool_create_ext", "pycool_se
            "pycool_linear_create", "pycool_linear_num_classes", "pycool_linear_set_background",
            "pycool_linear_set_perturbations", "pycool_linear_set_modes", "pycool_linear_step", "pycool_linear_read_modes",
            "pycool_linear_read_perturbations", "pycool_linear_background_state", "pycool_linear_growth",
-           "pycool_linear_time_ms", "pycool_linear_destroy", "pycool_linear_last_error")
+           "pycool_linear_time_ms", "pycool_linear_destroy", "pycool_linear_last_error", "pycool_linear_growth_static",
+           "pycool_linear_static_last_error")
 GROWTH, NAIVE = 0, 1
 
 
@@ -134,6 +135,9 @@ def lib():
         L.pycool_linear_destroy.argtypes = [vp]
         L.pycool_linear_last_error.argtypes = [vp]
         L.pycool_linear_last_error.restype = C.c_char_p
+        L.pycool_linear_growth_static.argtypes = [ip, d, ip, pp, ip, d, ip, d, d, dp, dp, vp, C.c_size_t, vp]
+        L.pycool_linear_static_last_error.argtypes = []
+        L.pycool_linear_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -484,6 +488,24 @@ class LinearLattice:
             self.close()
         except Exception:
             pass
+
+
+LINEAR_STATIC_MAX_STAGES = 4096      # PYCOOL_LINEAR_STATIC_MAX_STAGES of include/pycool_linear.h
+
+
+def linear_growth_static(N, L, nfields, model, p, order, dt, nsteps, a, p_a, phi0, pi0, M_device, max_classes,
+                         stream=0, **kw):
+    """pycool_linear_growth_static: growth matrices of (2.51) into caller-owned device memory, no allocation on the
+    way (scratch in a fixed device array of the library).  M_device: device address (int) of max_classes x (2 nf)^2
+    doubles on the current device; stream: a cudaStream_t handle (int), 0 = the default stream.  Asynchronous."""
+    if len(phi0) != nfields or len(pi0) != nfields:
+        raise PycoolError(EINVAL, "phi0 / pi0 need one value per field")
+    mp = make_params(model, p, **kw)
+    u, v = (C.c_double * nfields)(*map(float, phi0)), (C.c_double * nfields)(*map(float, pi0))
+    st = lib().pycool_linear_growth_static(N, L, nfields, C.byref(mp), order, dt, int(nsteps), float(a), float(p_a), u, v,
+                                           C.c_void_p(int(M_device)), int(max_classes), C.c_void_p(int(stream)))
+    if st != OK:
+        raise PycoolError(st, lib().pycool_linear_static_last_error().decode())
 
 
 def from_config(cfg, device=None, **over):

@@ -9,6 +9,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -416,5 +417,192 @@ int pycool_linear_destroy(pycool_linear_ctx* c) {
 }
 
 const char* pycool_linear_last_error(const pycool_linear_ctx* c) { return c ? c->err.c_str() : g_lin_create_err.c_str(); }
+
+}  // extern "C"
+
+// =============================================================================== growth matrices, no allocation
+// pycool_linear_growth_static (include/pycool_linear.h): the growth matrices of (2.51) for callers that cannot
+// allocate.  Same kernels as step_t above -- lin_background, lin_growth -- with their scratch (background state, stage
+// weights, per-stage coefficient table) in ONE file-scope device array instead of cudaMalloc'ed memory.  Nothing in
+// this section allocates: no cudaMalloc / cudaFree, no stream, event or plan creation.
+//
+// The array's name is a host-side stand-in in host code, not a device address: the host asks for the address once per
+// device with cudaGetSymbolAddress (that device current) and passes that pointer to the kernels.  Device code
+// (lin_static_seed below) names the array directly.
+namespace {
+
+constexpr size_t kMaxStages = PYCOOL_LINEAR_STATIC_MAX_STAGES;
+constexpr size_t kStageDoubles = 2 + kLinMaxNF * kLinMaxNF;            // LinStage<4>, the widest
+
+struct StaticScratch {
+  LinBackground bg;                          // in/out of lin_background
+  double w[16];                              // stage weights
+  alignas(256) double table[kMaxStages * kStageDoubles];   // LinStage<NF>[nsteps x nstages], NF <= 4
+};
+static_assert(sizeof(LinStage<kLinMaxNF>) == kStageDoubles * sizeof(double), "stage layout");
+static_assert(sizeof(StaticScratch) == 256 + kMaxStages * kStageDoubles * sizeof(double), "the size pycool_linear.h states");
+
+// 576 KiB + 256 bytes in the device image of every GPU that loads the library.  Shared by every call: see the header.
+static __device__ __align__(256) unsigned char g_static_scratch[sizeof(StaticScratch)];
+
+struct SeedArgs {
+  LinBackground bg;
+  double w[16];
+};
+// The call's inputs into the scratch, by value through the kernel arguments (no host-to-device copy to wait for).
+__global__ void lin_static_seed(const SeedArgs s) {
+  StaticScratch* sc = reinterpret_cast<StaticScratch*>(g_static_scratch);
+  if (threadIdx.x == 0) sc->bg = s.bg;
+  if (threadIdx.x < 16) sc->w[threadIdx.x] = s.w[threadIdx.x];
+}
+
+constexpr int kMaxDevices = 64;
+std::mutex g_mu;
+StaticScratch* g_dev_scratch[kMaxDevices];   // device address of g_static_scratch on device d; nullptr = not asked yet
+
+thread_local std::string g_err = "no error";
+
+int sfail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+#define ST_TRY(expr)                                                                          \
+  do {                                                                                        \
+    cudaError_t e_ = (expr);                                                                  \
+    if (e_ != cudaSuccess) return sfail(PYCOOL_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+// Once per device, with that device current.
+int scratch_of_current_device(StaticScratch** out) {
+  int dev = -1;
+  ST_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return sfail(PYCOOL_EINVAL, "device ordinal %d is beyond the %d this entry point tracks", dev, kMaxDevices);
+  std::lock_guard<std::mutex> lock(g_mu);
+  if (!g_dev_scratch[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p) {
+      cudaGetLastError();
+      return sfail(PYCOOL_ECUDA, "cudaGetSymbolAddress(static scratch) on device %d: %s", dev, cudaGetErrorString(e));
+    }
+    g_dev_scratch[dev] = static_cast<StaticScratch*>(p);
+  }
+  *out = g_dev_scratch[dev];
+  return PYCOOL_OK;
+}
+
+template <int NF>
+int launch(StaticScratch* sc, const SeedArgs& seed, bool solve_pa, const LinConst& k, const LinStencil& st, int N,
+           unsigned nclasses, int nstages, int nsteps, double dt, double* M, cudaStream_t stream) {
+  LinStage<NF>* table = reinterpret_cast<LinStage<NF>*>(sc->table);
+  const size_t nst = (size_t)nsteps * nstages;
+  lin_static_seed<<<1, 32, 0, stream>>>(seed);
+  ST_TRY(cudaGetLastError());
+  if (solve_pa) {
+    lin_set_pa<<<1, 1, 0, stream>>>(&sc->bg, k);
+    ST_TRY(cudaGetLastError());
+  }
+  lin_background<NF><<<1, 1, 0, stream>>>(&sc->bg, k, sc->w, nstages, nsteps, dt, table);
+  ST_TRY(cudaGetLastError());
+  const unsigned long long nthreads = (unsigned long long)nclasses * 2 * NF;
+  lin_growth<NF><<<(unsigned)((nthreads + kLinThreads - 1) / kLinThreads), kLinThreads, 0, stream>>>(table, nst, st, N,
+                                                                                                     nclasses, M);
+  ST_TRY(cudaGetLastError());
+  return PYCOOL_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pycool_linear_growth_static(int N, double L, int nf, const pycool_params* p, int order, double dt, int nsteps,
+                                double a, double p_a, const double* phi0, const double* pi0, double* M_device,
+                                size_t max_classes, void* stream) {
+  // ---- the checks of pycool_linear_create and pycool_linear_set_background
+  if (!p) return sfail(PYCOOL_EINVAL, "params is NULL");
+  if (N < 3 || N > 2048 || nf < 1 || nf > kLinMaxNF) return sfail(PYCOOL_EINVAL, "N must be 3..2048, nfields 1..4");
+  if (p->precision != 0 && p->precision != 64) return sfail(PYCOOL_EINVAL, "the linearised solver is double precision only");
+  if (!(L > 0) || !std::isfinite(L)) return sfail(PYCOOL_EINVAL, "L must be finite and > 0");
+  SeedArgs seed;
+  std::memset(&seed, 0, sizeof seed);
+  const int ns = pycool_stage_weights(order, seed.w, 16);                        // (2.42)-(2.45), Table 1
+  if (ns == 0) return sfail(PYCOOL_EINVAL, "order must be 2, 4, 6 or 8");
+  if (dt == 0 || !std::isfinite(dt)) return sfail(PYCOOL_EINVAL, "dt must be finite and non-zero");
+  if (p->model < PYCOOL_FREE || p->model > PYCOOL_QBALL) return sfail(PYCOOL_EINVAL, "unknown model");
+  if ((p->model == PYCOOL_CHAOTIC || p->model == PYCOOL_QBALL) && nf != 2) return sfail(PYCOOL_EINVAL, "this model needs nfields = 2");
+  if (p->model == PYCOOL_OSCILLON && nf != 1) return sfail(PYCOOL_EINVAL, "oscillon needs nfields = 1");
+  if (!(p->mpl > 0)) return sfail(PYCOOL_EINVAL, "mpl must be > 0 (+INF = static background)");
+  if (p->model == PYCOOL_QBALL && !(p->p[2] > 0)) return sfail(PYCOOL_EINVAL, "Q-ball needs M^2 > 0");
+  const double* cs = p->stencil;
+  const bool dflt = cs[0] == 0 && cs[1] == 0 && cs[2] == 0 && cs[3] == 0;
+  if (!dflt) {
+    const double s = 6 * cs[1] + 12 * cs[2] + 8 * cs[3];
+    if (!(std::fabs(cs[0] + s) <= 1e-12 * (std::fabs(cs[0]) + std::fabs(s))))
+      return sfail(PYCOOL_EINVAL, "stencil must satisfy c0 = -(6 c1 + 12 c2 + 8 c3)");
+  }
+  if (nsteps < 1) return sfail(PYCOOL_EINVAL, "nsteps must be >= 1");
+  if ((size_t)nsteps * (size_t)ns > kMaxStages)
+    return sfail(PYCOOL_EINVAL, "%d steps x %d stages (order %d) = %zu stages exceed PYCOOL_LINEAR_STATIC_MAX_STAGES = %zu, "
+                 "the size of the static scratch: split the call or use pycool_linear_step", nsteps, ns, order,
+                 (size_t)nsteps * ns, kMaxStages);
+  if (!(a > 0) || !std::isfinite(a)) return sfail(PYCOOL_EINVAL, "a must be finite and > 0");
+  if (!phi0 || !pi0) return sfail(PYCOOL_EINVAL, "phi0 / pi0 is NULL");
+  const bool solve = std::isnan(p_a);
+  if (solve && std::isinf(p->mpl)) return sfail(PYCOOL_EINVAL, "p_a = NaN with a static background (mpl = INF)");
+  if (!solve && !std::isfinite(p_a)) return sfail(PYCOOL_EINVAL, "p_a must be finite (or NaN: solve (2.18))");
+  seed.bg.a = a; seed.bg.p_a = solve ? 0.0 : p_a;
+  for (int f = 0; f < nf; ++f) {
+    if (!std::isfinite(phi0[f]) || !std::isfinite(pi0[f])) return sfail(PYCOOL_EINVAL, "phi0 / pi0 must be finite");
+    seed.bg.phi0[f] = phi0[f]; seed.bg.pi0[f] = pi0[f];
+  }
+  const size_t nclasses = pycool_linear_num_classes(N);
+  if (!M_device || max_classes < nclasses) return sfail(PYCOOL_EINVAL, "M_device must hold %zu classes", nclasses);
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return sfail(PYCOOL_ECUDA, "no CUDA device: libpycool has no CPU path");
+  }
+  int dev = -1;
+  ST_TRY(cudaGetDevice(&dev));
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, M_device) != cudaSuccess ||
+      (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) ||
+      (at.type == cudaMemoryTypeDevice && at.device != dev)) {
+    cudaGetLastError();
+    return sfail(PYCOOL_EINVAL, "M_device is not device memory of the current device (%d)", dev);
+  }
+  StaticScratch* sc = nullptr;
+  if (int st = scratch_of_current_device(&sc)) return st;
+
+  LinConst k;
+  std::memset(&k, 0, sizeof k);
+  k.model = p->model; k.nf = nf;
+  for (int i = 0; i < 8; ++i) k.p[i] = p->p[i];
+  k.inv_mpl2 = std::isinf(p->mpl) ? 0.0 : 1.0 / (p->mpl * p->mpl);
+  k.VL = (double)((size_t)N * N * N);
+  k.den = 6.0 * k.VL * p->mpl * p->mpl;
+  k.rho_g = p->rho_gamma0; k.rho_m = p->rho_m0; k.mpl = p->mpl;
+  k.dx2 = (L / N) * (L / N);
+  if (dflt) { k.c[0] = -128.0 / 30.0; k.c[1] = 14.0 / 30.0; k.c[2] = 3.0 / 30.0; k.c[3] = 1.0 / 30.0; }   // reading G1
+  else for (int i = 0; i < 4; ++i) k.c[i] = cs[i];
+  LinStencil sten;
+  for (int i = 0; i < 4; ++i) sten.c[i] = k.c[i];
+
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  switch (nf) {
+    case 1: return launch<1>(sc, seed, solve, k, sten, N, (unsigned)nclasses, ns, nsteps, dt, M_device, s);
+    case 2: return launch<2>(sc, seed, solve, k, sten, N, (unsigned)nclasses, ns, nsteps, dt, M_device, s);
+    case 3: return launch<3>(sc, seed, solve, k, sten, N, (unsigned)nclasses, ns, nsteps, dt, M_device, s);
+    default: return launch<4>(sc, seed, solve, k, sten, N, (unsigned)nclasses, ns, nsteps, dt, M_device, s);
+  }
+}
+
+const char* pycool_linear_static_last_error(void) { return g_err.c_str(); }
 
 }  // extern "C"

@@ -86,6 +86,33 @@ def test_linear_create_validates_then_needs_a_gpu(L):
     assert L.pycool_linear_step(None, 1, 0) == binding.EINVAL and L.pycool_linear_destroy(None) == binding.EINVAL
 
 
+def test_linear_growth_static_validates_then_needs_a_gpu(L):
+    """pycool_linear_growth_static: the size limit of its fixed scratch and its arguments are checked on the host,
+    before anything touches a device."""
+    import torch
+    from paper_1201_5029_b200 import binding
+    fake = 0x1000                                                  # never dereferenced: every call below is refused
+
+    def call(N=8, nf=2, model=binding.CHAOTIC, order=4, nsteps=10, a=1.0, p_a=0.0, M=fake, room=None, **kw):
+        room = L.pycool_linear_num_classes(N) if room is None else room
+        try:
+            binding.linear_growth_static(N, 1.0, nf, model, kw.pop("p", (1.0, 100.0)), order, 0.01, nsteps, a, p_a,
+                                         (0.1,) * nf, (0.2,) * nf, M, room, **kw)
+        except binding.PycoolError as e:
+            return e.code, str(e)
+        return binding.OK, ""
+
+    for bad in (dict(N=2), dict(nf=1), dict(order=3), dict(nsteps=0), dict(a=0.0), dict(p_a=math.inf), dict(M=0),
+                dict(room=3), dict(mpl=math.inf, p_a=math.nan), dict(precision=32)):
+        assert call(**bad)[0] == binding.EINVAL, bad
+    for order, stages in ((2, 1), (4, 3), (6, 7), (8, 15)):
+        code, msg = call(order=order, nsteps=binding.LINEAR_STATIC_MAX_STAGES // stages + 1)
+        assert code == binding.EINVAL and "PYCOOL_LINEAR_STATIC_MAX_STAGES = 4096" in msg
+    if not torch.cuda.is_available():
+        assert call()[0] == binding.ECUDA                          # valid arguments, no device: no CPU path
+        assert call(order=2, nsteps=binding.LINEAR_STATIC_MAX_STAGES)[0] == binding.ECUDA   # the limit itself is allowed
+
+
 def test_stage_weights_host_logic(L, golden_dir):
     from paper_1201_5029_b200 import binding
     from helpers import weights
