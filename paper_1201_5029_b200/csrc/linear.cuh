@@ -291,6 +291,23 @@ __device__ __forceinline__ bool lin_mode_of_thread(int N, size_t& m, int& ax, in
 // complex each.  No shared memory, no shuffles: a thread-per-mode version fetching its matrix in 8 strided loads kept
 // L1 95 % busy (0.57 of the HBM roofline), one staging the matrices of a warp through shared memory stalled on the
 // shared-memory queue (0.63).  The update is in place, so the block synchronises between its reads and its writes.
+// One row of a growth matrix, 2 NF doubles, read-only path.  Even NF: rows are 32-byte aligned (the table is, and a
+// row is 32 or 64 bytes), so a row moves in 256-bit loads (LDG.E.256, sm_100): the four threads of a mode at NF = 2
+// then fetch its whole 128-byte matrix in ONE instruction -- one L1 wavefront per mode where two 16-byte loads took two.
+template <int NF>
+__device__ __forceinline__ void lin_load_row(const double2* __restrict__ row, double2 (&mm)[NF]) {
+  if constexpr (NF % 2 == 0) {
+#pragma unroll
+    for (int c = 0; c < NF; c += 2)
+      asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];"
+          : "=d"(mm[c].x), "=d"(mm[c].y), "=d"(mm[c + 1].x), "=d"(mm[c + 1].y)
+          : "l"(row + c));
+  } else {
+#pragma unroll
+    for (int c = 0; c < NF; ++c) mm[c] = __ldg(row + c);
+  }
+}
+
 template <int NF> struct LinApplyCfg {
   static constexpr int C = 2 * NF;                            // threads per mode = rows of M
   static constexpr int NT = 256;
@@ -313,13 +330,14 @@ lin_apply(double2* __restrict__ dPhi, double2* __restrict__ dPi, const double* _
     const int ax = (int)(q - iy * nxh), ay = min((int)iy, N - (int)iy), az = min(iz, N - iz);
     m = (size_t)iz * plane + q;
     const double2* mrow = reinterpret_cast<const double2*>(M) + ((size_t)lin_class_of(ax, ay, az) * C + row) * NF;
+    double2 mm[NF];                                            // M[row][0 .. 2 NF)
+    lin_load_row<NF>(mrow, mm);
 #pragma unroll
     for (int c2 = 0; c2 < NF; ++c2) {
-      const double2 mm = __ldg(mrow + c2);                     // M[row][2 c2], M[row][2 c2 + 1]
       const double2 u = __ldcs(dPhi + (size_t)c2 * nmodes + m);   // the modes stream through once: evict-first, the
       const double2 w = __ldcs(dPi + (size_t)c2 * nmodes + m);    // matrix table (47 MB at 256^3) stays in L2
-      acc.x = fma(mm.x, u.x, acc.x); acc.y = fma(mm.x, u.y, acc.y);
-      acc.x = fma(mm.y, w.x, acc.x); acc.y = fma(mm.y, w.y, acc.y);
+      acc.x = fma(mm[c2].x, u.x, acc.x); acc.y = fma(mm[c2].x, u.y, acc.y);
+      acc.x = fma(mm[c2].y, w.x, acc.x); acc.y = fma(mm[c2].y, w.y, acc.y);
     }
   }
   __syncthreads();                                             // every read of the block before its first write
