@@ -259,6 +259,8 @@ def roofline_block(lat, workload, precision, N, nf, steps, barrier):
             "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src, "traffic": None,
             "algorithmic_bytes_per_launch": alg_bytes, "launches_timed": kick_n, "avg_launch_ms": kick_avg_ms,
             "kernel_share_of_step": kick_ms / ms_prof, "geometry": geo, "capture_key": key,
+            # both denominators -- the measured copy peak above and B200's nominal 8 TB/s
+            "nominal_peak": 8000.0, "frac_of_nominal": achieved / 8000.0,
             "measured": "second pass of the same %d steps with every launch bracketed by CUDA events" % steps}
     if cnt:
         roof["bound"], roof["limiter"] = bound_from_counters(cnt)
@@ -513,6 +515,7 @@ def main():
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f%d" % a.precision, "data": "synthetic", "config": config, "clocks": clocks,
             "gpu_launches": launches, "roofline": roof}
+    line["stage_su_per_s"] = value * {2: 1, 4: 3, 6: 7, 8: 15}[order]   # stage-normalised, SU/s x stages
     en_bytes = 2.0 * esz * N ** 3 * nf
     line["energies"] = {"ms": en_ms, "achieved": en_bytes / (en_ms * 1e-3) / 1e9, "unit": "GB/s",
                         "frac": en_bytes / (en_ms * 1e-3) / 1e9 / peak,

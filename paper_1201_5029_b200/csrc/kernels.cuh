@@ -134,14 +134,14 @@ __device__ __forceinline__ double block_sum_fixed(const double* v, int n, double
 template <int T>
 __device__ __forceinline__ void block_sum_fixed3(const double* v, size_t stride, int n, double* sh /* 3 T doubles */,
                                                  double (&out)[3]) {
-  static_assert((T & (T - 1)) == 0, "tree shape: power of two");
+  static_assert((T & (T - 1)) == 0 && T >= 64, "tree shape: power of two, at least two warps");
   double a0 = 0.0, a1 = 0.0, a2 = 0.0;
   for (int i = threadIdx.x; i < n; i += T) {
     a0 += __ldcg(v + i); a1 += __ldcg(v + stride + i); a2 += __ldcg(v + 2 * stride + i);
   }
   sh[threadIdx.x] = a0; sh[T + threadIdx.x] = a1; sh[2 * T + threadIdx.x] = a2;
   __syncthreads();
-  for (int s = T / 2; s > 0; s >>= 1) {
+  for (int s = T / 2; s >= 32; s >>= 1) {                      // levels that cross warps: through shared memory
     if ((int)threadIdx.x < s) {
       sh[threadIdx.x] += sh[threadIdx.x + s];
       sh[T + threadIdx.x] += sh[T + threadIdx.x + s];
@@ -149,6 +149,17 @@ __device__ __forceinline__ void block_sum_fixed3(const double* v, size_t stride,
     }
     __syncthreads();
   }
+  if (threadIdx.x < 32) {                                      // the last five levels inside warp 0: lane i adds lane
+    a0 = sh[threadIdx.x]; a1 = sh[T + threadIdx.x]; a2 = sh[2 * T + threadIdx.x];   // i + s, the tree's own pairs
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+      a0 += __shfl_down_sync(0xffffffffu, a0, s);
+      a1 += __shfl_down_sync(0xffffffffu, a1, s);
+      a2 += __shfl_down_sync(0xffffffffu, a2, s);
+    }
+    if (threadIdx.x == 0) { sh[0] = a0; sh[T] = a1; sh[2 * T] = a2; }
+  }
+  __syncthreads();
   out[0] = sh[0]; out[1] = sh[T]; out[2] = sh[2 * T];
   __syncthreads();
 }

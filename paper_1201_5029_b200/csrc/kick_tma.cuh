@@ -109,6 +109,7 @@ struct TmaSmem {
   static constexpr size_t TOTAL = RAW + PSI + BARS + RED + 128;                // + slack to align the base
   static_assert(T::S * 8 <= BARS, "mbarriers fit");
   static_assert(3 * T::NT * sizeof(double) <= RAW + PSI, "the stage tail's three trees fit in the idle ring + psi");
+  static constexpr bool kTreesFitPsi = 3 * T::NT * sizeof(double) <= PSI;   // kick_tma_coop: ring busy with the next stage
 };
 
 template <typename Real>
@@ -480,16 +481,18 @@ kick_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ CUt
 // one block per item, and between stages a grid-wide barrier instead of a kernel boundary -- the blocks stay
 // resident, keep their shared-memory carve-up, barriers and per-thread tables, and a stage costs no launch
 // hand-over (the paper returns to the CPU at every sub-step).  The barrier is the stage tail itself:
-// every block publishes its partial sums and takes a ticket; the block that draws the last ticket adds the partials
-// in item order, advances the scalars (scalar_advance, as stage_finish does) and releases the others, which wait on a
-// counter in global memory.  Same items, same partial-sum indices, same order of the final sum as the launch-per-
-// stage path: results are bitwise identical (tested).  Needs cudaLaunchCooperativeKernel (co-residency).
+// every block publishes its partial sums and arrives on a counter in global memory; once all have, EVERY block adds
+// the partials in item order and advances its own copy of the scalars (scalar_advance, as stage_finish does) -- the
+// same operations on the same numbers everywhere, hence the same bits, and no second round trip through one "last"
+// block -- while its first loads of the next stage are already in flight.  Same items, same partial-sum indices, same
+// order of the final sum as the launch-per-stage path: results are bitwise identical (tested).  Needs
+// cudaLaunchCooperativeKernel (co-residency).
 template <typename Real>
 struct CoopArgs {
   Real* phi[2];          // the two state buffers; stage k reads buffer (cur0 + k) & 1 and writes the other
   Real* pi[2];
   int cur0;
-  unsigned int* release; // stages completed in this launch (zero at launch)
+  unsigned int* release; // arrivals at the stage barriers of this launch, all blocks (zero at launch)
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -515,7 +518,9 @@ kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant
   Real* psi = reinterpret_cast<Real*>(base + SM::RAW);
   const uint32_t bars = smem_addr(base + SM::RAW + SM::PSI);
   double* red = reinterpret_cast<double*>(base + SM::RAW + SM::PSI + SM::BARS);
-  __shared__ int is_last;
+  static_assert(SM::kTreesFitPsi, "the stage tail's trees live in the psi planes while the ring refills");
+  __shared__ Scalars sc_sh;                                    // this block's copy of the scalars (thread 0 advances it)
+  __shared__ Real coef_sh[3];                                  // c_drift, kD, kV of the coming stage, in Real
 
   const Layout& L = g.L;
   const int N = L.N;
@@ -529,6 +534,12 @@ kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant
   if (tid == 0) {
     for (int s = 0; s < S; ++s) mbar_init(bars + 8u * s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    // the scalars the previous launch left: through L2 (this SM's L1 may hold an older copy)
+    const double* src = reinterpret_cast<const double*>(g.sc);
+    double* dst = reinterpret_cast<double*>(&sc_sh);
+    static_assert(sizeof(Scalars) % sizeof(double) == 0, "Scalars is copied as doubles");
+    for (int q = 0; q < (int)(sizeof(Scalars) / sizeof(double)); ++q) dst[q] = __ldcg(src + q);
+    coef_sh[0] = Real(sc_sh.c_drift); coef_sh[1] = Real(sc_sh.kD); coef_sh[2] = Real(sc_sh.kV);
   }
   const Real c1 = Real(g.c1), c2 = Real(g.c2), c3 = Real(g.c3);
   const Real c0 = -(Real(6) * c1 + Real(12) * c2 + Real(8) * c3);
@@ -541,34 +552,40 @@ kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant
   uint32_t phase = 0;
   __syncthreads();                                             // barriers initialised before anyone waits
 
-#pragma unroll 1
-  for (int k = 0; k < sch.nstages; ++k) {
-    const int cur = (ca.cur0 + k) & 1;
-    const CUtensorMap* tphi = cur ? &tm_phi1 : &tm_phi0;
-    const CUtensorMap* tpi = cur ? &tm_pi1 : &tm_pi0;
-    // the loads of this stage: planes z0-1 .. z0+nz of the block's item, S in flight
-    int pr_i = 0;
-    const int pr_nload = nz + 2;
-    auto issue_next = [&](int s) {
-      if (pr_i >= pr_nload) return;
-      if (tid == 0) {
-        const uint32_t bar = bars + 8u * s;
-        const uint32_t dst = smem_addr(raw + (size_t)s * 2 * SM::BOXA);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_expect_tx(bar, (uint32_t)(2 * SM::BOX));
-        int gz = z0 + pr_i - 1;
-        gz = gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
-        tma_load_4d(dst, tphi, bar, x0, y0, gz, 0);
-        tma_load_4d(dst + (uint32_t)SM::BOXA, tpi, bar, x0, y0, gz, 0);
-      }
-      ++pr_i;
-    };
-    for (int s = 0; s < S; ++s) {                              // ring slots in consumption order from `slot`
+  // the loads of a stage: planes z0-1 .. z0+nz of the block's item, S in flight
+  const CUtensorMap* tphi = nullptr;
+  const CUtensorMap* tpi = nullptr;
+  int pr_i = 0;
+  const int pr_nload = nz + 2;
+  auto issue_next = [&](int s) {
+    if (pr_i >= pr_nload) return;
+    if (tid == 0) {
+      const uint32_t bar = bars + 8u * s;
+      const uint32_t dst = smem_addr(raw + (size_t)s * 2 * SM::BOXA);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(bar, (uint32_t)(2 * SM::BOX));
+      int gz = z0 + pr_i - 1;
+      gz = gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+      tma_load_4d(dst, tphi, bar, x0, y0, gz, 0);
+      tma_load_4d(dst + (uint32_t)SM::BOXA, tpi, bar, x0, y0, gz, 0);
+    }
+    ++pr_i;
+  };
+  auto start_loads = [&](int cur) {                            // first S loads of a stage, ring slots in consumption
+    tphi = cur ? &tm_phi1 : &tm_phi0;                          // order from `slot`
+    tpi = cur ? &tm_pi1 : &tm_pi0;
+    pr_i = 0;
+    for (int s = 0; s < S; ++s) {
       int sl = slot + s; if (sl >= S) sl -= S;
       issue_next(sl);
     }
-    // the scalars the previous stage's tail left (other blocks wrote them: read through L2)
-    const Real cd = Real(__ldcg(&g.sc->c_drift)), kD = Real(__ldcg(&g.sc->kD)), kV = Real(__ldcg(&g.sc->kV));
+  };
+  start_loads(ca.cur0 & 1);
+
+#pragma unroll 1
+  for (int k = 0; k < sch.nstages; ++k) {
+    const int cur = (ca.cur0 + k) & 1;
+    const Real cd = coef_sh[0], kD = coef_sh[1], kV = coef_sh[2];
 
     double sD = 0.0, sV = 0.0, sP = 0.0;
     Real* po = ca.phi[cur ^ 1];
@@ -582,46 +599,41 @@ kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant
     double v[3] = {sD, sV, sP};
     block_reduce<3, NT>(v, red);
 
-    // ---- stage tail = grid barrier.  Thread 0 publishes, then takes a ticket (release: every store of this block,
-    // fields included, is ordered before it by the block barrier + fence).
-    __syncthreads();
-    if (tid == 0) {
-      publish_partials(g.partials, (unsigned)g.nitems, (unsigned)item, v);
+    // ---- stage tail = grid barrier.  Thread 0 publishes the block's partial sums (two sets of slots, by stage parity:
+    // a block a stage ahead must not overwrite what a slower one still reads) and arrives (release: every store of this
+    // block, fields included, is ordered before it by the block barrier + fence), then waits until every block has.
+    // EVERY block then adds the partials in item order and advances its own copy of the scalars -- the same operations
+    // on the same numbers in every block, so the same bits, with no second round trip through a "last" block; the next
+    // stage's first loads go out before that, so their latency hides the reduction and the scalar update.
+    const bool last_stage = k + 1 == sch.nstages;
+    const double* part = g.partials + (size_t)(k & 1) * 3 * (size_t)g.nitems;
+    if (tid == 0) {                                            // (the barrier inside block_reduce follows every thread's
+      publish_partials(const_cast<double*>(part), (unsigned)g.nitems, (unsigned)item, v);   // last field store)
       __threadfence();
-      is_last = atomicAdd(g.tail.ticket, 1u) == (unsigned)(k + 1) * gridDim.x - 1u;
-    }
-    __syncthreads();
-    if (is_last) {                                             // every block has published: reduce, advance, release
-      __threadfence();
-      double* sh = reinterpret_cast<double*>(raw);             // ring idle (every load consumed), psi behind it
-      double S3[3];
-      block_sum_fixed3<NT>(g.partials, (size_t)g.nitems, g.nitems, sh, S3);
-      const double SD = S3[0], SV = S3[1], SP = S3[2];
-      if (tid == 0) {
-        const int i = sch.first + k;                           // stage index within the call
-        StageLen len;
-        len.dt = sch.dt; len.adaptive = sch.adaptive;
-        len.w = sch.w[i % sch.ns];
-        len.w_next = (k + 1 < sch.nstages || !sch.call_ends) ? sch.w[(i + 1) % sch.ns] : 0.0;
-        len.ends_step = (i % sch.ns) == sch.ns - 1;
-        Scalars s;                                             // through L2: another block wrote them last stage, and
-        {                                                      // this SM's L1 may still hold an older copy
-          const double* src = reinterpret_cast<const double*>(g.sc);
-          double* dst = reinterpret_cast<double*>(&s);
-          static_assert(sizeof(Scalars) % sizeof(double) == 0, "Scalars is copied as doubles");
-#pragma unroll
-          for (int q = 0; q < (int)(sizeof(Scalars) / sizeof(double)); ++q) dst[q] = __ldcg(src + q);
-        }
-        scalar_advance(s, g.tail.k, len, 1, SD, SV, SP);
-        *g.tail.sc = s;
-        if (k + 1 == sch.nstages) *g.tail.ticket = 0u;         // counters ready for the next launch
-        __threadfence();
-        st_release_u32(ca.release, (unsigned)(k + 1));
+      atomicAdd(ca.release, 1u);
+      if (!last_stage || blockIdx.x == 0) {
+        const unsigned target = (unsigned)(k + 1) * gridDim.x;
+        while (ld_acquire_u32(ca.release) < target) { }
+        asm volatile("fence.proxy.async;" ::: "memory");       // other blocks' stores before this block's TMA loads
       }
     }
+    if (last_stage && blockIdx.x != 0) break;                  // block 0 leaves the final scalars; the others are done
+    __syncthreads();
+    if (!last_stage) start_loads(cur ^ 1);
+    double S3[3];
+    block_sum_fixed3<NT>(part, (size_t)g.nitems, g.nitems, reinterpret_cast<double*>(psi), S3);   // psi planes: idle
     if (tid == 0) {
-      while (ld_acquire_u32(ca.release) < (unsigned)(k + 1)) __nanosleep(20);
-      asm volatile("fence.proxy.async;" ::: "memory");         // other blocks' stores before this block's TMA loads
+      const int i = sch.first + k;                             // stage index within the call
+      StageLen len;
+      len.dt = sch.dt; len.adaptive = sch.adaptive;
+      len.w = sch.w[i % sch.ns];
+      len.w_next = (!last_stage || !sch.call_ends) ? sch.w[(i + 1) % sch.ns] : 0.0;
+      len.ends_step = (i % sch.ns) == sch.ns - 1;
+      Scalars s = sc_sh;
+      scalar_advance(s, g.tail.k, len, 1, S3[0], S3[1], S3[2]);
+      sc_sh = s;
+      coef_sh[0] = Real(s.c_drift); coef_sh[1] = Real(s.kD); coef_sh[2] = Real(s.kV);
+      if (last_stage) *g.tail.sc = s;                          // block 0 only gets here
     }
     __syncthreads();
   }

@@ -834,7 +834,8 @@ int pycool_step(pycool_ctx* c, int nsteps) {
   // between stages instead of a kernel boundary (kick_tma.cuh: kick_tma_coop); same results bit for bit.
   const long long nitems = (long long)c->grid.x * c->grid.y * c->grid.z;
   bool coop = c->cooperative && c->fused_tail && !c->profiling && kTiles[c->tile].stages > 0 &&
-                    dispatch(c, OP_COOP_RESIDENT, c->tile) >= nitems;
+                    dispatch(c, OP_COOP_RESIDENT, c->tile) >= nitems &&
+                    6 * nitems <= (long long)c->partials_cap;   // two sets of partial sums, by stage parity
   for (long long i = 0; i < S;) {
     if (coop) {
       // up to the end of the call, the next energy-log point, or 32 steps, whichever comes first
