@@ -200,7 +200,7 @@ __device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k,
     s.SD = SD; s.SV = SV; s.Spi2 = SP;
     if (!(isfinite(SD) && isfinite(SV) && isfinite(SP))) s.nonfinite = 1;
     flow_H3_pa(s, k, h);                       // H3(h), scalar part
-    const double e = __ddiv_rn(h, 2.0);
+    const double e = __dmul_rn(h, 0.5);          // = h / 2 exactly (a power of two, h far from the subnormals): no division
     flow_H2_pa(s, k, e);                       // H2(h/2), scalar part (pi is constant in H2: post-kick sum)
     c1 = drift_coef(s, e);                     //          field part, applied by the next kernel
     flow_H1(s, k, e);                          // H1(h/2)
@@ -216,7 +216,7 @@ __device__ __forceinline__ void scalar_advance(Scalars& s, const ScalarConst& k,
       s.dt_cur = next_len;
     }
     const double h_next = __dmul_rn(len.w_next, next_len);
-    const double e = __ddiv_rn(h_next, 2.0);
+    const double e = __dmul_rn(h_next, 0.5);
     flow_H1(s, k, e);                          // H1(h_next/2)
     flow_H2_pa(s, k, e);                       // H2(h_next/2), scalar part
     s.c_drift = __dadd_rn(c1, drift_coef(s, e));

@@ -571,15 +571,31 @@ kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant
     }
     ++pr_i;
   };
-  auto start_loads = [&](int cur) {                            // first S loads of a stage, ring slots in consumption
-    tphi = cur ? &tm_phi1 : &tm_phi0;                          // order from `slot`
+  // First loads of a stage (up to S, ring slots in consumption order from `slot`): thread 0 issues them -- one proxy
+  // fence for all -- as soon as IT may (the ring is idle: every thread is past the march's last barrier), the others
+  // only keep the books.
+  auto start_loads = [&](int cur) {
+    tphi = cur ? &tm_phi1 : &tm_phi0;
     tpi = cur ? &tm_pi1 : &tm_pi0;
-    pr_i = 0;
-    for (int s = 0; s < S; ++s) {
-      int sl = slot + s; if (sl >= S) sl -= S;
-      issue_next(sl);
+    pr_i = pr_nload < S ? pr_nload : S;
+  };
+  auto issue_first = [&](int cur) {                            // thread 0 only
+    const CUtensorMap* tp = cur ? &tm_phi1 : &tm_phi0;
+    const CUtensorMap* tq = cur ? &tm_pi1 : &tm_pi0;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    const int n = pr_nload < S ? pr_nload : S;
+    for (int i = 0; i < n; ++i) {
+      int sl = slot + i; if (sl >= S) sl -= S;
+      const uint32_t bar = bars + 8u * sl;
+      const uint32_t dst = smem_addr(raw + (size_t)sl * 2 * SM::BOXA);
+      mbar_expect_tx(bar, (uint32_t)(2 * SM::BOX));
+      int gz = z0 + i - 1;
+      gz = gz < 0 ? gz + N : (gz >= N ? gz - N : gz);
+      tma_load_4d(dst, tp, bar, x0, y0, gz, 0);
+      tma_load_4d(dst + (uint32_t)SM::BOXA, tq, bar, x0, y0, gz, 0);
     }
   };
+  if (tid == 0) issue_first(ca.cur0 & 1);
   start_loads(ca.cur0 & 1);
 
 #pragma unroll 1
@@ -615,7 +631,8 @@ kick_tma_coop(const __grid_constant__ CUtensorMap tm_phi0, const __grid_constant
         const unsigned target = (unsigned)(k + 1) * gridDim.x;
         while (ld_acquire_u32(ca.release) < target) { }
         asm volatile("fence.proxy.async;" ::: "memory");       // other blocks' stores before this block's TMA loads
-      }
+        if (!last_stage) issue_first(cur ^ 1);                 // at once: their latency hides the block barrier below,
+      }                                                        // the reduction and the scalar update
     }
     if (last_stage && blockIdx.x != 0) break;                  // block 0 leaves the final scalars; the others are done
     __syncthreads();
