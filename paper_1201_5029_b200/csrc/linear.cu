@@ -3,7 +3,7 @@
 // One pycool_linear_step(n, GROWTH) call enqueues, on the context's stream and without a host synchronisation:
 //     lin_background   (1 thread)   background through n x stages(order) stages + the per-stage coefficient table
 //     lin_growth       (thread per class x column)   growth matrices M(n dt, k_eff^2) of (2.51)
-//     lin_apply        (thread per mode x row of M)   every Fourier mode multiplied by its class's matrix
+//     lin_apply        (thread per mode x pair of rows of M)   every Fourier mode multiplied by its class's matrix
 // and with NAIVE: lin_background, then lin_naive (thread per mode through every stage).  Kernels: linear.cuh.
 #include <cmath>
 #include <cstdarg>
@@ -108,9 +108,9 @@ int step_t(pycool_linear_ctx* c, int nsteps, int method) {
         table, nst, c->sc, c->N, c->nclasses, c->M);
     LIN_TRY(c, cudaGetLastError());
     LIN_TRY(c, cudaEventRecord(c->ev[2], c->stream));
-    constexpr int kApplyModes = LinApplyCfg<NF>::MPB;
-    lin_apply<NF><<<dim3((unsigned)((plane + kApplyModes - 1) / kApplyModes), (unsigned)c->N), LinApplyCfg<NF>::NT, 0,
-                    c->stream>>>(c->dPhi, c->dPi, c->M, c->N, c->nmodes);
+    using Apply = LinApplyCfg<NF, kLinApplyRows>;
+    lin_apply<NF, kLinApplyRows><<<dim3((unsigned)((plane + Apply::MPB - 1) / Apply::MPB), (unsigned)c->N), Apply::NT, 0,
+                                   c->stream>>>(c->dPhi, c->dPi, c->M, c->N, c->nmodes);
     LIN_TRY(c, cudaGetLastError());
     c->have_growth = true;
   } else {

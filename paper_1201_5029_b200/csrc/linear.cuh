@@ -285,12 +285,18 @@ __device__ __forceinline__ bool lin_mode_of_thread(int N, size_t& m, int& ax, in
 }
 
 // mode <- M(class of the mode) mode   (2.51).  dPhi, dPi: [NF][nmodes] complex.
-// The matrices are a gather: neighbouring modes belong to different classes.  One thread per (mode, row of M): the
-// 2 NF threads of a mode read the 2 NF rows of its matrix -- together one contiguous (2 NF)^2 x 8 bytes, a whole line
-// at NF = 2 -- and each the mode's 2 NF complex values (the same addresses within the group: broadcast), and write one
-// complex each.  No shared memory, no shuffles: a thread-per-mode version fetching its matrix in 8 strided loads kept
-// L1 95 % busy (0.57 of the HBM roofline), one staging the matrices of a warp through shared memory stalled on the
-// shared-memory queue (0.63).  The update is in place, so the block synchronises between its reads and its writes.
+// The matrices are a gather: neighbouring modes belong to different classes.  One thread per (mode, R rows of M),
+// R = kLinApplyRows = 2: the NF threads of a mode read the 2 NF rows of its matrix -- together one contiguous
+// (2 NF)^2 x 8 bytes, a whole line at NF = 2, in 256-bit loads -- and each the mode's 2 NF complex values (the same
+// addresses within the group: broadcast), and write the field's (dPhi, dPi) pair.  No shared memory, no shuffles.
+// The kernel is bound by L1 wavefronts, not by bytes in flight: a 16-byte load costs a wavefront per quarter warp
+// however many of its threads share an address, so what counts is how many modes a quarter warp covers -- R = 1 (a
+// thread per row; two 16-byte loads per row) ran at 0.66 of the HBM roofline at 256^3, with 256-bit row loads 0.75,
+// R = 2 0.86, R = 2 NF (a thread per mode, its matrix in strided loads) 0.80; earlier forms: thread per mode with
+// 16-byte matrix loads 0.57 (L1 95 % busy), matrices staged through shared memory 0.63, several modes per thread
+// 0.52-0.56.  The update is in place, so the block synchronises between its reads and its writes.
+constexpr int kLinApplyRows = 2;
+
 // One row of a growth matrix, 2 NF doubles, read-only path.  Even NF: rows are 32-byte aligned (the table is, and a
 // row is 32 or 64 bytes), so a row moves in 256-bit loads (LDG.E.256, sm_100): the four threads of a mode at NF = 2
 // then fetch its whole 128-byte matrix in ONE instruction -- one L1 wavefront per mode where two 16-byte loads took two.
@@ -308,40 +314,54 @@ __device__ __forceinline__ void lin_load_row(const double2* __restrict__ row, do
   }
 }
 
-template <int NF> struct LinApplyCfg {
-  static constexpr int C = 2 * NF;                            // threads per mode = rows of M
+template <int NF, int R> struct LinApplyCfg {
+  static constexpr int C = 2 * NF;                            // rows of M
+  static_assert(C % R == 0, "rows per thread divide the rows of M");
+  static constexpr int TPM = C / R;                           // threads per mode
   static constexpr int NT = 256;
-  static constexpr int MPB = NT / C;                          // modes per block (NF = 3: 42, four threads idle)
+  static constexpr int MPB = NT / TPM;                        // modes per block (NF = 3, R = 2: 85, one thread idle)
 };
-template <int NF>
-__global__ void __launch_bounds__(LinApplyCfg<NF>::NT)
+template <int NF, int R>
+__global__ void __launch_bounds__(LinApplyCfg<NF, R>::NT)
 lin_apply(double2* __restrict__ dPhi, double2* __restrict__ dPi, const double* __restrict__ M, int N, size_t nmodes) {
-  using K = LinApplyCfg<NF>;
-  constexpr int C = K::C;
+  using K = LinApplyCfg<NF, R>;
+  constexpr int C = K::C, TPM = K::TPM;
   const unsigned nxh = (unsigned)N / 2 + 1, plane = (unsigned)N * nxh;
-  const unsigned ml = threadIdx.x / C, row = threadIdx.x - ml * C;
+  const unsigned ml = threadIdx.x / TPM, rp = threadIdx.x - ml * TPM;   // mode of the block, row group of the mode
   const unsigned q = blockIdx.x * K::MPB + ml;                // mode within the i_z plane: iy (N/2 + 1) + ix
   const int iz = (int)blockIdx.y;
   const bool live = ml < (unsigned)K::MPB && q < plane;
-  double2 acc = {0.0, 0.0};
+  double2 acc[R];
+#pragma unroll
+  for (int r = 0; r < R; ++r) acc[r] = double2{0.0, 0.0};
   size_t m = 0;
   if (live) {
     const unsigned iy = q / nxh;
     const int ax = (int)(q - iy * nxh), ay = min((int)iy, N - (int)iy), az = min(iz, N - iz);
     m = (size_t)iz * plane + q;
-    const double2* mrow = reinterpret_cast<const double2*>(M) + ((size_t)lin_class_of(ax, ay, az) * C + row) * NF;
-    double2 mm[NF];                                            // M[row][0 .. 2 NF)
-    lin_load_row<NF>(mrow, mm);
+    const double2* mrow = reinterpret_cast<const double2*>(M) + ((size_t)lin_class_of(ax, ay, az) * C + rp * R) * NF;
+    double2 mm[R][NF];                                         // rows rp R .. rp R + R - 1 of M: R x 2 NF doubles, contiguous
+#pragma unroll
+    for (int r = 0; r < R; ++r) lin_load_row<NF>(mrow + r * NF, mm[r]);
 #pragma unroll
     for (int c2 = 0; c2 < NF; ++c2) {
       const double2 u = __ldcs(dPhi + (size_t)c2 * nmodes + m);   // the modes stream through once: evict-first, the
       const double2 w = __ldcs(dPi + (size_t)c2 * nmodes + m);    // matrix table (47 MB at 256^3) stays in L2
-      acc.x = fma(mm[c2].x, u.x, acc.x); acc.y = fma(mm[c2].x, u.y, acc.y);
-      acc.x = fma(mm[c2].y, w.x, acc.x); acc.y = fma(mm[c2].y, w.y, acc.y);
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        acc[r].x = fma(mm[r][c2].x, u.x, acc[r].x); acc[r].y = fma(mm[r][c2].x, u.y, acc[r].y);
+        acc[r].x = fma(mm[r][c2].y, w.x, acc[r].x); acc[r].y = fma(mm[r][c2].y, w.y, acc[r].y);
+      }
     }
   }
   __syncthreads();                                             // every read of the block before its first write
-  if (live) __stcs(((row & 1) ? dPi : dPhi) + (size_t)(row >> 1) * nmodes + m, acc);
+  if (live) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const unsigned row = rp * R + r;
+      __stcs(((row & 1) ? dPi : dPhi) + (size_t)(row >> 1) * nmodes + m, acc[r]);
+    }
+  }
 }
 
 // Every mode through every stage on its own ("naive version").  Real coefficients: the real and
