@@ -90,20 +90,22 @@ def test_two_calls_in_a_row_match_the_existing_path(pc):
 
 
 def test_a_call_allocates_nothing(pc):
-    """Device memory in use is the same before and after (the first call of a process may load the kernels' module;
-    that is why one call comes first)."""
+    """Free device memory does not drop across calls (the first call of a process may load the kernels' module; that
+    is why one call comes first)."""
+    import gc
     import torch
     torch.cuda.set_device(0)
     c = CASES["chaotic"]
     out = new_out(pc, c)
     static_call(pc, c, out)
     torch.cuda.synchronize()
+    gc.collect()
     free0, _ = torch.cuda.mem_get_info(0)
     for _ in range(3):
         static_call(pc, c, out)
     torch.cuda.synchronize()
     free1, _ = torch.cuda.mem_get_info(0)
-    assert free1 == free0
+    assert free1 >= free0        # nothing taken (objects of earlier tests may be collected, and freed, at any time)
 
 
 def test_limits_and_arguments(pc):
