@@ -59,6 +59,9 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
   const int N = L.N;
   const int tid = threadIdx.x;
   const int tx2 = tid % (TX / 2), tyj = tid / (TX / 2);
+  constexpr int NB_RUN = 128 / (2 * (int)sizeof(Real));        // neighbour loads, every other run of threads swapped:
+  const bool nb_swap = ((tx2 / NB_RUN) & 1) != 0;              // no bank conflict (kick_tma.cuh: march_item)
+  const int nb_first = nb_swap ? 2 : -1, nb_second = nb_swap ? -1 : 2;
   const int item = blockIdx.x, nbxy = g.nbx * g.nby;
   const int bz = item / nbxy, r_ = item - bz * nbxy, by = r_ / g.nbx;
   const int x0 = (r_ - by * g.nbx) * TX, y0 = by * TY, z0 = bz * g.zc;
@@ -164,10 +167,10 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
       double Rx[J + 2], Cx[J + 2], Ry[J + 2], Cy[J + 2];       // psi: side sums and centres of x-outputs 0, 1
 #pragma unroll
       for (int r = 0; r < J + 2; ++r) {
-        const double l = (double)sp[r * PX - 1];
+        const Real n0 = sp[r * PX + nb_first], n1 = sp[r * PX + nb_second];   // bank-conflict-free order: kick_tma.cuh
         const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
         const double mx = (double)m.x, my = (double)m.y;
-        const double rr = (double)sp[r * PX + 2];
+        const double l = (double)(nb_swap ? n1 : n0), rr = (double)(nb_swap ? n0 : n1);
         Rx[r] = l + my; Cx[r] = mx; Ry[r] = mx + rr; Cy[r] = my;
       }
 #pragma unroll

@@ -222,6 +222,14 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, Real* phi_out
     else if (valid[j]) store_edge(plane, j, v);
   };
 
+  // The stencil's single-element loads of the x-neighbours (x = -1 and x = XW of the thread's group) run at the group
+  // stride, XW elements: threads 128 / (XW sizeof(Real)) apart hit the same banks, a 2-way conflict that costs the load
+  // as many shared-memory wavefronts as the full-width load of the group itself.  Every other such run of threads takes
+  // the RIGHT neighbour first and the left one second: the two halves then fall on disjoint banks in both loads.
+  constexpr int NB_RUN = 128 / (XW * (int)sizeof(Real));
+  const bool nb_swap = ((txw / NB_RUN) & 1) != 0;
+  const int nb_first = nb_swap ? XW : -1, nb_second = nb_swap ? -1 : XW;
+
   RV qa_phi[NF][J], qa_pi[NF][J], qb_phi[NF][J], qb_pi[NF][J];  // phi', pi of planes p and p-1 (roles swap)
   RV A[NF][J], B[NF][J];                                     // stencil accumulators
   Real ref[NF];                                              // item-uniform; D annihilates constants
@@ -295,11 +303,12 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, Real* phi_out
 #pragma unroll
       for (int r = 0; r < J + 2; ++r) {
         Real e[XW + 2];                                      // x = -1 .. XW of this row
-        e[0] = sp[r * PX - 1];
+        const Real n0 = sp[r * PX + nb_first], n1 = sp[r * PX + nb_second];   // the two neighbours, see nb_swap
         const RV m = *reinterpret_cast<const RV*>(sp + r * PX);
 #pragma unroll
         for (int k = 0; k < XW; ++k) e[k + 1] = m.v[k];
-        e[XW + 1] = sp[r * PX + XW];
+        e[0] = nb_swap ? n1 : n0;
+        e[XW + 1] = nb_swap ? n0 : n1;
 #pragma unroll
         for (int k = 0; k < XW; ++k) { Sd[r][k] = e[k] + e[k + 2]; Ce[r][k] = e[k + 1]; }
       }
