@@ -168,8 +168,13 @@ energy_tma(const __grid_constant__ CUtensorMap tm_phi, const __grid_constant__ C
 #pragma unroll
       for (int r = 0; r < J + 2; ++r) {
         const Real n0 = sp[r * PX + nb_first], n1 = sp[r * PX + nb_second];   // bank-conflict-free order: kick_tma.cuh
-        const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
-        const double mx = (double)m.x, my = (double)m.y;
+        double mx, my;
+        if (r >= 1 && r <= J) {                                // an own row: what this thread stored, from its registers
+          mx = (double)(Real(cphi[f][r - 1].x) - ref[f]); my = (double)(Real(cphi[f][r - 1].y) - ref[f]);
+        } else {
+          const R2 m = *reinterpret_cast<const R2*>(sp + r * PX);
+          mx = (double)m.x; my = (double)m.y;
+        }
         const double l = (double)(nb_swap ? n1 : n0), rr = (double)(nb_swap ? n0 : n1);
         Rx[r] = l + my; Cx[r] = mx; Ry[r] = mx + rr; Cy[r] = my;
       }

@@ -304,9 +304,14 @@ __device__ __forceinline__ void march_item(const TmaArgs<Real>& g, Real* phi_out
       for (int r = 0; r < J + 2; ++r) {
         Real e[XW + 2];                                      // x = -1 .. XW of this row
         const Real n0 = sp[r * PX + nb_first], n1 = sp[r * PX + nb_second];   // the two neighbours, see nb_swap
-        const RV m = *reinterpret_cast<const RV*>(sp + r * PX);
+        if (J >= 2 && r >= 1 && r <= J) {                    // an own row: its psi is phi' - ref of this thread's own
+#pragma unroll                                               // registers, the very operation the drift stored -- no load
+          for (int k = 0; k < XW; ++k) e[k + 1] = cphi[f][r - 1].v[k] - ref[f];   // (one-row variants: no gain measured,
+        } else {                                             // and their 128-register budget is full)
+          const RV m = *reinterpret_cast<const RV*>(sp + r * PX);
 #pragma unroll
-        for (int k = 0; k < XW; ++k) e[k + 1] = m.v[k];
+          for (int k = 0; k < XW; ++k) e[k + 1] = m.v[k];
+        }
         e[0] = nb_swap ? n1 : n0;
         e[XW + 1] = nb_swap ? n0 : n1;
 #pragma unroll
